@@ -1,0 +1,198 @@
+"""oracle/ -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Plain CPU oracle of the THOR HE-VI large step (arXiv 1607.05535), written from PAPER.md with the
+readings of SURVEY.md 8(c) / DESIGN.md.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It never imports
+paper_1607_05535_b200 and shares no code with it.
+
+This file is argument marshalling only (ctypes around oracle/thor_oracle.c); grid_oracle.py is the
+independent numpy grid generator.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "thor_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+# -ffp-contract=off: no FMA contraction, so the oracle's rounding is the plain IEEE one
+_CFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c99"]
+
+_lib = None
+
+
+def build(force=False):
+    """Compile thor_oracle.c with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc"] + _CFLAGS + [_SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_D = ctypes.POINTER(ctypes.c_double)
+_I = ctypes.POINTER(ctypes.c_int)
+
+
+class _Planet(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in ("radius", "omega", "gravity", "Rd", "Cp", "p_ref", "z_top")]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        L.orc_geom_build.restype = ctypes.c_void_p
+        L.orc_geom_build.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Planet), _D, _I, _D]
+        L.orc_geom_free.argtypes = [ctypes.c_void_p]
+        for name in ("Ac", "len", "nrm", "C", "bary"):
+            f = getattr(L, "orc_geom_" + name)
+            f.restype = _D
+            f.argtypes = [ctypes.c_void_p]
+        L.orc_geom_deg.restype = _I
+        L.orc_geom_deg.argtypes = [ctypes.c_void_p]
+        L.orc_hdiv.argtypes = [ctypes.c_void_p, _D, _D]
+        L.orc_hgrad.argtypes = [ctypes.c_void_p, _D, _D]
+        L.orc_thomas.argtypes = [ctypes.c_int, _D, _D, _D, _D, _D]
+        L.orc_centroid_eq13.argtypes = [_D, ctypes.c_int, _D]
+        L.orc_step.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D]
+        L.orc_diagnostics.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, _D, _D]
+        L.orc_tridiag_coefficients.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D, _D]
+        L.orc_slow_terms.argtypes = [ctypes.c_void_p] + [_D] * 12
+        L.orc_substep.argtypes = [ctypes.c_void_p, ctypes.c_double] + [_D] * 14
+        L.orc_num_threads.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(_D)
+
+
+def _c(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads():
+    return int(_load().orc_num_threads())
+
+
+class Geometry:
+    """All geometric coefficients recomputed from the grid description (O2): positions xyz [N][3],
+    neighbour lists nbr [N][6] and control-volume vertices C [N][6][3] (None: triangle centroids
+    of xyz)."""
+
+    def __init__(self, xyz, nbr, nv, planet, C=None):
+        L = _load()
+        self.xyz = _c(xyz)
+        self.nbr = np.ascontiguousarray(nbr, dtype=np.int32)
+        self.N = int(self.xyz.shape[0])
+        self.nv = int(nv)
+        self.planet = dict(planet)
+        self._P = _Planet(**{k: float(planet[k]) for k in ("radius", "omega", "gravity", "Rd", "Cp", "p_ref", "z_top")})
+        Cin = None if C is None else _c(C)
+        assert Cin is None or Cin.shape == (self.N, 6, 3)
+        self._h = L.orc_geom_build(self.N, self.nv, ctypes.byref(self._P), _p(self.xyz),
+                                   self.nbr.ctypes.data_as(_I), _p(Cin))
+        N = self.N
+        self.Ac = np.ctypeslib.as_array(L.orc_geom_Ac(self._h), (N,)).copy()
+        self.len = np.ctypeslib.as_array(L.orc_geom_len(self._h), (N, 6)).copy()
+        self.nrm = np.ctypeslib.as_array(L.orc_geom_nrm(self._h), (N, 6, 3)).copy()
+        self.C = np.ctypeslib.as_array(L.orc_geom_C(self._h), (N, 6, 3)).copy()
+        self.bary = np.ctypeslib.as_array(L.orc_geom_bary(self._h), (N, 6, 3)).copy()
+        self.deg = np.ctypeslib.as_array(L.orc_geom_deg(self._h), (N,)).copy()
+        self.dz = planet["z_top"] / nv
+        self.z_c = (np.arange(nv) + 0.5) * self.dz
+        self.r_c = planet["radius"] + self.z_c
+        self.r_h = planet["radius"] + np.arange(nv + 1) * self.dz
+
+    def __del__(self):
+        try:
+            if self._h:
+                _load().orc_geom_free(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    # Eq. 4-6: horizontal divergence of vec [N][nv][3] at radius r_k -> [N][nv]
+    def hdiv(self, vec):
+        vec = _c(vec)
+        assert vec.shape == (self.N, self.nv, 3)
+        out = np.empty((self.N, self.nv))
+        _load().orc_hdiv(self._h, _p(vec), _p(out))
+        return out
+
+    # Eq. 7 (difference form, projected): horizontal gradient of s [N][nv] -> [N][nv][3]
+    def hgrad(self, s):
+        s = _c(s)
+        assert s.shape == (self.N, self.nv)
+        out = np.empty((self.N, self.nv, 3))
+        _load().orc_hgrad(self._h, _p(s), _p(out))
+        return out
+
+    def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None):
+        """n_large large steps; returns new (rho, V, W, p); inputs are not modified."""
+        rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
+        assert rho.shape == (self.N, self.nv) and V.shape == (self.N, self.nv, 3)
+        assert W.shape == (self.N, self.nv + 1) and p.shape == (self.N, self.nv)
+        assert n_sub >= 2 and n_sub % 2 == 0
+        T_eq = k_T = k_v = None
+        if forcing is not None:
+            T_eq = None if forcing.get("T_eq") is None else _c(forcing["T_eq"])
+            k_T = None if forcing.get("k_T") is None else _c(forcing["k_T"])
+            k_v = None if forcing.get("k_v") is None else _c(forcing["k_v"])
+        _load().orc_step(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
+                         _p(T_eq), _p(k_T), _p(k_v))
+        return rho, V, W, p
+
+    def diagnostics(self, rho, V, W, p):
+        rho, V, W, p = (_c(x) for x in (rho, V, W, p))
+        m = ctypes.c_double()
+        e = ctypes.c_double()
+        _load().orc_diagnostics(self._h, _p(rho), _p(V), _p(W), _p(p), ctypes.byref(m), ctypes.byref(e))
+        return m.value, e.value
+
+    def tridiag_coefficients(self, delta, h, gt):
+        h, gt = _c(h), _c(gt)
+        a, b, c = (np.zeros(self.nv + 1) for _ in range(3))
+        _load().orc_tridiag_coefficients(self._h, float(delta), _p(h), _p(gt), _p(a), _p(b), _p(c))
+        return a, b, c
+
+    def slow_terms(self, rho, V, W, p):
+        rho, V, W, p = (_c(x) for x in (rho, V, W, p))
+        N, nv = self.N, self.nv
+        out = dict(slowV=np.zeros((N, nv, 3)), slowrho=np.zeros((N, nv)), Svr=np.zeros((N, nv + 1)),
+                   slowp=np.zeros((N, nv)), slowrt=np.zeros((N, nv)), h=np.zeros((N, nv)),
+                   th=np.zeros((N, nv)), gt=np.zeros((N, nv + 1)))
+        _load().orc_slow_terms(self._h, _p(rho), _p(V), _p(W), _p(p), *[_p(out[k]) for k in
+                               ("slowV", "slowrho", "Svr", "slowp", "slowrt", "h", "th", "gt")])
+        return out
+
+    def substep(self, delta, stage, dev):
+        """One acoustic substep.  stage: dict(h, th, gt, p_t, slowV, slowrho, Svr, slowp, slowrt);
+        dev: dict(rho_s, V_s, W_s, p_s, rt).  Returns the updated dev (copies)."""
+        st = {k: _c(v) for k, v in stage.items()}
+        dv = {k: _c(v).copy() for k, v in dev.items()}
+        _load().orc_substep(self._h, float(delta), _p(st["h"]), _p(st["th"]), _p(st["gt"]), _p(st["p_t"]),
+                            _p(st["slowV"]), _p(st["slowrho"]), _p(st["Svr"]), _p(st["slowp"]), _p(st["slowrt"]),
+                            _p(dv["rho_s"]), _p(dv["V_s"]), _p(dv["W_s"]), _p(dv["p_s"]), _p(dv["rt"]))
+        return dv
+
+
+def thomas(a, b, c, d):
+    """Thomas algorithm on arrays indexed 1..n (index 0 unused)."""
+    a, b, c, d = (_c(x) for x in (a, b, c, d))
+    n = len(b) - 1
+    x = np.zeros(n + 2)
+    a2, b2, c2, d2 = (np.concatenate([v, [0.0]]) for v in (a, b, c, d))
+    _load().orc_thomas(n, _p(a2), _p(b2), _p(c2), _p(d2), _p(x))
+    return x[: n + 1]
+
+
+def centroid_eq13(r):
+    r = _c(r)
+    out = np.zeros(3)
+    _load().orc_centroid_eq13(_p(r), int(r.shape[0]), _p(out))
+    return out

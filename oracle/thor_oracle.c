@@ -1,0 +1,700 @@
+/*
+ * oracle/thor_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, FP64 CPU statement of what one THOR HE-VI large time step computes
+ * (arXiv 1607.05535; citations are PAPER.md:L<line> + equation; readings R-n and G-n are the ones
+ * listed in SURVEY.md 8(c) and restated in DESIGN.md).  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code, header, table or constant with paper_1607_05535_b200/ (the CUDA path),
+ * and recomputes every geometric coefficient from the point positions it is given.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/__init__.py).
+ * Array-at-a-time, in the paper's order (Fig. 6); no blocking, fusion or reordering.
+ * OpenMP only splits independent columns; there are no reductions inside a step, so results do
+ * not depend on the thread count.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   geometry/div/grad ........ P2 P4 P5 P6 P7 P8 P9 (closed forms, convergence order, identities)
+ *   tridiagonal (orc_substep)  P10 (dense solve of the three discrete fast equations)
+ *   step ..................... P11 (mass), P12 (rest state), P13 (Coriolis), P14 (RK order), P15
+ *   PARITY UNPINNED: the discrete advection form R7, the stage convention R1, the forcing
+ *   convention R9 -- the paper fixes no value for them; only the invariants above constrain them.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+    double radius, omega, gravity, Rd, Cp, p_ref, z_top; /* Table 1 (L409-L418), L213, L454 */
+} orc_planet;
+
+typedef struct {
+    int N, nv;
+    orc_planet P;
+    double dz;
+    double *r_c;  /* [nv]   centre radii     r_k   = A + (k+1/2) dz   (R6: uniform dz, L339, L432) */
+    double *r_h;  /* [nv+1] interface radii  r_h,k = A + k dz */
+    double *z_c;  /* [nv]   centre altitudes */
+    double *xyz;  /* [N][3] unit-sphere positions P_i */
+    int *nbr;     /* [N][6] neighbours, counter-clockwise seen from outside; -1 pads pentagons */
+    int *deg;     /* [N] 5 or 6 */
+    double *C;    /* [N][6][3] control-volume vertices C_k (L61-L63, Fig. 2) */
+    double *len;  /* [N][6]    l_k geodesic arc C_k..C_k+1 (L67) */
+    double *nrm;  /* [N][6][3] outward unit normal of that arc (L67) */
+    double *bary; /* [N][6][3] Eq. 5 weights of (Phi_0, Phi_k, Phi_k+1) at corner k: A2,A3,A1 / sum */
+    double *Ac;   /* [N] control-volume area (Eq. 6) */
+} orc_geom;
+
+static void cross3(const double *a, const double *b, double *c) {
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+static double dot3(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+static double norm3(const double *a) { return sqrt(dot3(a, a)); }
+
+/* geodesic arc between unit vectors (L67 "geodesic arc length"; G4: atan2(|axb|, a.b)) */
+static double arc3(const double *a, const double *b) {
+    double c[3];
+    cross3(a, b, c);
+    return atan2(norm3(c), dot3(a, b));
+}
+
+/* area of the spherical triangle a,b,c on the unit sphere (spherical excess) */
+static double tri_area(const double *a, const double *b, const double *c) {
+    double bc[3];
+    cross3(b, c, bc);
+    double t = fabs(dot3(a, bc));
+    return 2.0 * atan2(t, 1.0 + dot3(a, b) + dot3(b, c) + dot3(c, a));
+}
+
+/* Eq. 13 (L122) with reading G4: r_c ~ sum_i (r_i x r_i+1)/|r_i x r_i+1| * arc(r_i, r_i+1),
+ * normalised to the unit sphere (the printed 1/2pi prefactor is irrelevant after normalising). */
+static void centroid_eq13(const double *r, int n, double *out) {
+    double s[3] = {0, 0, 0};
+    for (int i = 0; i < n; i++) {
+        const double *a = r + 3 * i, *b = r + 3 * ((i + 1) % n);
+        double c[3];
+        cross3(a, b, c);
+        double l = norm3(c);
+        double ang = atan2(l, dot3(a, b));
+        for (int d = 0; d < 3; d++) s[d] += c[d] / l * ang;
+    }
+    double l = norm3(s);
+    for (int d = 0; d < 3; d++) out[d] = s[d] / l;
+}
+
+void orc_geom_free(orc_geom *G) {
+    if (!G) return;
+    free(G->r_c); free(G->r_h); free(G->z_c); free(G->xyz); free(G->nbr); free(G->deg);
+    free(G->C); free(G->len); free(G->nrm); free(G->bary); free(G->Ac);
+    free(G);
+}
+
+/* O2 of SURVEY 8(c): every geometric coefficient from the grid description alone: positions P,
+ * neighbour lists and the control-volume vertices C [N][6][3] that L120 leaves fixed while the
+ * P_i move to the centroids (reading R4 as revised in DESIGN.md).  Cin == NULL: C_k = Eq. 13
+ * centroid of the triangle (P_0, P_k, P_k+1) of the given positions (unmodified grid). */
+orc_geom *orc_geom_build(int N, int nv, const orc_planet *P, const double *xyz, const int *nbr,
+                         const double *Cin) {
+    orc_geom *G = (orc_geom *)calloc(1, sizeof(orc_geom));
+    G->N = N; G->nv = nv; G->P = *P;
+    G->dz = P->z_top / nv;
+    G->r_c = (double *)malloc(sizeof(double) * nv);
+    G->z_c = (double *)malloc(sizeof(double) * nv);
+    G->r_h = (double *)malloc(sizeof(double) * (nv + 1));
+    for (int k = 0; k < nv; k++) { G->z_c[k] = (k + 0.5) * G->dz; G->r_c[k] = P->radius + G->z_c[k]; }
+    for (int k = 0; k <= nv; k++) G->r_h[k] = P->radius + k * G->dz;
+    G->xyz = (double *)malloc(sizeof(double) * 3 * N);
+    memcpy(G->xyz, xyz, sizeof(double) * 3 * N);
+    G->nbr = (int *)malloc(sizeof(int) * 6 * N);
+    memcpy(G->nbr, nbr, sizeof(int) * 6 * N);
+    G->deg = (int *)malloc(sizeof(int) * N);
+    G->C = (double *)calloc((size_t)N * 18, sizeof(double));
+    G->len = (double *)calloc((size_t)N * 6, sizeof(double));
+    G->nrm = (double *)calloc((size_t)N * 18, sizeof(double));
+    G->bary = (double *)calloc((size_t)N * 18, sizeof(double));
+    G->Ac = (double *)calloc((size_t)N, sizeof(double));
+    for (int i = 0; i < N; i++) {
+        int m = 6;
+        if (nbr[6 * i + 5] < 0) m = 5;
+        G->deg[i] = m;
+    }
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        int m = G->deg[i];
+        double *Ci = G->C + 18 * (size_t)i;
+        for (int k = 0; k < m; k++) {
+            int a = nbr[6 * i + k], b = nbr[6 * i + (k + 1) % m];
+            /* canonical rotation (smallest index first, orientation kept) so that the three
+             * columns sharing this triangle obtain bit-identical C_k and Eq. 5 weights */
+            int v[3] = {i, a, b}, rot = 0;
+            if (a < i && a < b) rot = 1;
+            if (b < i && b < a) rot = 2;
+            int c0 = v[rot], c1 = v[(rot + 1) % 3], c2 = v[(rot + 2) % 3];
+            double tri[9];
+            memcpy(tri + 0, xyz + 3 * c0, 24);
+            memcpy(tri + 3, xyz + 3 * c1, 24);
+            memcpy(tri + 6, xyz + 3 * c2, 24);
+            double Ck[3];
+            if (Cin) memcpy(Ck, Cin + 18 * (size_t)i + 3 * k, 24);
+            else centroid_eq13(tri, 3, Ck);
+            memcpy(Ci + 3 * k, Ck, 24);
+            /* Eq. 5 (L73-L75): each vertex is weighted by the sub-triangle opposite to it */
+            double wa[3];
+            wa[0] = tri_area(tri + 3, tri + 6, Ck);
+            wa[1] = tri_area(tri + 6, tri + 0, Ck);
+            wa[2] = tri_area(tri + 0, tri + 3, Ck);
+            double ws = wa[0] + wa[1] + wa[2];
+            /* (Phi_0, Phi_k, Phi_k+1) = canonical vertices (rot*2)%3 ... undo the rotation */
+            double *B = G->bary + 18 * (size_t)i + 3 * k;
+            B[0] = wa[(3 - rot) % 3] / ws;       /* A2/sum: weight of P_0   */
+            B[1] = wa[(4 - rot) % 3] / ws;       /* A3/sum: weight of P_k   */
+            B[2] = wa[(5 - rot) % 3] / ws;       /* A1/sum: weight of P_k+1 */
+        }
+        double area = 0.0;
+        for (int k = 0; k < m; k++) {
+            const double *c0 = Ci + 3 * k, *c1 = Ci + 3 * ((k + 1) % m);
+            G->len[6 * i + k] = arc3(c0, c1);
+            double n[3];
+            cross3(c0, c1, n);
+            double l = norm3(n);
+            /* outward for counter-clockwise ordering: -(C_k x C_k+1)/|.| */
+            for (int d = 0; d < 3; d++) G->nrm[18 * (size_t)i + 3 * k + d] = -n[d] / l;
+            /* control-volume area as a fan of spherical triangles around P_0 */
+            area += tri_area(xyz + 3 * i, c0, c1);
+        }
+        G->Ac[i] = area;
+    }
+    return G;
+}
+
+/* read-only accessors for the tests */
+const double *orc_geom_Ac(const orc_geom *G) { return G->Ac; }
+const double *orc_geom_len(const orc_geom *G) { return G->len; }
+const double *orc_geom_nrm(const orc_geom *G) { return G->nrm; }
+const double *orc_geom_C(const orc_geom *G) { return G->C; }
+const double *orc_geom_bary(const orc_geom *G) { return G->bary; }
+const int *orc_geom_deg(const orc_geom *G) { return G->deg; }
+
+/* Eq. 13 exposed for pin P4 */
+void orc_centroid_eq13(const double *r, int n, double *out) { centroid_eq13(r, n, out); }
+
+/* ---------------------------------------------------------------------------------------------
+ * Horizontal operators (O2).  vec: [N][nv][3], scalars: [N][nv].  Both return the operator at
+ * radius r_k, i.e. the unit-sphere result times 1/r_k (L229, deep atmosphere).
+ * ------------------------------------------------------------------------------------------- */
+
+/* Eq. 4-6 (L65-L79): div_0 = (1/A_c) sum_k l_k (Phi*_k + Phi*_k+1)/2 . n_k, Phi* from Eq. 5 */
+void orc_hdiv(const orc_geom *G, const double *vec, double *out) {
+    const int N = G->N, nv = G->nv;
+#pragma omp parallel
+    {
+        double *phis = (double *)malloc(sizeof(double) * 6 * nv * 3);
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            int m = G->deg[i];
+            const int *nb = G->nbr + 6 * i;
+            const double *v0 = vec + (size_t)i * nv * 3;
+            for (int k = 0; k < m; k++) {
+                const double *B = G->bary + 18 * (size_t)i + 3 * k;
+                const double *va = vec + (size_t)nb[k] * nv * 3;
+                const double *vb = vec + (size_t)nb[(k + 1) % m] * nv * 3;
+                double *ph = phis + (size_t)k * nv * 3;
+                for (int q = 0; q < nv * 3; q++) ph[q] = B[0] * v0[q] + B[1] * va[q] + B[2] * vb[q];
+            }
+            for (int lay = 0; lay < nv; lay++) {
+                double sum = 0.0;
+                for (int k = 0; k < m; k++) {
+                    const double *p0 = phis + ((size_t)k * nv + lay) * 3;
+                    const double *p1 = phis + ((size_t)((k + 1) % m) * nv + lay) * 3;
+                    const double *n = G->nrm + 18 * (size_t)i + 3 * k;
+                    double f = 0.5 * (p0[0] + p1[0]) * n[0] + 0.5 * (p0[1] + p1[1]) * n[1] +
+                               0.5 * (p0[2] + p1[2]) * n[2];
+                    sum += G->len[6 * i + k] * f;                               /* F_k, Eq. 4 */
+                }
+                out[(size_t)i * nv + lay] = sum / G->Ac[i] / G->r_c[lay];      /* Eq. 6 */
+            }
+        }
+        free(phis);
+    }
+}
+
+/* Eq. 7 (L83-L86) in difference form: subtracting s_0 inside the sum IS the correction term,
+ * because Eq. 5's weights sum to one.  R5: the radial part is projected out with
+ * Eq. 28 as corrected by G5, Phi_h = Phi - (Phi.r)r. */
+void orc_hgrad(const orc_geom *G, const double *s, double *out) {
+    const int N = G->N, nv = G->nv;
+#pragma omp parallel
+    {
+        double *ds = (double *)malloc(sizeof(double) * 6 * nv);
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            int m = G->deg[i];
+            const int *nb = G->nbr + 6 * i;
+            const double *s0 = s + (size_t)i * nv;
+            const double *rh = G->xyz + 3 * i;
+            for (int k = 0; k < m; k++) {
+                const double *B = G->bary + 18 * (size_t)i + 3 * k;
+                const double *sa = s + (size_t)nb[k] * nv;
+                const double *sb = s + (size_t)nb[(k + 1) % m] * nv;
+                for (int lay = 0; lay < nv; lay++)
+                    ds[k * nv + lay] = B[1] * (sa[lay] - s0[lay]) + B[2] * (sb[lay] - s0[lay]);
+            }
+            for (int lay = 0; lay < nv; lay++) {
+                double g[3] = {0, 0, 0};
+                for (int k = 0; k < m; k++) {
+                    double f = G->len[6 * i + k] * 0.5 * (ds[k * nv + lay] + ds[((k + 1) % m) * nv + lay]);
+                    const double *n = G->nrm + 18 * (size_t)i + 3 * k;
+                    for (int d = 0; d < 3; d++) g[d] += f * n[d];
+                }
+                double gr = 0.0;
+                for (int d = 0; d < 3; d++) { g[d] /= G->Ac[i]; }
+                gr = g[0] * rh[0] + g[1] * rh[1] + g[2] * rh[2];
+                for (int d = 0; d < 3; d++)
+                    out[((size_t)i * nv + lay) * 3 + d] = (g[d] - gr * rh[d]) / G->r_c[lay];
+            }
+        }
+        free(ds);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Vertical operators (O3; Eq. 8-9 with k = 1, L88-L94; Eq. 27's radial part, L227).
+ * Centre arrays are [nv]; interface arrays are [nv+1] with index 0 = bottom, nv = top.
+ * ------------------------------------------------------------------------------------------- */
+static double I_h(const double *Y, int k) { return 0.5 * (Y[k - 1] + Y[k]); }            /* k=1..nv-1 */
+static double I_c(const double *X, int k) { return 0.5 * (X[k] + X[k + 1]); }            /* k=0..nv-1 */
+static double G_h(const double *Y, int k, double dz) { return (Y[k] - Y[k - 1]) / dz; }  /* k=1..nv-1 */
+static double D_c(const orc_geom *G, const double *X, int k) {                            /* k=0..nv-1 */
+    const double *rh = G->r_h;
+    return (rh[k + 1] * rh[k + 1] * X[k + 1] - rh[k] * rh[k] * X[k]) / (G->r_c[k] * G->r_c[k] * G->dz);
+}
+
+/* Eq. 24 (L210) and its inverse */
+static double eos_p(const orc_planet *P, double rt) {
+    double gam = P->Cp / (P->Cp - P->Rd);
+    return P->p_ref * pow(P->Rd * rt / P->p_ref, gam);
+}
+static double eos_rt(const orc_planet *P, double p) {
+    double gam = P->Cp / (P->Cp - P->Rd);
+    return P->p_ref / P->Rd * pow(p / P->p_ref, 1.0 / gam);
+}
+
+/* Thomas algorithm (L339) for a_k x_k-1 + b_k x_k + c_k x_k+1 = d_k, k = 1..n; arrays are
+ * indexed 1..n (index 0 unused); a_1 and c_n multiply the zero boundary values (rigid lid). */
+void orc_thomas(int n, const double *a, const double *b, const double *c, const double *d, double *x) {
+    double *cp = (double *)malloc(sizeof(double) * (n + 2));
+    double *dp = (double *)malloc(sizeof(double) * (n + 2));
+    cp[1] = c[1] / b[1];
+    dp[1] = d[1] / b[1];
+    for (int k = 2; k <= n; k++) {
+        double den = b[k] - a[k] * cp[k - 1];
+        cp[k] = c[k] / den;
+        dp[k] = (d[k] - a[k] * dp[k - 1]) / den;
+    }
+    x[n] = dp[n];
+    for (int k = n - 1; k >= 1; k--) x[k] = dp[k] - cp[k] * x[k + 1];
+    free(cp); free(dp);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Work space of one large step
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    size_t nc, ni;                      /* N*nv, N*(nv+1) */
+    /* Phi^n */
+    double *rho_n, *V_n, *W_n, *p_n, *rt_n;
+    /* reference state of the stage, Phi^[t] */
+    double *rho_t, *V_t, *W_t, *p_t;
+    /* a1: stage coefficients */
+    double *h, *th, *gt;                /* gt: [N][nv+1], interior interfaces only */
+    /* a2: slow terms */
+    double *slowV, *slowrho, *Svr, *slowp, *slowrt;
+    /* deviations */
+    double *rho_s, *V_s, *W_s, *p_s, *rt;
+    /* scratch */
+    double *vec, *sc1, *sc2, *sc3, *gradp, *u, *Avec, *Wc;
+} orc_work;
+
+static double *dalloc(size_t n) { return (double *)calloc(n, sizeof(double)); }
+
+static orc_work *work_new(const orc_geom *G) {
+    orc_work *w = (orc_work *)calloc(1, sizeof(orc_work));
+    size_t nc = (size_t)G->N * G->nv, ni = (size_t)G->N * (G->nv + 1);
+    w->nc = nc; w->ni = ni;
+    w->rho_n = dalloc(nc); w->V_n = dalloc(3 * nc); w->W_n = dalloc(ni); w->p_n = dalloc(nc); w->rt_n = dalloc(nc);
+    w->rho_t = dalloc(nc); w->V_t = dalloc(3 * nc); w->W_t = dalloc(ni); w->p_t = dalloc(nc);
+    w->h = dalloc(nc); w->th = dalloc(nc); w->gt = dalloc(ni);
+    w->slowV = dalloc(3 * nc); w->slowrho = dalloc(nc); w->Svr = dalloc(ni); w->slowp = dalloc(nc); w->slowrt = dalloc(nc);
+    w->rho_s = dalloc(nc); w->V_s = dalloc(3 * nc); w->W_s = dalloc(ni); w->p_s = dalloc(nc); w->rt = dalloc(nc);
+    w->vec = dalloc(3 * nc); w->sc1 = dalloc(nc); w->sc2 = dalloc(nc); w->sc3 = dalloc(nc);
+    w->gradp = dalloc(3 * nc); w->u = dalloc(3 * nc); w->Avec = dalloc(3 * nc); w->Wc = dalloc(nc);
+    return w;
+}
+static void work_free(orc_work *w) {
+    double **p[] = {&w->rho_n, &w->V_n, &w->W_n, &w->p_n, &w->rt_n, &w->rho_t, &w->V_t, &w->W_t, &w->p_t,
+                    &w->h, &w->th, &w->gt, &w->slowV, &w->slowrho, &w->Svr, &w->slowp, &w->slowrt,
+                    &w->rho_s, &w->V_s, &w->W_s, &w->p_s, &w->rt, &w->vec, &w->sc1, &w->sc2, &w->sc3,
+                    &w->gradp, &w->u, &w->Avec, &w->Wc};
+    for (size_t i = 0; i < sizeof(p) / sizeof(p[0]); i++) free(*p[i]);
+    free(w);
+}
+
+/* a1 (Eq. 38-39; Fig. 6 large-step 1): h = Cp T = Cp p/(Rd rho) (G9),
+ * theta = (rho theta)/rho with rho theta from Eq. 24 inverted, g~ = G_h[p]/I_h[rho] at interfaces */
+static void stage_coefficients(const orc_geom *G, orc_work *w) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rho = w->rho_t + (size_t)i * nv, *p = w->p_t + (size_t)i * nv;
+        double *h = w->h + (size_t)i * nv, *th = w->th + (size_t)i * nv, *gt = w->gt + (size_t)i * (nv + 1);
+        for (int k = 0; k < nv; k++) {
+            h[k] = P->Cp * p[k] / (P->Rd * rho[k]);
+            th[k] = eos_rt(P, p[k]) / rho[k];
+        }
+        gt[0] = 0.0; gt[nv] = 0.0;
+        for (int k = 1; k < nv; k++) gt[k] = G_h(p, k, G->dz) / I_h(rho, k);
+    }
+}
+
+/* a2 (RHS of Eq. 32-35, Eq. 40-42; L258-L299, L268; O4 with reading R7) */
+static void slow_terms(const orc_geom *G, orc_work *w) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double kv = P->Rd / (P->Cp - P->Rd);
+    const size_t nc = w->nc;
+
+    /* full Cartesian momentum M = V + I_c[W] r, velocity u = M/rho (L268 "non-projected") */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rh = G->xyz + 3 * i;
+        const double *W = w->W_t + (size_t)i * (nv + 1);
+        for (int k = 0; k < nv; k++) {
+            size_t c = (size_t)i * nv + k;
+            double wc = I_c(W, k);
+            w->Wc[c] = wc;
+            for (int d = 0; d < 3; d++) w->u[3 * c + d] = (w->V_t[3 * c + d] + wc * rh[d]) / w->rho_t[c];
+        }
+    }
+
+    /* advection A_j = div_h(V u_j) + D_c[W I_h[u_j]] for each Cartesian component j (Eq. 21, 27) */
+    for (int j = 0; j < 3; j++) {
+#pragma omp parallel for schedule(static)
+        for (size_t c = 0; c < nc; c++)
+            for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->V_t[3 * c + d] * w->u[3 * c + j];
+        orc_hdiv(G, w->vec, w->sc1);
+#pragma omp parallel
+        {
+            double *X = (double *)calloc(nv + 1, sizeof(double));
+            double *uj = (double *)malloc(sizeof(double) * nv);
+#pragma omp for schedule(static)
+            for (int i = 0; i < N; i++) {
+                const double *W = w->W_t + (size_t)i * (nv + 1);
+                for (int k = 0; k < nv; k++) uj[k] = w->u[3 * ((size_t)i * nv + k) + j];
+                X[0] = 0.0; X[nv] = 0.0;
+                for (int k = 1; k < nv; k++) X[k] = W[k] * I_h(uj, k);
+                for (int k = 0; k < nv; k++) {
+                    size_t c = (size_t)i * nv + k;
+                    w->Avec[3 * c + j] = w->sc1[c] + D_c(G, X, k);
+                }
+            }
+            free(X); free(uj);
+        }
+    }
+
+    /* grad_h p^[t] */
+    orc_hgrad(G, w->p_t, w->gradp);
+    /* div_h V, div_h (h V), div_h (theta V) */
+    orc_hdiv(G, w->V_t, w->sc1);
+#pragma omp parallel for schedule(static)
+    for (size_t c = 0; c < nc; c++)
+        for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->h[c] * w->V_t[3 * c + d];
+    orc_hdiv(G, w->vec, w->sc2);
+#pragma omp parallel for schedule(static)
+    for (size_t c = 0; c < nc; c++)
+        for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->th[c] * w->V_t[3 * c + d];
+    orc_hdiv(G, w->vec, w->sc3);
+
+#pragma omp parallel
+    {
+        double *X = (double *)calloc(nv + 1, sizeof(double));
+        double *Fr = (double *)malloc(sizeof(double) * nv);
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            const double *rh = G->xyz + 3 * i;
+            const double *W = w->W_t + (size_t)i * (nv + 1);
+            const double *rho = w->rho_t + (size_t)i * nv, *p = w->p_t + (size_t)i * nv;
+            const double *h = w->h + (size_t)i * nv, *th = w->th + (size_t)i * nv;
+            const double *gt = w->gt + (size_t)i * (nv + 1);
+            double *Svr = w->Svr + (size_t)i * (nv + 1);
+            for (int k = 0; k < nv; k++) {
+                size_t c = (size_t)i * nv + k;
+                const double *A = w->Avec + 3 * c;
+                /* Coriolis C = 2 Omega z x M (Eq. 21), rotation axis through the polar vertices */
+                double M[3], Cor[3];
+                for (int d = 0; d < 3; d++) M[d] = w->V_t[3 * c + d] + w->Wc[c] * rh[d];
+                Cor[0] = -2.0 * P->omega * M[1];
+                Cor[1] = 2.0 * P->omega * M[0];
+                Cor[2] = 0.0;
+                double Ar = dot3(A, rh), Cr = dot3(Cor, rh);                   /* Eq. 29 */
+                Fr[k] = Ar + Cr;
+                for (int d = 0; d < 3; d++) {                                   /* Eq. 28 (G5) */
+                    double Ah = A[d] - Ar * rh[d], Ch = Cor[d] - Cr * rh[d];
+                    w->slowV[3 * c + d] = -w->gradp[3 * c + d] - Ah - Ch;       /* RHS of Eq. 33 */
+                }
+            }
+            /* RHS of Eq. 32 */
+            for (int k = 0; k < nv; k++) w->slowrho[(size_t)i * nv + k] = -w->sc1[(size_t)i * nv + k] - D_c(G, W, k);
+            /* Eq. 42 at interior interfaces */
+            Svr[0] = 0.0; Svr[nv] = 0.0;
+            for (int k = 1; k < nv; k++) Svr[k] = -G_h(p, k, G->dz) - P->gravity * I_h(rho, k) - I_h(Fr, k);
+            /* slow part of the pressure equation (Eq. 40 with the signs of G10) */
+            X[0] = 0.0; X[nv] = 0.0;
+            for (int k = 1; k < nv; k++) X[k] = I_h(h, k) * W[k];
+            for (int k = 0; k < nv; k++) {
+                size_t c = (size_t)i * nv + k;
+                double vgp = 0.0;
+                for (int d = 0; d < 3; d++) vgp += w->V_t[3 * c + d] / rho[k] * w->gradp[3 * c + d];
+                double gW = 0.5 * (gt[k] * W[k] + gt[k + 1] * W[k + 1]);        /* I_c[g~ W] */
+                w->slowp[c] = -kv * (w->sc2[c] + D_c(G, X, k) - vgp - gW);
+            }
+            /* slow part of Eq. 35 (G7: with the r^2 factors of Eq. 27) */
+            for (int k = 1; k < nv; k++) X[k] = I_h(th, k) * W[k];
+            for (int k = 0; k < nv; k++) {
+                size_t c = (size_t)i * nv + k;
+                w->slowrt[c] = -w->sc3[c] - D_c(G, X, k);
+            }
+        }
+        free(X); free(Fr);
+    }
+}
+
+/* Tridiagonal coefficients of O6 item 3 for one column at interior interfaces k = 1..nv-1
+ * (exact elimination of Eq. 32, the linearised pressure equation and Eq. 34; reading R8). */
+static void tridiag_coefficients(const orc_geom *G, double delta, const double *h, const double *gt,
+                                 double *a, double *b, double *c) {
+    const int nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double kv = P->Rd / (P->Cp - P->Rd), dz = G->dz, g = P->gravity;
+    const double *rc = G->r_c, *rh = G->r_h;
+    const double d2 = delta * delta;
+    for (int k = 1; k < nv; k++) {
+        double hk = I_h(h, k);
+        double hkp = (k + 1 < nv) ? I_h(h, k + 1) : 0.0;   /* multiplies W_nv = 0 */
+        double hkm = (k - 1 > 0) ? I_h(h, k - 1) : 0.0;    /* multiplies W_0  = 0 */
+        double rk2 = rc[k] * rc[k], rkm2 = rc[k - 1] * rc[k - 1];
+        c[k] = -(d2 * kv / dz) * (rh[k + 1] * rh[k + 1] * hkp / (rk2 * dz) - gt[k + 1] / 2.0)
+               - (d2 * g / (2.0 * dz)) * rh[k + 1] * rh[k + 1] / rk2;
+        a[k] = -(d2 * kv / dz) * (rh[k - 1] * rh[k - 1] * hkm / (rkm2 * dz) + gt[k - 1] / 2.0)
+               + (d2 * g / (2.0 * dz)) * rh[k - 1] * rh[k - 1] / rkm2;
+        b[k] = 1.0 + (d2 * kv / (dz * dz)) * rh[k] * rh[k] * hk * (1.0 / rk2 + 1.0 / rkm2)
+               - (d2 * g / (2.0 * dz)) * rh[k] * rh[k] * (1.0 / rkm2 - 1.0 / rk2);
+    }
+}
+
+/* a4-a9: one acoustic substep (O6; Eq. 33, 37, 32, 35, 36; Fig. 6 small-step 2-6, L318-L329) */
+static void substep(const orc_geom *G, orc_work *w, double delta) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double kv = P->Rd / (P->Cp - P->Rd), dz = G->dz, g = P->gravity;
+    const size_t nc = w->nc;
+
+    /* a4: Eq. 33 */
+    orc_hgrad(G, w->p_s, w->gradp);
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < 3 * nc; q++) w->V_s[q] = w->V_s[q] + delta * (-w->gradp[q] + w->slowV[q]);
+
+    /* a5: divergences of the new momentum */
+    orc_hdiv(G, w->V_s, w->sc1);
+#pragma omp parallel for schedule(static)
+    for (size_t c = 0; c < nc; c++)
+        for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->h[c] * w->V_s[3 * c + d];
+    orc_hdiv(G, w->vec, w->sc2);
+#pragma omp parallel for schedule(static)
+    for (size_t c = 0; c < nc; c++)
+        for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->th[c] * w->V_s[3 * c + d];
+    orc_hdiv(G, w->vec, w->sc3);
+
+#pragma omp parallel
+    {
+        double *a = (double *)calloc(nv + 1, sizeof(double)), *b = (double *)calloc(nv + 1, sizeof(double));
+        double *c = (double *)calloc(nv + 1, sizeof(double)), *d = (double *)calloc(nv + 1, sizeof(double));
+        double *Wn = (double *)calloc(nv + 1, sizeof(double)), *X = (double *)calloc(nv + 1, sizeof(double));
+        double *Srho = (double *)malloc(sizeof(double) * nv), *Sp = (double *)malloc(sizeof(double) * nv);
+        double *pq = (double *)malloc(sizeof(double) * nv), *rq = (double *)malloc(sizeof(double) * nv);
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            size_t c0 = (size_t)i * nv;
+            const double *h = w->h + c0, *th = w->th + c0, *gt = w->gt + (size_t)i * (nv + 1);
+            double *Ws = w->W_s + (size_t)i * (nv + 1);
+            const double *Svr = w->Svr + (size_t)i * (nv + 1);
+            for (int k = 0; k < nv; k++) {
+                Srho[k] = w->slowrho[c0 + k] - w->sc1[c0 + k];                 /* Eq. 41 */
+                Sp[k] = w->slowp[c0 + k] - kv * w->sc2[c0 + k];                /* Eq. 40 (G10) */
+                pq[k] = w->p_s[c0 + k] + delta * Sp[k];
+                rq[k] = w->rho_s[c0 + k] + delta * Srho[k];
+            }
+            /* a6: assemble and solve (Eq. 37 as defined by elimination, R8; L339) */
+            tridiag_coefficients(G, delta, h, gt, a, b, c);
+            for (int k = 1; k < nv; k++)
+                d[k] = Ws[k] + delta * Svr[k] - delta * G_h(pq, k, dz) - delta * g * I_h(rq, k);
+            Wn[0] = 0.0; Wn[nv] = 0.0;
+            if (nv > 1) orc_thomas(nv - 1, a, b, c, d, Wn);
+            /* a7: Eq. 32 with the new momenta (L341) */
+            for (int k = 0; k < nv; k++) w->rho_s[c0 + k] = w->rho_s[c0 + k] + delta * (Srho[k] - D_c(G, Wn, k));
+            /* a8: Eq. 35 (G7) */
+            X[0] = 0.0; X[nv] = 0.0;
+            for (int k = 1; k < nv; k++) X[k] = I_h(th, k) * Wn[k];
+            for (int k = 0; k < nv; k++)
+                w->rt[c0 + k] = w->rt[c0 + k] + delta * (w->slowrt[c0 + k] - w->sc3[c0 + k] - D_c(G, X, k));
+            /* a9: Eq. 36 */
+            for (int k = 0; k < nv; k++) w->p_s[c0 + k] = eos_p(P, w->rt[c0 + k]) - w->p_t[c0 + k];
+            for (int k = 0; k <= nv; k++) Ws[k] = Wn[k];
+        }
+        free(a); free(b); free(c); free(d); free(Wn); free(X); free(Srho); free(Sp); free(pq); free(rq);
+    }
+}
+
+/* a11: Eq. 51-52 backward Euler with the large step (L385-L399; R9).  Tables are [N][nv]; NULL = off */
+static void forcing(const orc_geom *G, double dt, double *rho, double *V, double *p,
+                    const double *T_eq, const double *k_T, const double *k_v) {
+    const size_t nc = (size_t)G->N * G->nv;
+    const double Rd = G->P.Rd;
+#pragma omp parallel for schedule(static)
+    for (size_t c = 0; c < nc; c++) {
+        if (k_v)
+            for (int d = 0; d < 3; d++) V[3 * c + d] = V[3 * c + d] / (1.0 + k_v[c] * dt);      /* Eq. 51 */
+        if (k_T && T_eq) {
+            double T = p[c] / (rho[c] * Rd);                                                    /* Eq. 25 */
+            T = (T + k_T[c] * dt * T_eq[c]) / (1.0 + k_T[c] * dt);                              /* Eq. 52 */
+            p[c] = rho[c] * Rd * T;
+        }
+    }
+}
+
+/* One call = n_large large steps (Fig. 6; stage convention R1 of SURVEY O5).
+ * State arrays are updated in place: rho,p [N][nv]; V [N][nv][3]; W [N][nv+1] (ends forced to 0). */
+void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
+              int n_sub, const double *T_eq, const double *k_T, const double *k_v) {
+    const int N = G->N, nv = G->nv;
+    orc_work *w = work_new(G);
+    const size_t nc = w->nc, ni = w->ni;
+    for (int i = 0; i < N; i++) { W[(size_t)i * (nv + 1)] = 0.0; W[(size_t)i * (nv + 1) + nv] = 0.0; }
+    for (int step = 0; step < n_large; step++) {
+        memcpy(w->rho_n, rho, 8 * nc); memcpy(w->V_n, V, 24 * nc); memcpy(w->W_n, W, 8 * ni); memcpy(w->p_n, p, 8 * nc);
+#pragma omp parallel for schedule(static)
+        for (size_t c = 0; c < nc; c++) w->rt_n[c] = eos_rt(&G->P, w->p_n[c]);
+        memcpy(w->rho_t, rho, 8 * nc); memcpy(w->V_t, V, 24 * nc); memcpy(w->W_t, W, 8 * ni); memcpy(w->p_t, p, 8 * nc);
+        for (int stage = 1; stage <= 3; stage++) {                 /* Eq. 30 (L245-L250) */
+            stage_coefficients(G, w);                              /* Fig. 6 large-step 1 */
+            slow_terms(G, w);                                      /* Fig. 6 large-step 3 */
+            int ns; double delta;                                  /* L252, L312-L316 */
+            if (stage == 1) { ns = 1; delta = dt / 3.0; }
+            else if (stage == 2) { ns = n_sub / 2; delta = dt / n_sub; }
+            else { ns = n_sub; delta = dt / n_sub; }
+            /* Eq. 31: deviations from the stage reference, every stage starting from t_n */
+#pragma omp parallel for schedule(static)
+            for (size_t c = 0; c < nc; c++) {
+                w->rho_s[c] = w->rho_n[c] - w->rho_t[c];
+                w->p_s[c] = w->p_n[c] - w->p_t[c];
+                w->rt[c] = w->rt_n[c];
+                for (int d = 0; d < 3; d++) w->V_s[3 * c + d] = w->V_n[3 * c + d] - w->V_t[3 * c + d];
+            }
+#pragma omp parallel for schedule(static)
+            for (size_t c = 0; c < ni; c++) w->W_s[c] = w->W_n[c] - w->W_t[c];
+            for (int s = 0; s < ns; s++) substep(G, w, delta);
+            /* Fig. 6 large-step 4: Phi^(s) = Phi^[t] + Phi* */
+#pragma omp parallel for schedule(static)
+            for (size_t c = 0; c < nc; c++) {
+                w->rho_t[c] = w->rho_t[c] + w->rho_s[c];
+                w->p_t[c] = w->p_t[c] + w->p_s[c];
+                for (int d = 0; d < 3; d++) w->V_t[3 * c + d] = w->V_t[3 * c + d] + w->V_s[3 * c + d];
+            }
+#pragma omp parallel for schedule(static)
+            for (size_t c = 0; c < ni; c++) w->W_t[c] = w->W_t[c] + w->W_s[c];
+        }
+        memcpy(rho, w->rho_t, 8 * nc); memcpy(V, w->V_t, 24 * nc); memcpy(W, w->W_t, 8 * ni); memcpy(p, w->p_t, 8 * nc);
+        forcing(G, dt, rho, V, p, T_eq, k_T, k_v);
+    }
+    work_free(w);
+}
+
+/* a12 (O8, R10): total mass and total energy with the weight A_c r_k^2 dz under which D_c telescopes.
+ * Neumaier-compensated sums, serial, so the result does not depend on threads. */
+static void ksum(double *s, double *comp, double x) {
+    double t = *s + x;
+    if (fabs(*s) >= fabs(x)) *comp += (*s - t) + x; else *comp += (x - t) + *s;
+    *s = t;
+}
+void orc_diagnostics(const orc_geom *G, const double *rho, const double *V, const double *W, const double *p,
+                     double *mass, double *energy) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double Cv = P->Cp - P->Rd;
+    double sm = 0, cm = 0, se = 0, ce = 0;
+    for (int i = 0; i < N; i++)
+        for (int k = 0; k < nv; k++) {
+            size_t c = (size_t)i * nv + k;
+            double vol = G->Ac[i] * G->r_c[k] * G->r_c[k] * G->dz;
+            double wc = I_c(W + (size_t)i * (nv + 1), k);
+            double ke = 0.5 * (V[3 * c] * V[3 * c] + V[3 * c + 1] * V[3 * c + 1] + V[3 * c + 2] * V[3 * c + 2] + wc * wc) / rho[c];
+            double e = Cv * p[c] / P->Rd + ke + rho[c] * P->gravity * G->z_c[k];
+            ksum(&sm, &cm, rho[c] * vol);
+            ksum(&se, &ce, e * vol);
+        }
+    *mass = sm + cm;
+    *energy = se + ce;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Pieces exposed one at a time for the pins (same code the step runs)
+ * ------------------------------------------------------------------------------------------- */
+
+/* P10: tridiagonal coefficients of one column, arrays [nv+1] indexed by interface */
+void orc_tridiag_coefficients(const orc_geom *G, double delta, const double *h, const double *gt,
+                              double *a, double *b, double *c) {
+    tridiag_coefficients(G, delta, h, gt, a, b, c);
+}
+
+/* P13 / P12: slow terms of a given state; outputs sized as in orc_work */
+void orc_slow_terms(const orc_geom *G, const double *rho, const double *V, const double *W, const double *p,
+                    double *slowV, double *slowrho, double *Svr, double *slowp, double *slowrt,
+                    double *h, double *th, double *gt) {
+    orc_work *w = work_new(G);
+    memcpy(w->rho_t, rho, 8 * w->nc); memcpy(w->V_t, V, 24 * w->nc); memcpy(w->W_t, W, 8 * w->ni); memcpy(w->p_t, p, 8 * w->nc);
+    stage_coefficients(G, w);
+    slow_terms(G, w);
+    memcpy(slowV, w->slowV, 24 * w->nc); memcpy(slowrho, w->slowrho, 8 * w->nc); memcpy(Svr, w->Svr, 8 * w->ni);
+    memcpy(slowp, w->slowp, 8 * w->nc); memcpy(slowrt, w->slowrt, 8 * w->nc);
+    memcpy(h, w->h, 8 * w->nc); memcpy(th, w->th, 8 * w->nc); memcpy(gt, w->gt, 8 * w->ni);
+    work_free(w);
+}
+
+/* P10: one substep on caller-provided stage data (all arrays in/out as named in O6) */
+void orc_substep(const orc_geom *G, double delta, const double *h, const double *th, const double *gt,
+                 const double *p_t, const double *slowV, const double *slowrho, const double *Svr,
+                 const double *slowp, const double *slowrt,
+                 double *rho_s, double *V_s, double *W_s, double *p_s, double *rt) {
+    orc_work *w = work_new(G);
+    size_t nc = w->nc, ni = w->ni;
+    memcpy(w->h, h, 8 * nc); memcpy(w->th, th, 8 * nc); memcpy(w->gt, gt, 8 * ni); memcpy(w->p_t, p_t, 8 * nc);
+    memcpy(w->slowV, slowV, 24 * nc); memcpy(w->slowrho, slowrho, 8 * nc); memcpy(w->Svr, Svr, 8 * ni);
+    memcpy(w->slowp, slowp, 8 * nc); memcpy(w->slowrt, slowrt, 8 * nc);
+    memcpy(w->rho_s, rho_s, 8 * nc); memcpy(w->V_s, V_s, 24 * nc); memcpy(w->W_s, W_s, 8 * ni);
+    memcpy(w->p_s, p_s, 8 * nc); memcpy(w->rt, rt, 8 * nc);
+    substep(G, w, delta);
+    memcpy(rho_s, w->rho_s, 8 * nc); memcpy(V_s, w->V_s, 24 * nc); memcpy(W_s, w->W_s, 8 * ni);
+    memcpy(p_s, w->p_s, 8 * nc); memcpy(rt, w->rt, 8 * nc);
+    work_free(w);
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,320 @@
+"""Pins P10-P15 of the oracle's time step plus closed-form checks of the slow
+terms.  Grids come from the oracle's own generator; nothing comes from the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import thor_inputs as ti
+
+
+def _geom(ogrid, level, nv, planet):
+    xyz, nbr, C = ogrid(level, True)
+    return oracle.Geometry(xyz, nbr, nv, planet, C)
+
+
+# ------------------------------------------------------------------------------------------ P10
+def test_p10_thomas_matches_dense_lu():
+    rng = np.random.default_rng(10)
+    for n in (1, 2, 5, 7):
+        a, b, c, d = (rng.standard_normal(n + 1) for _ in range(4))
+        b = b + 4.0 * np.sign(b)                                   # diagonally dominant
+        x = oracle.thomas(a, b, c, d)
+        A = np.zeros((n, n))
+        for k in range(1, n + 1):
+            A[k - 1, k - 1] = b[k]
+            if k > 1:
+                A[k - 1, k - 2] = a[k]
+            if k < n:
+                A[k - 1, k] = c[k]
+        ref = np.linalg.solve(A, d[1:])
+        assert np.abs(x[1:] - ref).max() < 1e-13 * max(1.0, np.abs(ref).max())
+
+
+def _dense_column_solve(G, delta, col, stage, dev, divV, divhV):
+    """Solve the THREE discrete fast equations of one column as one dense linear system in the
+    unknowns (W'_1..nv-1, rho*'_0..nv-1, p'_lin_0..nv-1), written out directly from Eq. 32, the
+    linearised pressure equation and Eq. 34 (no elimination)."""
+    nv = G.nv
+    P = G.planet
+    kv = P["Rd"] / (P["Cp"] - P["Rd"])
+    g, dz = P["gravity"], G.dz
+    rc, rh = G.r_c, G.r_h
+    h, gt = stage["h"][col], stage["gt"][col]
+    hh = np.zeros(nv + 1)
+    hh[1:nv] = 0.5 * (h[:-1] + h[1:])
+    nW = nv - 1
+    n = nW + 2 * nv
+    A = np.zeros((n, n))
+    b = np.zeros(n)
+    iW = lambda k: k - 1            # interface k = 1..nv-1
+    iR = lambda j: nW + j
+    iP = lambda j: nW + nv + j
+    S_rho = stage["slowrho"][col] - divV[col]
+    S_p = stage["slowp"][col] - kv * divhV[col]
+    for j in range(nv):
+        # Eq. 32: rho' + delta * D_c[W'] = rho* + delta S_rho
+        A[iR(j), iR(j)] = 1.0
+        if j + 1 <= nv - 1:
+            A[iR(j), iW(j + 1)] += delta * rh[j + 1] ** 2 / (rc[j] ** 2 * dz)
+        if j >= 1:
+            A[iR(j), iW(j)] -= delta * rh[j] ** 2 / (rc[j] ** 2 * dz)
+        b[iR(j)] = dev["rho_s"][col, j] + delta * S_rho[j]
+        # pressure: p' + delta kv (D_c[h_h W'] - I_c[g~ W']) = p* + delta S_p
+        A[iP(j), iP(j)] = 1.0
+        if j + 1 <= nv - 1:
+            A[iP(j), iW(j + 1)] += delta * kv * (rh[j + 1] ** 2 * hh[j + 1] / (rc[j] ** 2 * dz) - 0.5 * gt[j + 1])
+        if j >= 1:
+            A[iP(j), iW(j)] += delta * kv * (-rh[j] ** 2 * hh[j] / (rc[j] ** 2 * dz) - 0.5 * gt[j])
+        b[iP(j)] = dev["p_s"][col, j] + delta * S_p[j]
+    for k in range(1, nv):
+        # Eq. 34: (W' - W*)/delta + G_h[p'] + g I_h[rho'] = S_vr
+        A[iW(k), iW(k)] = 1.0 / delta
+        A[iW(k), iP(k)] += 1.0 / dz
+        A[iW(k), iP(k - 1)] -= 1.0 / dz
+        A[iW(k), iR(k)] += 0.5 * g
+        A[iW(k), iR(k - 1)] += 0.5 * g
+        b[iW(k)] = stage["Svr"][col, k] + dev["W_s"][col, k] / delta
+    x = np.linalg.solve(A, b)
+    return x[:nW], x[nW:nW + nv], x[nW + nv:]
+
+
+def test_p10_substep_matches_dense_solve_of_the_three_fast_equations(ogrid):
+    cfg = ti.CONFIGS[0]
+    xyz, nbr, C = ogrid(2, True)
+    nv = 6
+    G = oracle.Geometry(xyz, nbr, nv, cfg["planet"], C)
+    rng = np.random.default_rng(11)
+    rho, V, W, p = ti.rest_state(cfg["planet"], nv, G.N, 1e5, 300.0)
+    T = 300.0 * (1 + rng.uniform(-2e-2, 2e-2, size=rho.shape))
+    rho = p / (287.0 * T)
+    vel = rng.uniform(-5, 5, size=V.shape)
+    vel -= np.sum(vel * xyz[:, None, :], axis=-1, keepdims=True) * xyz[:, None, :]
+    V = rho[..., None] * vel
+    W[:, 1:nv] = rng.uniform(-0.5, 0.5, size=(G.N, nv - 1))
+    st = G.slow_terms(rho, V, W, p)
+    stage = dict(st, p_t=p)
+    dev = dict(rho_s=rng.uniform(-1e-3, 1e-3, size=rho.shape), V_s=rng.uniform(-1, 1, size=V.shape),
+               W_s=np.zeros_like(W), p_s=rng.uniform(-50, 50, size=p.shape),
+               rt=p / 287.0 * (1e5 / p) ** (287.0 / 1005.0) * 0 + (1e5 / 287.0) * (p / 1e5) ** (1 - 287.0 / 1005.0))
+    dev["V_s"] -= np.sum(dev["V_s"] * xyz[:, None, :], axis=-1, keepdims=True) * xyz[:, None, :]
+    dev["W_s"][:, 1:nv] = rng.uniform(-0.1, 0.1, size=(G.N, nv - 1))
+    delta = 300.0
+    new = G.substep(delta, stage, dev)
+    # Eq. 33 by hand from the (separately pinned) gradient operator
+    Vexp = dev["V_s"] + delta * (-G.hgrad(dev["p_s"]) + st["slowV"])
+    assert np.abs(new["V_s"] - Vexp).max() < 1e-12 * np.abs(Vexp).max()
+    divV = G.hdiv(new["V_s"])
+    divhV = G.hdiv(st["h"][..., None] * new["V_s"])
+    divtV = G.hdiv(st["th"][..., None] * new["V_s"])
+    for col in (0, 3, 77, G.N - 1):
+        Wd, rd, pl = _dense_column_solve(G, delta, col, stage, dev, divV, divhV)
+        assert np.abs(new["W_s"][col, 1:nv] - Wd).max() < 1e-11 * np.abs(Wd).max()
+        assert np.abs(new["rho_s"][col] - rd).max() < 1e-11 * np.abs(rd).max()
+        assert new["W_s"][col, 0] == 0.0 and new["W_s"][col, nv] == 0.0          # rigid lid, L339
+        # Eq. 35 (G7) and Eq. 36 from the dense W'
+        Wn = np.concatenate([[0.0], Wd, [0.0]])
+        thh = np.zeros(nv + 1)
+        thh[1:nv] = 0.5 * (st["th"][col, :-1] + st["th"][col, 1:])
+        X = thh * Wn
+        Dc = (G.r_h[1:] ** 2 * X[1:] - G.r_h[:-1] ** 2 * X[:-1]) / (G.r_c ** 2 * G.dz)
+        rt_exp = dev["rt"][col] + delta * (st["slowrt"][col] - divtV[col] - Dc)
+        assert np.abs(new["rt"][col] - rt_exp).max() < 1e-12 * np.abs(rt_exp).max()
+        gam = 1005.0 / (1005.0 - 287.0)
+        p_exp = 1e5 * (287.0 * rt_exp / 1e5) ** gam - p[col]
+        assert np.abs(new["p_s"][col] - p_exp).max() < 1e-9
+    # tridiagonal is diagonally dominant enough for Thomas without pivoting
+    a, b, c = G.tridiag_coefficients(delta, st["h"][5], st["gt"][5])
+    assert np.all(np.abs(b[1:nv]) > 0.9 * (np.abs(a[1:nv]) + np.abs(c[1:nv])))
+
+
+# ------------------------------------------------------------------------------------- P11, P12
+def test_p12_resting_isothermal_atmosphere_stays_at_rest(ogrid):
+    cfg = ti.CONFIGS[0]
+    G = _geom(ogrid, 3, cfg["nv"], cfg["planet"])
+    rho, V, W, p = ti.rest_state(cfg["planet"], cfg["nv"], G.N, cfg["p_s"], cfg["T0"])
+    r2, V2, W2, p2 = G.step(rho, V, W, p, 10, cfg["dt"], cfg["n_sub"])
+    w = W2[:, 1:-1] / (0.5 * (r2[:, 1:] + r2[:, :-1]))
+    assert np.abs(w).max() < 1e-9                                     # m/s
+    assert np.abs(V2 / r2[..., None]).max() < 1e-9
+    assert np.abs(r2 - rho).max() < 1e-13 * rho.max()
+    assert np.abs(p2 - p).max() < 1e-13 * p.max()
+    # an analytically exponential profile is NOT at rest discretely (O(dz^2) residual): sanity
+    z = G.z_c
+    p_exp = np.tile(1e5 * np.exp(-9.8 * z / (287.0 * 300.0)), (G.N, 1))
+    r3, V3, W3, p3 = G.step(p_exp / (287.0 * 300.0), V, W, p_exp, 1, cfg["dt"], cfg["n_sub"])
+    assert np.abs(W3).max() > 1e-6
+
+
+@pytest.mark.parametrize("forced", [False, True])
+def test_p11_total_mass_is_conserved_to_roundoff(ogrid, forced):
+    cfg = ti.CONFIGS[0]
+    xyz, nbr, C = ogrid(3, True)
+    G = oracle.Geometry(xyz, nbr, cfg["nv"], cfg["planet"], C)
+    state = ti.initial_state(0, xyz)
+    forcing = None
+    if forced:
+        rng = np.random.default_rng(5)
+        forcing = dict(T_eq=300 + rng.uniform(-20, 20, size=state[0].shape),
+                       k_T=np.full(state[0].shape, 1e-5), k_v=np.full(state[0].shape, 2e-5))
+    m0, e0 = G.diagnostics(*state)
+    new = G.step(*state, 5, cfg["dt"], cfg["n_sub"], forcing)
+    m1, e1 = G.diagnostics(*new)
+    assert abs(m1 - m0) < 1e-14 * m0
+    # closed form of the initial mass: sum over layers of rho * shell weight; rho is known
+    assert abs(m0 - np.sum(state[0] * G.Ac[:, None] * (G.r_c ** 2 * G.dz)[None, :])) < 1e-12 * m0
+    if not forced:                                                    # P15 (soft)
+        assert abs(e1 - e0) < 1e-6 * abs(e0)
+
+
+# ------------------------------------------------------------------------- slow-term closed forms
+def test_p13_coriolis_closed_form_and_no_work(ogrid):
+    cfg = ti.CONFIGS[0]
+    xyz, nbr, C = ogrid(3, True)
+    nv = 4
+    rot = dict(cfg["planet"])
+    norot = dict(cfg["planet"], omega=0.0)
+    G1, G0 = oracle.Geometry(xyz, nbr, nv, rot, C), oracle.Geometry(xyz, nbr, nv, norot, C)
+    rng = np.random.default_rng(13)
+    rho, V, W, p = ti.rest_state(rot, nv, G1.N, 1e5, 300.0)
+    vel = rng.uniform(-10, 10, size=V.shape)
+    vel -= np.sum(vel * xyz[:, None, :], axis=-1, keepdims=True) * xyz[:, None, :]
+    V = rho[..., None] * vel
+    s1, s0 = G1.slow_terms(rho, V, W, p), G0.slow_terms(rho, V, W, p)
+    Ch = -(s1["slowV"] - s0["slowV"])                      # horizontal Coriolis term C_h
+    f = 2 * rot["omega"] * xyz[:, 2]                       # 2 Omega sin(lat)
+    expect = f[:, None, None] * np.cross(np.broadcast_to(xyz[:, None, :], V.shape), V)
+    assert np.abs(Ch - expect).max() < 1e-12 * np.abs(expect).max()
+    assert np.abs(np.sum(Ch * V, axis=-1)).max() < 1e-12 * np.abs(expect).max() * np.abs(V).max()
+    # radial part: C_r = 2 Omega (z x V).r, averaged to interfaces, enters S_vr with a minus sign
+    Cr = 2 * rot["omega"] * (-V[..., 1] * xyz[:, None, 0] + V[..., 0] * xyz[:, None, 1])
+    dS = -(s1["Svr"] - s0["Svr"])[:, 1:nv]
+    assert np.abs(dS - 0.5 * (Cr[:, :-1] + Cr[:, 1:])).max() < 1e-12 * np.abs(Cr).max()
+
+
+def test_advection_of_solid_body_rotation_is_centripetal(ogrid):
+    """For u = w x r with rho = rho(r): div(rho u u) = rho w x (w x r) exactly, i.e.
+    A = -rho w^2 s s_hat (s = distance from the axis).  The discrete A (reading R7) must converge
+    to it at second order; its horizontal part shows up in slowV, its radial part in S_vr."""
+    cfg = ti.CONFIGS[0]
+    planet = dict(cfg["planet"], omega=0.0, gravity=0.0)
+    errs = []
+    wrot = 2e-5
+    for lvl in (2, 3):
+        xyz, nbr, C = ogrid(lvl, True)
+        nv = 4
+        G = oracle.Geometry(xyz, nbr, nv, planet, C)
+        rho = np.tile(1.2 * np.exp(-G.z_c / 8000.0), (G.N, 1))
+        p = np.full((G.N, nv), 1e5)                        # uniform p, g = 0: no other force
+        r = G.r_c[None, :, None] * xyz[:, None, :]
+        u = wrot * np.stack([-r[..., 1], r[..., 0], np.zeros_like(r[..., 0])], axis=-1)
+        V = rho[..., None] * u
+        W = np.zeros((G.N, nv + 1))
+        st = G.slow_terms(rho, V, W, p)
+        A_exact = -rho[..., None] * wrot ** 2 * np.stack([r[..., 0], r[..., 1], np.zeros_like(r[..., 0])], axis=-1)
+        Ar = np.sum(A_exact * xyz[:, None, :], axis=-1)
+        Ah = A_exact - Ar[..., None] * xyz[:, None, :]
+        scale = np.abs(A_exact).max()
+        wgt = (G.Ac / G.Ac.sum())[:, None]
+        d_h = np.linalg.norm(-st["slowV"] - Ah, axis=-1) / scale
+        d_r = np.abs(-st["Svr"][:, 1:nv] - 0.5 * (Ar[:, :-1] + Ar[:, 1:])) / scale
+        errs.append((math.sqrt(np.sum(wgt * d_h ** 2)), math.sqrt(np.sum(wgt * d_r ** 2)), d_h.max(), d_r.max()))
+        # mass tendency of a divergence-free flow: second-order small
+        assert np.abs(st["slowrho"]).max() < 0.05 * np.abs(rho * wrot).max()
+    # l2 (Eq. 17) second order; l_inf slower (hexagons next to the pentagons), as in L154
+    assert errs[1][0] < 0.35 * errs[0][0] and errs[1][0] < 0.005
+    assert errs[1][1] < 0.35 * errs[0][1] and errs[1][1] < 0.005
+    assert errs[1][2] < 0.7 * errs[0][2] and errs[1][3] < 0.7 * errs[0][3]
+
+
+def test_pressure_and_entropy_tendencies_are_consistent(ogrid):
+    """dp/dt = (gamma p / (rho theta)) d(rho theta)/dt (Eq. 24): the slow part of the pressure
+    equation (Eq. 40 with the signs of G10) and of Eq. 35 discretise the same quantity; their
+    mismatch is a truncation error that shrinks with resolution, for a smooth state."""
+    cfg = ti.CONFIGS[0]
+    planet = dict(cfg["planet"])
+    gam = planet["Cp"] / (planet["Cp"] - planet["Rd"])
+    mism = []
+    for lvl, nv in ((2, 8), (3, 16)):
+        xyz, nbr, C = ogrid(lvl, True)
+        G = oracle.Geometry(xyz, nbr, nv, planet, C)
+        x, y, z = xyz[:, 0:1], xyz[:, 1:2], xyz[:, 2:3]
+        zc = G.z_c[None, :]
+        T = 280.0 + 15.0 * x * y + 10.0 * z - 3e-4 * zc
+        p = 1e5 * np.exp(-zc / 8000.0) * (1 + 0.01 * (x - 0.5 * z * y))
+        rho = p / (planet["Rd"] * T)
+        hr = ti.heikes_randall_fields(xyz, 1, 1)
+        vel = 20.0 * hr["v"][:, None, :] * (1 + zc[..., None] / 36e3)
+        V = rho[..., None] * vel
+        W = np.zeros((G.N, nv + 1))
+        W[:, 1:nv] = 0.02 * (0.5 * (rho[:, 1:] + rho[:, :-1])) * (x + z) * np.sin(np.pi * G.r_h[None, 1:nv] / 1.0 % 1.0 * 0 + np.pi * np.arange(1, nv)[None, :] / nv)
+        st = G.slow_terms(rho, V, W, p)
+        rt = planet["p_ref"] / planet["Rd"] * (p / planet["p_ref"]) ** (1 / gam)
+        lhs = st["slowp"]
+        rhs = gam * p / rt * st["slowrt"]
+        mism.append(np.abs(lhs - rhs)[:, 1:-1].max() / np.abs(rhs).max())
+    assert mism[1] < 0.5 * mism[0] and mism[1] < 0.05, mism
+
+
+def test_vertical_slow_term_is_second_order_hydrostatic_residual(ogrid):
+    """S_vr of an analytic hydrostatic isothermal column is an O(dz^2) residual (Eq. 42)."""
+    cfg = ti.CONFIGS[0]
+    planet = dict(cfg["planet"], omega=0.0)
+    xyz, nbr, C = ogrid(1, True)
+    res = []
+    for nv in (16, 32):
+        G = oracle.Geometry(xyz, nbr, nv, planet, C)
+        H = 287.0 * 300.0 / 9.8
+        p = np.tile(1e5 * np.exp(-G.z_c / H), (G.N, 1))
+        rho = p / (287.0 * 300.0)
+        st = G.slow_terms(rho, np.zeros((G.N, nv, 3)), np.zeros((G.N, nv + 1)), p)
+        res.append(np.abs(st["Svr"][:, 1:nv]).max())
+        assert np.all(st["slowV"] == 0.0)
+    assert 3.5 < res[0] / res[1] < 4.5
+
+
+# ------------------------------------------------------------------------------------------ P14
+def test_p14_rk3_split_explicit_is_second_order_in_dt(ogrid):
+    cfg = ti.CONFIGS[0]
+    xyz, nbr, C = ogrid(2, True)
+    nv = 6
+    planet = cfg["planet"]
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1e5, 300.0)
+    x, y, z = xyz[:, 0:1], xyz[:, 1:2], xyz[:, 2:3]
+    T = 300.0 * (1 + 0.01 * x * z + 0.005 * y)               # smooth warm anomaly drives a flow
+    rho = p / (287.0 * T)
+    Ttot, n = 3600.0, 4
+    ref = G.step(rho, V, W, p, 16, Ttot / 16, n)
+    e = []
+    for k in (2, 4):
+        out = G.step(rho, V, W, p, k, Ttot / k, n)
+        e.append(max(np.abs(out[1] - ref[1]).max() / np.abs(ref[1]).max(),
+                     np.abs(out[3] - ref[3]).max() / np.abs(ref[3] - p).max()))
+    assert e[1] < 0.45 * e[0], e                               # ~4x per halving (second order, L243)
+
+
+# ------------------------------------------------------------------------------------- forcing R9
+def test_forcing_limits(ogrid):
+    cfg = ti.CONFIGS[0]
+    xyz, nbr, C = ogrid(2, True)
+    nv = cfg["nv"]
+    G = oracle.Geometry(xyz, nbr, nv, cfg["planet"], C)
+    rho, V, W, p = ti.rest_state(cfg["planet"], nv, G.N, 1e5, 300.0)
+    shape = rho.shape
+    # k = 0: nothing happens; T_eq = T: nothing happens
+    for F in (dict(T_eq=np.full(shape, 250.0), k_T=np.zeros(shape), k_v=np.zeros(shape)),
+              dict(T_eq=np.full(shape, 300.0), k_T=np.full(shape, 1e-3), k_v=np.full(shape, 1e-3))):
+        out = G.step(rho, V, W, p, 1, 600.0, 2, F)
+        assert np.abs(out[3] - p).max() < 1e-9 and np.abs(out[0] - rho).max() < 1e-15
+    # k -> infinity: T -> T_eq exactly, rho untouched (L200), p = rho Rd T_eq
+    Teq = 250.0 + 10 * xyz[:, 2:3] * np.ones(shape)
+    out = G.step(rho, V, W, p, 1, 600.0, 2, dict(T_eq=Teq, k_T=np.full(shape, 1e12), k_v=None))
+    assert np.abs(out[3] / (out[0] * 287.0) - Teq).max() < 1e-6
+    # Rayleigh drag divides the horizontal momentum by (1 + k dt) and leaves W alone (Eq. 51)
+    state = ti.initial_state(0, ogrid(2, True)[0])
+    a = G.step(*state, 1, 600.0, 2, None)
+    b = G.step(*state, 1, 600.0, 2, dict(T_eq=None, k_T=None, k_v=np.full(shape, 1e-3)))
+    assert np.abs(b[1] * 1.6 - a[1]).max() < 1e-12 * np.abs(a[1]).max()
+    assert np.array_equal(a[2], b[2]) and np.array_equal(a[0], b[0]) and np.array_equal(a[3], b[3])
