@@ -1,0 +1,132 @@
+/*
+ * thor.h -- C-ABI boundary of the B200-native THOR HE-VI hot path (arXiv 1607.05535).
+ *
+ * One FP64 large time step of the horizontally-explicit / vertically-implicit split-explicit
+ * integrator (Fig. 6) on a spring-smoothed icosahedral grid (L43-L125), the
+ * PROFX forcing (Eq. 51-52) and the conserved diagnostics (L190, L200, L339).
+ * Citations are PAPER.md:L<line> + equation; R-n / G-n are the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns THOR_OK (0) or a negative code; nothing is written to outputs on
+ *    failure; no exception crosses the boundary; thor_last_error() gives the message of the last
+ *    failure on the calling thread.
+ *  - Unless a parameter is marked DEVICE, pointers are HOST pointers.  The caller owns every array
+ *    it passes in or receives results in; the library copies.  Opaque handles are owned by the
+ *    caller and released with the matching _destroy.
+ *  - Arrays at the boundary are FP64, C-contiguous, in CANONICAL column order (the grid
+ *    generator's numbering), layer index fastest:
+ *        rho, p, T_eq, k_T, k_v : [n_cols][n_layers]        at layer centres
+ *        mom_h = rho v_h        : [n_cols][n_layers][3]     Cartesian, tangent to the sphere
+ *        W     = rho v_r        : [n_cols][n_layers+1]      on layer interfaces, index 0 = bottom;
+ *                                 both ends are the rigid lid (L339) and are forced to 0.
+ *    The device keeps a different, locality-preserving column order; it is internal
+ *    (thor_grid_view.device_order documents it for the *_device entry points).
+ *  - Layers are uniform in altitude: dz = z_top / n_layers, centre k at (k+1/2) dz (R6).
+ *  - thor_step and thor_acoustic_substeps are asynchronous on the stream given to thor_state_init;
+ *    thor_state_get, thor_state_set and thor_diagnostics synchronise that stream.
+ *  - The library never falls back to the CPU: without a usable CUDA device every device entry
+ *    point returns THOR_ECUDA.  thor_grid_create / thor_grid_get are host-only and need no GPU.
+ */
+#ifndef THOR_H_
+#define THOR_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define THOR_OK      0
+#define THOR_EINVAL (-1)  /* null pointer, level < 0 or > 9, n_layers < 2 or > 128, dt <= 0, odd or < 2 substep count */
+#define THOR_ENOMEM (-2)
+#define THOR_ECUDA  (-3)  /* CUDA runtime failure or no device */
+
+/* Planet and domain (Table 1; p_ref L213; model top L454).  SI units. */
+typedef struct {
+    double radius;   /* A, m */
+    double omega;    /* rotation rate about the axis through the two polar vertices (L45), 1/s */
+    double gravity;  /* constant, radial (L184; R11), m/s^2 */
+    double Rd;       /* gas constant, J/kg/K */
+    double Cp;       /* specific heat at constant pressure, J/kg/K */
+    double p_ref;    /* reference pressure of Eq. 24, Pa */
+    double z_top;    /* altitude of the rigid lid, m */
+} thor_planet;
+
+typedef struct thor_grid thor_grid;    /* host geometry (+ device copy, made on first device use) */
+typedef struct thor_state thor_state;  /* device prognostics, stage arrays and work space */
+
+/* Read-only view of the generated grid; pointers are owned by the grid and live as long as it. */
+typedef struct {
+    int level, n_cols, n_layers;
+    const double *xyz;          /* [n_cols][3] unit-sphere positions P_i after spring dynamics and centroid move */
+    const int *nbr;             /* [n_cols][6] neighbours, counter-clockwise seen from outside; pentagons: nbr[5] = -1 */
+    const double *cv_vertex;    /* [n_cols][6][3] control-volume vertices C_k (Fig. 2); C_k belongs to the triangle
+                                   (P_0, P_nbr[k], P_nbr[k+1]); fixed while P moves (L120) */
+    const double *area;         /* [n_cols] unit-sphere control-volume areas A_c (sum = 4 pi) */
+    const double *edge_len;     /* [n_cols][6] geodesic arc C_k..C_k+1, l_k of Eq. 4 */
+    const double *edge_nrm;     /* [n_cols][6][3] outward unit normal of that arc, n_k of Eq. 4 */
+    const int *device_order;    /* [n_cols] canonical index of the column stored at device slot d */
+    int spring_iterations;      /* total spring-dynamics steps taken by the generator (all levels) */
+} thor_grid_view;
+
+/* PROFX tables (Eq. 51-52; R9: fixed in time).  Any pointer may be NULL = that term is off
+ * (Newtonian relaxation needs both T_eq and k_T).  resident != 0: reuse the tables uploaded by
+ * the previous thor_step call on this state (no host read, no copy). */
+typedef struct {
+    const double *T_eq;  /* K   */
+    const double *k_T;   /* 1/s */
+    const double *k_v;   /* 1/s */
+    int resident;
+} thor_forcing;
+
+typedef struct { double total_mass, total_energy; } thor_diag;
+
+/* Grid (L43-L125): icosahedron with two polar vertices -> `level` edge bisections (Eq. 1:
+ * n_cols = 10*4^level + 2) -> spring dynamics (Eq. 10-12, beta = 1.15) -> centroid move (Eq. 13);
+ * then the finite-volume stencil weights of Eq. 4-7 and the device column order.  Host only. */
+int thor_grid_create(int level, int n_layers, const thor_planet *planet, thor_grid **out);
+int thor_grid_get(const thor_grid *grid, thor_grid_view *out);
+void thor_grid_destroy(thor_grid *grid);
+
+/* State: uploads the four prognostic fields (L333) and allocates all stage/work arrays on the
+ * current CUDA device.  cuda_stream is a cudaStream_t (NULL = default stream). */
+int thor_state_init(const thor_grid *grid, const double *rho, const double *mom_h, const double *W,
+                    const double *p, void *cuda_stream, thor_state **out);
+int thor_state_set(thor_state *state, const double *rho, const double *mom_h, const double *W, const double *p);
+int thor_state_get(const thor_state *state, double *rho, double *mom_h, double *W, double *p);
+void thor_state_destroy(thor_state *state);
+
+/* n_large large steps of Fig. 6 (L301-L337): per step three Runge-Kutta stages (Eq. 30) of
+ * slow terms (RHS of Eq. 32-35, 42) + 1, n/2, n acoustic substeps (Eq. 33, 37, 32, 35, 36; L252),
+ * then the forcing (NULL = none) with the large step dt (L385).  n_acoustic_substeps = n, even, >= 2. */
+int thor_step(thor_state *state, int n_large, double dt, int n_acoustic_substeps, const thor_forcing *forcing);
+
+/* Only the hot loop: n_substeps acoustic substeps (steps a4-a9 of DESIGN.md) of length delta on the
+ * stage data left by the last thor_step.  which: 1 = explicit horizontal momentum kernel only,
+ * 2 = divergence + column-solve kernel only, 3 = both.  For measurement; the state it leaves is
+ * not a physical one. */
+int thor_acoustic_substeps(thor_state *state, int n_substeps, double delta, int which);
+
+/* Total mass sum(rho A_c r_k^2 dz) and total energy sum((Cv p/Rd + |rho v|^2/(2 rho) + rho g z) A_c r_k^2 dz) (R10). */
+int thor_diagnostics(const thor_state *state, thor_diag *out);
+
+/* Config-1 operators at radius r_k (unit-sphere operator / r_k): Eq. 6 divergence of vec
+ * [n_cols][n_layers][3] -> out [n_cols][n_layers]; Eq. 7 gradient (difference form, projected with
+ * Eq. 28) of s [n_cols][n_layers] -> out [n_cols][n_layers][3].  Host arrays, canonical order. */
+int thor_apply_div(const thor_grid *grid, const double *vec, double *out);
+int thor_apply_grad(const thor_grid *grid, const double *s, double *out);
+
+/* The same two kernels on DEVICE arrays already in device column order, component-separated:
+ * each pointer is a DEVICE [n_cols][n_layers] array.  Asynchronous on cuda_stream. */
+int thor_apply_div_device(const thor_grid *grid, const double *vx, const double *vy, const double *vz,
+                          double *out, void *cuda_stream);
+int thor_apply_grad_device(const thor_grid *grid, const double *s, double *gx, double *gy, double *gz,
+                           void *cuda_stream);
+
+/* Number of kernels this library has launched in the calling process so far. */
+long long thor_launch_count(void);
+
+const char *thor_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* THOR_H_ */

@@ -1,0 +1,361 @@
+// Host icosahedral grid generator + finite-volume stencil weights.
+//
+//   icosahedron, two vertices on the poles
+//   -> recursive edge bisection, new points projected to the unit sphere (L45-L49, Fig. 1)
+//   -> spring dynamics (Eq. 10-12; beta = 1.15, alpha = 1, k = 1 (G2), dt = 0.01)
+//   -> centroid move (Eq. 13 with reading G4, L120-L125): C_k to the triangle centroids, then,
+//      C fixed, P_i to the centroid of its control volume
+//   -> stencil weights of Eq. 4-7 expanded per neighbour, device column order.
+//
+// Design choices that differ from a literal reading ("grid generator"):
+//   * The relaxation is hierarchical: every refinement level is relaxed before it is bisected
+//     again, so the finer level starts next to its equilibrium and only its short wavelengths
+//     have to decay.  The equilibrium of Eq. 10 does not depend on where the iteration starts.
+//   * G3: the paper's stopping test (no point moves more than 1e-5 in a step) is met by the very
+//     first step of a grid that starts at rest; here the iteration runs until the largest
+//     per-step displacement stays below kSpringTol after the initial transient.
+#include "grid_host.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <unordered_map>
+
+namespace thor {
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kBeta = 1.15;       // L118
+constexpr double kAlpha = 1.0;       // L118
+constexpr double kSpringK = 1.0;     // G2
+constexpr double kSpringDt = 0.01;   // L118
+constexpr double kSpringTol = 1e-9;  // G3 (per-step displacement on the unit sphere)
+constexpr double kSpringTolGrowth = 4.0;   // per level above 4; measured: no effect on the operator errors
+constexpr int kSpringMinIter = 200;
+constexpr int kSpringMaxIter = 60000;
+
+struct V3 {
+    double x, y, z;
+};
+inline V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline V3 operator*(double s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+inline double dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline V3 cross(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
+inline double norm(V3 a) { return std::sqrt(dot(a, a)); }
+inline V3 unit(V3 a) { return (1.0 / norm(a)) * a; }
+inline double arc(V3 a, V3 b) { return std::atan2(norm(cross(a, b)), dot(a, b)); }
+
+struct Tri {
+    int a, b, c;
+};
+
+void icosahedron(std::vector<V3>& pts, std::vector<Tri>& tris) {
+    const double lat = std::atan(0.5);
+    pts.clear();
+    tris.clear();
+    pts.push_back({0, 0, 1});
+    for (int j = 0; j < 5; ++j) {
+        double lon = 2 * kPi * j / 5;
+        pts.push_back({std::cos(lat) * std::cos(lon), std::cos(lat) * std::sin(lon), std::sin(lat)});
+    }
+    for (int j = 0; j < 5; ++j) {
+        double lon = 2 * kPi * (j + 0.5) / 5;
+        pts.push_back({std::cos(lat) * std::cos(lon), std::cos(lat) * std::sin(lon), -std::sin(lat)});
+    }
+    pts.push_back({0, 0, -1});
+    // five north-to-south strips of four faces; counter-clockwise seen from outside
+    for (int j = 0; j < 5; ++j) {
+        int u0 = 1 + j, u1 = 1 + (j + 1) % 5, l0 = 6 + j, l1 = 6 + (j + 1) % 5;
+        tris.push_back({0, u0, u1});
+        tris.push_back({u0, l0, u1});
+        tris.push_back({u1, l0, l1});
+        tris.push_back({11, l1, l0});
+    }
+}
+
+// One refinement (L45): children of triangle t are stored at 4t..4t+3, so the triangle list stays
+// in quadtree (depth-first) order -- the device column order below relies on that.
+void bisect(std::vector<V3>& pts, std::vector<Tri>& tris) {
+    std::unordered_map<uint64_t, int> mid;
+    mid.reserve(tris.size() * 2);
+    auto midpoint = [&](int a, int b) {
+        uint64_t key = a < b ? (uint64_t(a) << 32) | uint32_t(b) : (uint64_t(b) << 32) | uint32_t(a);
+        auto it = mid.find(key);
+        if (it != mid.end()) return it->second;
+        int id = int(pts.size());
+        pts.push_back(unit(pts[a] + pts[b]));
+        mid.emplace(key, id);
+        return id;
+    };
+    std::vector<Tri> out;
+    out.reserve(tris.size() * 4);
+    for (const Tri& t : tris) {
+        int ab = midpoint(t.a, t.b), bc = midpoint(t.b, t.c), ca = midpoint(t.c, t.a);
+        out.push_back({t.a, ab, ca});
+        out.push_back({ab, bc, ca});   // centre child second: keeps consecutive children adjacent
+        out.push_back({ab, t.b, bc});
+        out.push_back({ca, bc, t.c});
+    }
+    tris.swap(out);
+}
+
+// Neighbours of every vertex in counter-clockwise order (seen from outside), starting from the
+// smallest neighbour index; pentagons are padded with -1.
+bool neighbour_table(int N, const std::vector<Tri>& tris, std::vector<int>& nbr, std::vector<int>& deg) {
+    std::vector<int> from(size_t(N) * 6, -1), to(size_t(N) * 6, -1), cnt(N, 0);
+    auto add = [&](int v, int a, int b) {
+        if (cnt[v] >= 6) return false;
+        from[size_t(v) * 6 + cnt[v]] = a;
+        to[size_t(v) * 6 + cnt[v]] = b;
+        ++cnt[v];
+        return true;
+    };
+    for (const Tri& t : tris)
+        if (!add(t.a, t.b, t.c) || !add(t.b, t.c, t.a) || !add(t.c, t.a, t.b)) return false;
+    nbr.assign(size_t(N) * 6, -1);
+    deg.assign(N, 0);
+    for (int v = 0; v < N; ++v) {
+        int m = cnt[v];
+        if (m != 5 && m != 6) return false;
+        const int* f = &from[size_t(v) * 6];
+        const int* t = &to[size_t(v) * 6];
+        int cur = *std::min_element(f, f + m);
+        for (int k = 0; k < m; ++k) {
+            nbr[size_t(v) * 6 + k] = cur;
+            int nxt = -1;
+            for (int q = 0; q < m; ++q)
+                if (f[q] == cur) nxt = t[q];
+            if (nxt < 0) return false;
+            cur = nxt;
+        }
+        deg[v] = m;
+    }
+    return true;
+}
+
+// Eq. 10-12.  Returns the number of steps taken.
+int spring_dynamics(std::vector<V3>& x, const std::vector<int>& nbr, const std::vector<int>& deg, int level) {
+    const int N = int(x.size());
+    const double dspr = kBeta * 2 * kPi / (10.0 * std::pow(2.0, level - 1));   // Eq. 12, A = 1
+    std::vector<V3> v(N, V3{0, 0, 0}), xn(N);
+    // the tolerance follows the grid spacing above level 4 (a fixed displacement is a smaller and
+    // smaller fraction of an edge there, and the long waves were already relaxed on the coarser levels)
+    const double tol = kSpringTol * std::pow(kSpringTolGrowth, std::max(0, level - 4));
+    int it = 0;
+    for (; it < kSpringMaxIter; ++it) {
+        double worst = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : worst)
+        for (int i = 0; i < N; ++i) {
+            if (deg[i] == 5) {   // the twelve pentagon centres stay fixed (L109)
+                xn[i] = x[i];
+                continue;
+            }
+            const V3 p0 = x[i];
+            V3 f{0, 0, 0};
+            for (int k = 0; k < 6; ++k) {
+                const V3 pj = x[nbr[size_t(i) * 6 + k]];
+                double d = arc(p0, pj);
+                V3 e = unit(pj - dot(pj, p0) * p0);               // unit tangent at P_0 towards P_j
+                f = f + (kSpringK * (d - dspr)) * e;
+            }
+            f = f - kAlpha * v[i];                                // Eq. 10
+            V3 vi = v[i] + kSpringDt * f;
+            V3 pn = unit(p0 + kSpringDt * vi);                    // Eq. 11, back onto the sphere
+            v[i] = vi - dot(vi, pn) * pn;
+            xn[i] = pn;
+            worst = std::max(worst, norm(pn - p0));
+        }
+        x.swap(xn);
+        if (it >= kSpringMinIter && worst < tol) {
+            ++it;
+            break;
+        }
+    }
+    return it;
+}
+
+// Eq. 13 (G4): sum_i (r_i x r_i+1)/|r_i x r_i+1| * arc(r_i, r_i+1), normalised.
+V3 centroid(const V3* r, int n) {
+    V3 s{0, 0, 0};
+    for (int i = 0; i < n; ++i) {
+        V3 c = cross(r[i], r[(i + 1) % n]);
+        double l = norm(c);
+        s = s + (std::atan2(l, dot(r[i], r[(i + 1) % n])) / l) * c;
+    }
+    return unit(s);
+}
+
+double tri_area(V3 a, V3 b, V3 c) {   // spherical excess
+    return 2.0 * std::atan2(std::fabs(dot(a, cross(b, c))), 1.0 + dot(a, b) + dot(b, c) + dot(c, a));
+}
+
+}  // namespace
+
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
+    if (level < 0 || level > 9 || nv < 2 || nv > 128) return THOR_EINVAL;
+    if (!(P.radius > 0) || !(P.z_top > 0) || !(P.Rd > 0) || !(P.Cp > P.Rd) || !(P.p_ref > 0)) return THOR_EINVAL;
+    g.level = level;
+    g.nv = nv;
+    g.P = P;
+
+    std::vector<V3> pts;
+    std::vector<Tri> tris;
+    std::vector<int> nbr, deg;
+    icosahedron(pts, tris);
+    g.spring_iterations = 0;
+    for (int l = 1; l <= level; ++l) {
+        bisect(pts, tris);
+        if (!neighbour_table(int(pts.size()), tris, nbr, deg)) return THOR_EINVAL;
+        g.spring_iterations += spring_dynamics(pts, nbr, deg, l);
+    }
+    if (level == 0 && !neighbour_table(int(pts.size()), tris, nbr, deg)) return THOR_EINVAL;
+    const int N = int(pts.size());
+    g.N = N;
+    g.nbr = nbr;
+    g.deg = deg;
+
+    // --- centroid move (L120).  One C per triangle, shared bit-identically by its three columns.
+    const int T = int(tris.size());
+    std::vector<V3> Ctri(T);
+    for (int t = 0; t < T; ++t) {
+        V3 r[3] = {pts[tris[t].a], pts[tris[t].b], pts[tris[t].c]};
+        Ctri[t] = centroid(r, 3);
+    }
+    // corner k of column i = the triangle (i, nbr[k], nbr[k+1]); find it through an edge map
+    std::unordered_map<uint64_t, int> tri_of_edge;   // directed edge (a -> b) -> triangle on its left
+    tri_of_edge.reserve(size_t(T) * 3);
+    auto ekey = [](int a, int b) { return (uint64_t(uint32_t(a)) << 32) | uint32_t(b); };
+    for (int t = 0; t < T; ++t) {
+        tri_of_edge[ekey(tris[t].a, tris[t].b)] = t;
+        tri_of_edge[ekey(tris[t].b, tris[t].c)] = t;
+        tri_of_edge[ekey(tris[t].c, tris[t].a)] = t;
+    }
+    std::vector<int> corner_tri(size_t(N) * 6, -1);
+    g.cv.assign(size_t(N) * 18, 0.0);
+    for (int i = 0; i < N; ++i)
+        for (int k = 0; k < deg[i]; ++k) {
+            auto it = tri_of_edge.find(ekey(i, nbr[size_t(i) * 6 + k]));
+            if (it == tri_of_edge.end()) return THOR_EINVAL;
+            corner_tri[size_t(i) * 6 + k] = it->second;
+            const V3 c = Ctri[it->second];
+            double* o = &g.cv[size_t(i) * 18 + 3 * k];
+            o[0] = c.x; o[1] = c.y; o[2] = c.z;
+        }
+    if (level > 0) {
+        std::vector<V3> moved(N);
+        for (int i = 0; i < N; ++i) {
+            V3 poly[6];
+            for (int k = 0; k < deg[i]; ++k) poly[k] = Ctri[corner_tri[size_t(i) * 6 + k]];
+            moved[i] = centroid(poly, deg[i]);
+        }
+        pts.swap(moved);
+    }
+    g.xyz.resize(size_t(N) * 3);
+    for (int i = 0; i < N; ++i) { g.xyz[3 * i] = pts[i].x; g.xyz[3 * i + 1] = pts[i].y; g.xyz[3 * i + 2] = pts[i].z; }
+
+    // --- Eq. 5 weights per triangle (vertex order of the triangle list), from the FINAL P and the fixed C
+    std::vector<double> bary(size_t(T) * 3);
+    for (int t = 0; t < T; ++t) {
+        V3 a = pts[tris[t].a], b = pts[tris[t].b], c = pts[tris[t].c], C = Ctri[t];
+        double wa = tri_area(b, c, C), wb = tri_area(c, a, C), wc = tri_area(a, b, C);
+        double s = wa + wb + wc;
+        bary[size_t(t) * 3 + 0] = wa / s;   // each vertex is weighted by the sub-triangle opposite to it
+        bary[size_t(t) * 3 + 1] = wb / s;
+        bary[size_t(t) * 3 + 2] = wc / s;
+    }
+    auto weight_of = [&](int t, int v) {
+        if (tris[t].a == v) return bary[size_t(t) * 3 + 0];
+        if (tris[t].b == v) return bary[size_t(t) * 3 + 1];
+        return bary[size_t(t) * 3 + 2];
+    };
+
+    // --- device column order: first touch in quadtree order of the leaf triangles
+    g.order.assign(N, -1);
+    g.rank.assign(N, -1);
+    {
+        int next = 0;
+        auto touch = [&](int v) {
+            if (g.rank[v] < 0) { g.rank[v] = next; g.order[next] = v; ++next; }
+        };
+        for (const Tri& t : tris) { touch(t.a); touch(t.b); touch(t.c); }
+        if (next != N) return THOR_EINVAL;
+    }
+
+    // --- l_k, n_k, A_c (Eq. 4, 6) and the expanded stencil weights
+    g.area.assign(N, 0.0);
+    g.len.assign(size_t(N) * 6, 0.0);
+    g.nrm.assign(size_t(N) * 18, 0.0);
+    g.d_nbr.assign(size_t(N) * 6, 0);
+    g.d_wdiv.assign(size_t(N) * 21, 0.0);
+    g.d_wgrad.assign(size_t(N) * 18, 0.0);
+    g.d_rhat.assign(size_t(N) * 3, 0.0);
+    g.d_area.assign(N, 0.0);
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        const int m = deg[i];
+        const V3 p0 = pts[i];
+        V3 C[6], E[6], ln[6];
+        for (int k = 0; k < m; ++k) C[k] = Ctri[corner_tri[size_t(i) * 6 + k]];
+        double area = 0.0;
+        for (int k = 0; k < m; ++k) {
+            V3 c0 = C[k], c1 = C[(k + 1) % m];
+            V3 n = cross(c0, c1);
+            double l = arc(c0, c1);
+            V3 nh = (-1.0 / norm(n)) * n;                      // outward for counter-clockwise order
+            g.len[size_t(i) * 6 + k] = l;
+            g.nrm[size_t(i) * 18 + 3 * k + 0] = nh.x;
+            g.nrm[size_t(i) * 18 + 3 * k + 1] = nh.y;
+            g.nrm[size_t(i) * 18 + 3 * k + 2] = nh.z;
+            ln[k] = l * nh;
+            area += tri_area(p0, c0, c1);
+        }
+        g.area[i] = area;
+        // corner k sits on edges k-1 and k: Phi*_k is multiplied by E_k = (l_k-1 n_k-1 + l_k n_k)/2
+        for (int k = 0; k < m; ++k) E[k] = 0.5 * (ln[(k + m - 1) % m] + ln[k]);
+        V3 w[7];
+        for (int j = 0; j < 7; ++j) w[j] = V3{0, 0, 0};
+        for (int k = 0; k < m; ++k) {
+            int t = corner_tri[size_t(i) * 6 + k];
+            int na = nbr[size_t(i) * 6 + k], nb = nbr[size_t(i) * 6 + (k + 1) % m];
+            w[0] = w[0] + weight_of(t, i) * E[k];
+            w[1 + k] = w[1 + k] + weight_of(t, na) * E[k];
+            w[1 + (k + 1) % m] = w[1 + (k + 1) % m] + weight_of(t, nb) * E[k];
+        }
+        const int d = g.rank[i];
+        for (int j = 0; j < 7; ++j) {
+            V3 wj = (1.0 / area) * w[j];
+            g.d_wdiv[size_t(d) * 21 + 3 * j + 0] = wj.x;
+            g.d_wdiv[size_t(d) * 21 + 3 * j + 1] = wj.y;
+            g.d_wdiv[size_t(d) * 21 + 3 * j + 2] = wj.z;
+            if (j >= 1) {
+                V3 gj = wj - dot(wj, p0) * p0;                  // Eq. 28 (G5): tangential part
+                g.d_wgrad[size_t(d) * 18 + 3 * (j - 1) + 0] = gj.x;
+                g.d_wgrad[size_t(d) * 18 + 3 * (j - 1) + 1] = gj.y;
+                g.d_wgrad[size_t(d) * 18 + 3 * (j - 1) + 2] = gj.z;
+            }
+        }
+        for (int k = 0; k < 6; ++k) g.d_nbr[size_t(d) * 6 + k] = k < m ? g.rank[nbr[size_t(i) * 6 + k]] : d;
+        g.d_rhat[size_t(d) * 3 + 0] = p0.x;
+        g.d_rhat[size_t(d) * 3 + 1] = p0.y;
+        g.d_rhat[size_t(d) * 3 + 2] = p0.z;
+        g.d_area[d] = area;
+    }
+
+    // --- vertical tables (R6: uniform dz; Eq. 27's radial operator)
+    g.dz = P.z_top / nv;
+    g.rinv.resize(nv); g.dlo.resize(nv); g.dhi.resize(nv); g.vol.resize(nv); g.zc.resize(nv);
+    for (int k = 0; k < nv; ++k) {
+        double zc = (k + 0.5) * g.dz, rc = P.radius + zc;
+        double rl = P.radius + k * g.dz, ru = P.radius + (k + 1) * g.dz;
+        g.zc[k] = zc;
+        g.rinv[k] = 1.0 / rc;
+        g.dlo[k] = rl * rl / (rc * rc * g.dz);
+        g.dhi[k] = ru * ru / (rc * rc * g.dz);
+        g.vol[k] = rc * rc * g.dz;
+    }
+    return THOR_OK;
+}
+
+}  // namespace thor

@@ -1,0 +1,42 @@
+// Host-side icosahedral grid generator and finite-volume stencil weights (PAPER.md:L43-L125,
+// Eq. 1-13).  Internal to the library; the C-ABI in include/thor.h exposes it as thor_grid_*.
+#pragma once
+#include <vector>
+
+#include "thor.h"
+
+namespace thor {
+
+struct HostGrid {
+    int level = 0, N = 0, nv = 0;
+    thor_planet P{};
+    int spring_iterations = 0;
+    // canonical order (the generator's numbering)
+    std::vector<double> xyz;       // [N][3]
+    std::vector<int> nbr;          // [N][6], -1 pads pentagons
+    std::vector<int> deg;          // [N]
+    std::vector<double> cv;        // [N][6][3] control-volume vertices C_k
+    std::vector<double> area;      // [N]
+    std::vector<double> len;       // [N][6]
+    std::vector<double> nrm;       // [N][6][3]
+    std::vector<int> order;        // [N] device slot -> canonical index
+    std::vector<int> rank;         // [N] canonical index -> device slot
+    // device order, ready to upload
+    std::vector<int> d_nbr;        // [N][6] device slots of the neighbours; pentagons: slot 5 = self
+    std::vector<double> d_wdiv;    // [N][7][3] div_i = sum_j wdiv[j] . Phi_j   (j = 0 self, 1..6 neighbours)
+    std::vector<double> d_wgrad;   // [N][6][3] grad_i = sum_j wgrad[j] (s_j - s_i), already tangent (Eq. 28)
+    std::vector<double> d_rhat;    // [N][3]
+    std::vector<double> d_area;    // [N]
+    // per-layer tables
+    std::vector<double> rinv;      // [nv] 1/r_k
+    std::vector<double> dlo;       // [nv] r_h,k^2   / (r_k^2 dz)
+    std::vector<double> dhi;       // [nv] r_h,k+1^2 / (r_k^2 dz)
+    std::vector<double> vol;       // [nv] r_k^2 dz
+    std::vector<double> zc;        // [nv] centre altitude
+    double dz = 0;
+};
+
+// Builds everything above.  Returns THOR_OK or THOR_EINVAL / THOR_ENOMEM.
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g);
+
+}  // namespace thor

@@ -1,0 +1,474 @@
+// C-ABI of include/thor.h: argument checks, device memory, the launch sequence of one large
+// step (Fig. 6).  Every step of the path runs in the kernels of
+// thor_kernels.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "grid_host.h"
+#include "thor.h"
+#include "thor_kernels.cuh"
+
+using namespace thor;
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(THOR_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
+    } while (0)
+
+struct DeviceGeom {
+    bool ready = false;
+    int device = -1;
+    int* nbr = nullptr;
+    int* order = nullptr;
+    double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
+    double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr;
+};
+
+}  // namespace
+
+struct thor_grid {
+    HostGrid h;
+    mutable DeviceGeom d;
+};
+
+struct thor_state {
+    const thor_grid* grid = nullptr;
+    cudaStream_t stream = nullptr;
+    Fields f{};
+    std::vector<double*> owned;      // every cudaMalloc'ed field
+    double* stage_buf = nullptr;     // canonical-order staging, max(N*nv*3, N*(nv+1)) doubles
+    double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;
+    bool has_Teq = false, has_kT = false, has_kv = false;
+    double *col_mass = nullptr, *col_energy = nullptr;
+    double last_delta = 0.0;
+    bool stepped = false;
+};
+
+namespace {
+
+template <class T>
+int upload(T** dst, const std::vector<T>& src) {
+    CU(cudaMalloc(reinterpret_cast<void**>(dst), src.size() * sizeof(T)));
+    CU(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return THOR_OK;
+}
+
+int ensure_device_geom(const thor_grid* grid) {
+    DeviceGeom& d = grid->d;
+    if (d.ready) return THOR_OK;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0)
+        return fail(THOR_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
+    CU(cudaGetDevice(&d.device));
+    const HostGrid& h = grid->h;
+    int rc;
+    if ((rc = upload(&d.nbr, h.d_nbr))) return rc;
+    if ((rc = upload(&d.order, h.order))) return rc;
+    if ((rc = upload(&d.wdiv, h.d_wdiv))) return rc;
+    if ((rc = upload(&d.wgrad, h.d_wgrad))) return rc;
+    if ((rc = upload(&d.rhat, h.d_rhat))) return rc;
+    if ((rc = upload(&d.area, h.d_area))) return rc;
+    if ((rc = upload(&d.rinv, h.rinv))) return rc;
+    if ((rc = upload(&d.dlo, h.dlo))) return rc;
+    if ((rc = upload(&d.dhi, h.dhi))) return rc;
+    if ((rc = upload(&d.vol, h.vol))) return rc;
+    if ((rc = upload(&d.zc, h.zc))) return rc;
+    d.ready = true;
+    return THOR_OK;
+}
+
+Geom make_geom(const thor_grid* grid) {
+    const HostGrid& h = grid->h;
+    const DeviceGeom& d = grid->d;
+    Geom g;
+    g.N = h.N; g.nv = h.nv;
+    g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
+    g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc;
+    g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
+    return g;
+}
+
+// lane-group width G and layers per lane E for a given layer count
+struct Shape { int G, E; };
+Shape shape_for(int nv) {
+    if (nv <= 8) return {8, 1};
+    if (nv <= 16) return {16, 1};
+    if (nv <= 32) return {32, 1};
+    if (nv <= 64) return {32, 2};
+    if (nv <= 96) return {32, 3};
+    return {32, 4};
+}
+int column_blocks(int N, int G) {
+    const int cols_per_block = kWarpsPerBlock * (32 / G);
+    return (N + cols_per_block - 1) / cols_per_block;
+}
+
+// dispatch a column kernel template over the supported (G, E) shapes
+#define THOR_DISPATCH(KERNEL, nv, N, stream, ...)                                                  \
+    do {                                                                                           \
+        const Shape sh_ = shape_for(nv);                                                           \
+        const dim3 grid_(column_blocks(N, sh_.G)), block_(kWarpsPerBlock * 32);                    \
+        if (sh_.G == 8) KERNEL<8, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                   \
+        else if (sh_.G == 16) KERNEL<16, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);            \
+        else if (sh_.E == 1) KERNEL<32, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
+        else if (sh_.E == 2) KERNEL<32, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
+        else if (sh_.E == 3) KERNEL<32, 3><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
+        else KERNEL<32, 4><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                             \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                                        \
+    } while (0)
+
+int flat_blocks(size_t n) { return int((n + 255) / 256); }
+
+// host canonical arrays -> device fields (through the staging buffer, permuted on the device)
+int upload_state(thor_state* s, const double* rho, const double* mom_h, const double* W, const double* p) {
+    const HostGrid& h = s->grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    const int* order = s->grid->d.order;
+    cudaStream_t st = s->stream;
+    auto gather = [&](const double* host, size_t count, int row_len, int cs, int c0, double* dst) -> int {
+        if (host) CU(cudaMemcpyAsync(s->stage_buf, host, count * sizeof(double), cudaMemcpyHostToDevice, st));
+        k_gather_rows<<<flat_blocks(nc), 256, 0, st>>>(N, nv, order, s->stage_buf, row_len, cs, c0, dst);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return THOR_OK;
+    };
+    int rc;
+    if ((rc = gather(rho, nc, nv, 1, 0, s->f.rho_n))) return rc;
+    if ((rc = gather(p, nc, nv, 1, 0, s->f.p_n))) return rc;
+    if ((rc = gather(mom_h, nc * 3, nv * 3, 3, 0, s->f.Vx_n))) return rc;
+    if ((rc = gather(nullptr, 0, nv * 3, 3, 1, s->f.Vy_n))) return rc;
+    if ((rc = gather(nullptr, 0, nv * 3, 3, 2, s->f.Vz_n))) return rc;
+    if ((rc = gather(W, size_t(N) * (nv + 1), nv + 1, 1, 0, s->f.W_n))) return rc;   // lower interfaces 0..nv-1
+    k_zero_ground<<<(N + 255) / 256, 256, 0, st>>>(N, nv, s->f.W_n);                 // rigid lid (L339)
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    return THOR_OK;
+}
+
+int upload_table(thor_state* s, const double* host, double** dev) {
+    const HostGrid& h = s->grid->h;
+    const size_t nc = size_t(h.N) * h.nv;
+    if (!*dev) {
+        CU(cudaMalloc(reinterpret_cast<void**>(dev), nc * sizeof(double)));
+    }
+    CU(cudaMemcpyAsync(s->stage_buf, host, nc * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    k_gather_rows<<<flat_blocks(nc), 256, 0, s->stream>>>(h.N, h.nv, s->grid->d.order, s->stage_buf, h.nv, 1, 0, *dev);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* thor_last_error(void) { return g_err.c_str(); }
+long long thor_launch_count(void) { return g_launches.load(); }
+
+int thor_grid_create(int level, int n_layers, const thor_planet* planet, thor_grid** out) {
+    if (!planet || !out) return fail(THOR_EINVAL, "thor_grid_create: null argument");
+    thor_grid* g = new (std::nothrow) thor_grid();
+    if (!g) return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
+    int rc;
+    try {
+        rc = build_host_grid(level, n_layers, *planet, g->h);
+    } catch (const std::bad_alloc&) {
+        delete g;
+        return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
+    }
+    if (rc != THOR_OK) {
+        delete g;
+        return fail(rc, "thor_grid_create: invalid level, layer count or planet parameters");
+    }
+    *out = g;
+    return THOR_OK;
+}
+
+int thor_grid_get(const thor_grid* grid, thor_grid_view* out) {
+    if (!grid || !out) return fail(THOR_EINVAL, "thor_grid_get: null argument");
+    const HostGrid& h = grid->h;
+    out->level = h.level; out->n_cols = h.N; out->n_layers = h.nv;
+    out->xyz = h.xyz.data(); out->nbr = h.nbr.data(); out->cv_vertex = h.cv.data();
+    out->area = h.area.data(); out->edge_len = h.len.data(); out->edge_nrm = h.nrm.data();
+    out->device_order = h.order.data();
+    out->spring_iterations = h.spring_iterations;
+    return THOR_OK;
+}
+
+void thor_grid_destroy(thor_grid* grid) {
+    if (!grid) return;
+    DeviceGeom& d = grid->d;
+    if (d.ready) {
+        cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
+        cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc);
+    }
+    delete grid;
+}
+
+void thor_state_destroy(thor_state* s) {
+    if (!s) return;
+    for (double* p : s->owned) cudaFree(p);
+    cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
+    cudaFree(s->col_mass); cudaFree(s->col_energy);
+    delete s;
+}
+
+int thor_state_init(const thor_grid* grid, const double* rho, const double* mom_h, const double* W,
+                    const double* p, void* cuda_stream, thor_state** out) {
+    if (!grid || !rho || !mom_h || !W || !p || !out) return fail(THOR_EINVAL, "thor_state_init: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    thor_state* s = new (std::nothrow) thor_state();
+    if (!s) return fail(THOR_ENOMEM, "thor_state_init: out of host memory");
+    s->grid = grid;
+    s->stream = static_cast<cudaStream_t>(cuda_stream);
+    const HostGrid& h = grid->h;
+    const size_t nc = size_t(h.N) * h.nv;
+    double** slots[] = {&s->f.rho_n, &s->f.Vx_n, &s->f.Vy_n, &s->f.Vz_n, &s->f.W_n, &s->f.p_n, &s->f.rt_n,
+                        &s->f.rho_t, &s->f.Vx_t, &s->f.Vy_t, &s->f.Vz_t, &s->f.W_t, &s->f.p_t,
+                        &s->f.h, &s->f.th, &s->f.ux, &s->f.uy, &s->f.uz, &s->f.fa, &s->f.fi, &s->f.fc,
+                        &s->f.sVx, &s->f.sVy, &s->f.sVz, &s->f.srho, &s->f.sW, &s->f.sp, &s->f.srt,
+                        &s->f.rho_s, &s->f.Vx_s, &s->f.Vy_s, &s->f.Vz_s, &s->f.W_s, &s->f.p_s, &s->f.rt};
+    for (double** slot : slots) {
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(slot), nc * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemsetAsync(*slot, 0, nc * sizeof(double), s->stream);
+        if (e != cudaSuccess) {
+            thor_state_destroy(s);
+            return fail(e == cudaErrorMemoryAllocation ? THOR_ENOMEM : THOR_ECUDA,
+                        std::string("thor_state_init: ") + cudaGetErrorString(e));
+        }
+        s->owned.push_back(*slot);
+    }
+    const size_t stage_n = std::max(nc * 3, size_t(h.N) * (h.nv + 1));
+    if (cudaMalloc(reinterpret_cast<void**>(&s->stage_buf), stage_n * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&s->col_mass), h.N * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(reinterpret_cast<void**>(&s->col_energy), h.N * sizeof(double)) != cudaSuccess) {
+        thor_state_destroy(s);
+        return fail(THOR_ENOMEM, "thor_state_init: out of device memory");
+    }
+    rc = upload_state(s, rho, mom_h, W, p);
+    if (rc) {
+        thor_state_destroy(s);
+        return rc;
+    }
+    *out = s;
+    return THOR_OK;
+}
+
+int thor_state_set(thor_state* s, const double* rho, const double* mom_h, const double* W, const double* p) {
+    if (!s || !rho || !mom_h || !W || !p) return fail(THOR_EINVAL, "thor_state_set: null argument");
+    return upload_state(s, rho, mom_h, W, p);
+}
+
+int thor_state_get(const thor_state* s, double* rho, double* mom_h, double* W, double* p) {
+    if (!s || !rho || !mom_h || !W || !p) return fail(THOR_EINVAL, "thor_state_get: null argument");
+    const HostGrid& h = s->grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    const int* order = s->grid->d.order;
+    cudaStream_t st = s->stream;
+    auto scatter = [&](const double* src, int row_len, int cs, int c0) {
+        k_scatter_rows<<<flat_blocks(nc), 256, 0, st>>>(N, nv, order, src, row_len, cs, c0, s->stage_buf);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    };
+    scatter(s->f.rho_n, nv, 1, 0);
+    CU(cudaMemcpyAsync(rho, s->stage_buf, nc * sizeof(double), cudaMemcpyDeviceToHost, st));
+    scatter(s->f.p_n, nv, 1, 0);
+    CU(cudaMemcpyAsync(p, s->stage_buf, nc * sizeof(double), cudaMemcpyDeviceToHost, st));
+    scatter(s->f.Vx_n, nv * 3, 3, 0);
+    scatter(s->f.Vy_n, nv * 3, 3, 1);
+    scatter(s->f.Vz_n, nv * 3, 3, 2);
+    CU(cudaMemcpyAsync(mom_h, s->stage_buf, nc * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    k_fill<<<flat_blocks(size_t(N) * (nv + 1)), 256, 0, st>>>(size_t(N) * (nv + 1), s->stage_buf, 0.0);   // lid = 0
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    scatter(s->f.W_n, nv + 1, 1, 0);
+    CU(cudaMemcpyAsync(W, s->stage_buf, size_t(N) * (nv + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    return THOR_OK;
+}
+
+int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* forcing) {
+    if (!s) return fail(THOR_EINVAL, "thor_step: null state");
+    if (n_large < 0 || !(dt > 0) || n < 2 || (n & 1)) return fail(THOR_EINVAL, "thor_step: need n_large >= 0, dt > 0, even n >= 2");
+    const HostGrid& h = s->grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    cudaStream_t st = s->stream;
+    if (forcing && !forcing->resident) {
+        int rc;
+        s->has_Teq = forcing->T_eq != nullptr; s->has_kT = forcing->k_T != nullptr; s->has_kv = forcing->k_v != nullptr;
+        if (s->has_Teq && (rc = upload_table(s, forcing->T_eq, &s->tab_Teq))) return rc;
+        if (s->has_kT && (rc = upload_table(s, forcing->k_T, &s->tab_kT))) return rc;
+        if (s->has_kv && (rc = upload_table(s, forcing->k_v, &s->tab_kv))) return rc;
+    }
+    Fields f = s->f;
+    f.T_eq = (forcing && s->has_Teq) ? s->tab_Teq : nullptr;
+    f.k_T = (forcing && s->has_kT) ? s->tab_kT : nullptr;
+    f.k_v = (forcing && s->has_kv) ? s->tab_kv : nullptr;
+    const Geom g = make_geom(s->grid);
+    for (int step = 0; step < n_large; ++step) {
+        for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
+            const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
+            const double delta = stage == 1 ? dt / 3.0 : dt / n;
+            THOR_DISPATCH(k_stage_prepare, nv, N, st, g, f, stage, delta);
+            THOR_DISPATCH(k_slow_terms, nv, N, st, g, f);
+            for (int sub = 0; sub < ns; ++sub) {
+                THOR_DISPATCH(k_momentum, nv, N, st, g, f, delta);
+                THOR_DISPATCH(k_vertical, nv, N, st, g, f, delta);
+            }
+            s->last_delta = delta;
+        }
+        k_finish<<<flat_blocks(nc), 256, 0, st>>>(nc, f, dt, g.Rd);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    CU(cudaGetLastError());
+    s->stepped = s->stepped || n_large > 0;
+    return THOR_OK;
+}
+
+int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int which) {
+    if (!s) return fail(THOR_EINVAL, "thor_acoustic_substeps: null state");
+    if (n_substeps < 0 || !(delta > 0) || which < 1 || which > 3) return fail(THOR_EINVAL, "thor_acoustic_substeps: bad argument");
+    if (!s->stepped) return fail(THOR_EINVAL, "thor_acoustic_substeps: call thor_step first (no stage data yet)");
+    const HostGrid& h = s->grid->h;
+    const Geom g = make_geom(s->grid);
+    Fields f = s->f;
+    for (int i = 0; i < n_substeps; ++i) {
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, h.N, s->stream, g, f, delta);
+        if (which & 2) THOR_DISPATCH(k_vertical, h.nv, h.N, s->stream, g, f, delta);
+    }
+    CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+int thor_diagnostics(const thor_state* s, thor_diag* out) {
+    if (!s || !out) return fail(THOR_EINVAL, "thor_diagnostics: null argument");
+    const HostGrid& h = s->grid->h;
+    const Geom g = make_geom(s->grid);
+    THOR_DISPATCH(k_diag, h.nv, h.N, s->stream, g, s->f, s->col_mass, s->col_energy);
+    CU(cudaGetLastError());
+    std::vector<double> m(h.N), e(h.N);
+    CU(cudaMemcpyAsync(m.data(), s->col_mass, h.N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaMemcpyAsync(e.data(), s->col_energy, h.N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    // Neumaier-compensated sum of the per-column partials
+    auto ksum = [](const std::vector<double>& v) {
+        double sum = 0.0, c = 0.0;
+        for (double x : v) {
+            double t = sum + x;
+            c += (std::fabs(sum) >= std::fabs(x)) ? (sum - t) + x : (x - t) + sum;
+            sum = t;
+        }
+        return sum + c;
+    };
+    out->total_mass = ksum(m);
+    out->total_energy = ksum(e);
+    return THOR_OK;
+}
+
+int thor_apply_div_device(const thor_grid* grid, const double* vx, const double* vy, const double* vz,
+                          double* out, void* cuda_stream) {
+    if (!grid || !vx || !vy || !vz || !out) return fail(THOR_EINVAL, "thor_apply_div_device: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const Geom g = make_geom(grid);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    THOR_DISPATCH(k_div, g.nv, g.N, st, g, vx, vy, vz, out);
+    CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+int thor_apply_grad_device(const thor_grid* grid, const double* sfield, double* gx, double* gy, double* gz,
+                           void* cuda_stream) {
+    if (!grid || !sfield || !gx || !gy || !gz) return fail(THOR_EINVAL, "thor_apply_grad_device: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const Geom g = make_geom(grid);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    THOR_DISPATCH(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
+    CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+// host wrappers of the two operators: upload, permute, run, permute back, download
+int thor_apply_div(const thor_grid* grid, const double* vec, double* out) {
+    if (!grid || !vec || !out) return fail(THOR_EINVAL, "thor_apply_div: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const HostGrid& h = grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    double* buf = nullptr;   // [3nc staging][vx][vy][vz][out]
+    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 7 * nc * sizeof(double)));
+    double *stg = buf, *vx = buf + 3 * nc, *vy = vx + nc, *vz = vy + nc, *o = vz + nc;
+    cudaError_t e = cudaMemcpy(stg, vec, 3 * nc * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_gather_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, stg, nv * 3, 3, 0, vx);
+        k_gather_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, stg, nv * 3, 3, 1, vy);
+        k_gather_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, stg, nv * 3, 3, 2, vz);
+        g_launches.fetch_add(3, std::memory_order_relaxed);
+        rc = thor_apply_div_device(grid, vx, vy, vz, o, nullptr);
+        if (rc == THOR_OK) {
+            k_scatter_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, o, nv, 1, 0, stg);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            e = cudaMemcpy(out, stg, nc * sizeof(double), cudaMemcpyDeviceToHost);
+        }
+    }
+    cudaFree(buf);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_div: ") + cudaGetErrorString(e));
+    return THOR_OK;
+}
+
+int thor_apply_grad(const thor_grid* grid, const double* sfield, double* out) {
+    if (!grid || !sfield || !out) return fail(THOR_EINVAL, "thor_apply_grad: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const HostGrid& h = grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    double* buf = nullptr;   // [3nc staging][s][gx][gy][gz]
+    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 7 * nc * sizeof(double)));
+    double *stg = buf, *sd = buf + 3 * nc, *gx = sd + nc, *gy = gx + nc, *gz = gy + nc;
+    cudaError_t e = cudaMemcpy(stg, sfield, nc * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_gather_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, stg, nv, 1, 0, sd);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        rc = thor_apply_grad_device(grid, sd, gx, gy, gz, nullptr);
+        if (rc == THOR_OK) {
+            k_scatter_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, gx, nv * 3, 3, 0, stg);
+            k_scatter_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, gy, nv * 3, 3, 1, stg);
+            k_scatter_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, gz, nv * 3, 3, 2, stg);
+            g_launches.fetch_add(3, std::memory_order_relaxed);
+            e = cudaMemcpy(out, stg, 3 * nc * sizeof(double), cudaMemcpyDeviceToHost);
+        }
+    }
+    cudaFree(buf);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_grad: ") + cudaGetErrorString(e));
+    return THOR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,189 @@
+"""Parity of the CUDA path with the oracle, element by element, through the C-ABI (-m gpu).
+
+Tolerances (BASELINE.json north_star): max relative error per prognostic field (max|gpu-oracle| /
+max|oracle| over the field) <= 1e-12 after one large step and <= 1e-9 after 100; total mass to 1e-13.
+The grid description (positions, neighbour lists, control-volume vertices) comes from the library's
+host generator and is handed to the oracle, which recomputes every coefficient itself; the seeded
+state and forcing tables come from thor_inputs for both.
+"""
+import numpy as np
+import pytest
+
+import thor_inputs as ti
+from conftest import have_cuda
+
+pytestmark = pytest.mark.gpu
+
+if have_cuda():
+    import oracle
+    import paper_1607_05535_b200 as thor
+
+FIELDS = ("rho", "mom_h", "W", "p")
+_CACHE = {}
+
+
+def _setup(level, nv, planet):
+    key = (level, nv, tuple(sorted(planet.items())))
+    if key not in _CACHE:
+        g = thor.Grid(level, nv, planet)
+        v = g.view
+        G = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"])
+        _CACHE[key] = (g, G)
+    return _CACHE[key]
+
+
+def _rel(a, b):
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+def _compare(gpu, ref, tol, what):
+    for name, a, b in zip(FIELDS, gpu, ref):
+        assert np.all(np.isfinite(a)), (what, name)
+        err = _rel(a, b)
+        assert err <= tol, "%s: field %s rel err %.3e > %.1e" % (what, name, err, tol)
+
+
+def _random_state(G, planet, seed, vel=3.0, wamp=0.3):
+    rng = np.random.default_rng(seed)
+    N, nv = G.N, G.nv
+    rho, V, W, p = ti.rest_state(planet, nv, N, 1.0e5, 290.0)
+    T = 290.0 * (1 + rng.uniform(-1e-2, 1e-2, size=rho.shape))
+    rho = p / (planet["Rd"] * T)
+    u = rng.uniform(-vel, vel, size=V.shape)
+    u -= np.sum(u * G.xyz[:, None, :], axis=-1, keepdims=True) * G.xyz[:, None, :]
+    V = rho[..., None] * u
+    W[:, 1:nv] = rng.uniform(-wamp, wamp, size=(N, nv - 1))
+    return rho, V, W, p
+
+
+def test_state_roundtrip_is_bit_exact():
+    g, G = _setup(3, 8, ti.EARTH)
+    s = _random_state(G, ti.EARTH, 1)
+    st = thor.State(g, *s)
+    out = st.get()
+    for a, b in zip(out, s):
+        assert np.array_equal(a, b)
+    st.set(*[2 * x for x in s])
+    out = st.get()
+    assert np.array_equal(out[0], 2 * s[0]) and np.array_equal(out[1], 2 * s[1])
+
+
+@pytest.mark.parametrize("level", [4, 5])
+def test_config1_operators_match_oracle_and_closed_form(level):
+    nv = 32
+    g, G = _setup(level, nv, ti.EARTH)
+    f = ti.harmonic_test_fields(G.xyz, ti.EARTH, nv, seed=ti.SEED0 + 1)
+    div = g.apply_div(f["v"])
+    grad = g.apply_grad(f["s"])
+    assert _rel(div, G.hdiv(f["v"])) <= 1e-12
+    assert _rel(grad, G.hgrad(f["s"])) <= 1e-12
+    # against the analytic result: a few per cent at these levels, second order (pins P5/P8)
+    assert _rel(div, f["div_exact"]) < (0.08 if level == 4 else 0.02)
+    assert _rel(grad, f["grad_exact"]) < (0.04 if level == 4 else 0.01)
+    # gradient of a constant is exactly zero (L86)
+    assert np.all(g.apply_grad(np.full((G.N, nv), 7.25)) == 0.0)
+
+
+@pytest.mark.parametrize("nv", [8, 16, 32, 64, 37, 5, 70, 128])
+def test_every_layer_shape_one_step(nv):
+    """All lane-group shapes (G, E) incl. ragged layer counts, one large step with forcing."""
+    planet = dict(ti.EARTH)
+    g, G = _setup(2, nv, planet)
+    s = _random_state(G, planet, 100 + nv)
+    rng = np.random.default_rng(nv)
+    F = dict(T_eq=280 + rng.uniform(-10, 10, size=s[0].shape), k_T=np.full(s[0].shape, 1e-5),
+             k_v=rng.uniform(0, 2e-5, size=s[0].shape))
+    st = thor.State(g, *s)
+    st.step(1, 600.0, 4, F)
+    ref = G.step(*s, 1, 600.0, 4, F)
+    _compare(st.get(), ref, 1e-12, "nv=%d" % nv)
+
+
+def test_config0_parity_1_and_10_steps_and_mass():
+    cfg = ti.CONFIGS[0]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.initial_state(0, G.xyz)
+    st = thor.State(g, *s)
+    m0, e0 = st.diagnostics()
+    mo, eo = G.diagnostics(*s)
+    assert abs(m0 - mo) <= 1e-13 * mo and abs(e0 - eo) <= 1e-12 * abs(eo)
+    st.step(1, cfg["dt"], cfg["n_sub"])
+    ref = G.step(*s, 1, cfg["dt"], cfg["n_sub"])
+    _compare(st.get(), ref, 1e-12, "cfg0 1 step")
+    st.step(9, cfg["dt"], cfg["n_sub"])
+    ref = G.step(*ref, 9, cfg["dt"], cfg["n_sub"])
+    _compare(st.get(), ref, 1e-10, "cfg0 10 steps")
+    m1, e1 = st.diagnostics()
+    mr, er = G.diagnostics(*ref)
+    assert abs(m1 - mr) <= 1e-13 * mr
+    assert abs(m1 - m0) <= 1e-13 * m0                                   # conserved on the GPU too (P11)
+    assert abs(e1 - er) <= 1e-11 * abs(er)
+
+
+def test_rest_state_stays_at_rest_on_gpu():
+    cfg = ti.CONFIGS[0]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.rest_state(cfg["planet"], cfg["nv"], G.N, cfg["p_s"], cfg["T0"])
+    st = thor.State(g, *s)
+    st.step(10, cfg["dt"], cfg["n_sub"])
+    rho, V, W, p = st.get()
+    assert np.abs(V / rho[..., None]).max() < 1e-9
+    assert np.abs(W).max() < 1e-9
+    assert np.abs(p - s[3]).max() < 1e-13 * s[3].max()
+
+
+def test_config2_parity_1_and_100_steps():
+    cfg = ti.CONFIGS[2]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.initial_state(2, G.xyz)
+    F = ti.forcing_tables(2, G.xyz)
+    st = thor.State(g, *s)
+    m0, _ = st.diagnostics()
+    st.step(1, cfg["dt"], cfg["n_sub"], F)
+    ref = G.step(*s, 1, cfg["dt"], cfg["n_sub"], F)
+    _compare(st.get(), ref, 1e-12, "cfg2 1 step")
+    st.step(99, cfg["dt"], cfg["n_sub"], F)
+    ref = G.step(*ref, 99, cfg["dt"], cfg["n_sub"], F)
+    _compare(st.get(), ref, 1e-9, "cfg2 100 steps")
+    m1, _ = st.diagnostics()
+    mr, _ = G.diagnostics(*ref)
+    assert abs(m1 - mr) <= 1e-13 * mr and abs(m1 - m0) <= 1e-13 * m0
+
+
+def test_config3_parity_1_and_100_steps():
+    """The bench workload (level 6 x 32, hot Jupiter), in the launch configuration bench.py times."""
+    cfg = ti.CONFIGS[3]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.initial_state(3, G.xyz)
+    F = ti.forcing_tables(3, G.xyz)
+    st = thor.State(g, *s)
+    m0, _ = st.diagnostics()
+    st.step(1, cfg["dt"], cfg["n_sub"], F)
+    ref = G.step(*s, 1, cfg["dt"], cfg["n_sub"], F)
+    _compare(st.get(), ref, 1e-12, "cfg3 1 step")
+    st.step(99, cfg["dt"], cfg["n_sub"], F)
+    ref = G.step(*ref, 99, cfg["dt"], cfg["n_sub"], F)
+    _compare(st.get(), ref, 1e-9, "cfg3 100 steps")
+    m1, _ = st.diagnostics()
+    mr, _ = G.diagnostics(*ref)
+    assert abs(m1 - mr) <= 1e-13 * mr and abs(m1 - m0) <= 1e-13 * m0
+
+
+def test_config4_parity_one_step_and_mass_over_the_run():
+    """Level 7 x 64: one large step element by element; mass conservation (a property that holds
+    at any size) over more steps."""
+    cfg = ti.CONFIGS[4]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.initial_state(4, G.xyz)
+    F = ti.forcing_tables(4, G.xyz)
+    st = thor.State(g, *s)
+    m0, _ = st.diagnostics()
+    st.step(1, cfg["dt"], cfg["n_sub"], F)
+    ref = G.step(*s, 1, cfg["dt"], cfg["n_sub"], F)
+    _compare(st.get(), ref, 1e-12, "cfg4 1 step")
+    st.step(9, cfg["dt"], cfg["n_sub"], F)
+    m1, _ = st.diagnostics()
+    assert abs(m1 - m0) <= 1e-13 * m0
+    out = st.get()
+    assert all(np.all(np.isfinite(a)) for a in out)
+    _CACHE.clear()

@@ -1,0 +1,79 @@
+"""Host grid generator of the library (thor_grid_create) against the oracle's independent
+generator (pin P3) and the oracle's geometry.  Host only: runs without a GPU."""
+import math
+
+import numpy as np
+import pytest
+from scipy.spatial import cKDTree
+
+import oracle
+import paper_1607_05535_b200 as thor
+import thor_inputs as ti
+from oracle import grid_oracle
+
+
+@pytest.fixture(scope="module")
+def lib_grid3():
+    return thor.Grid(3, 4, ti.EARTH)
+
+
+def test_p3_library_grid_matches_the_oracle_generator(lib_grid3):
+    v = lib_grid3.view
+    xyz, nbr, C, _ = grid_oracle.build(3, tol=1e-9)
+    assert v["n_cols"] == len(xyz) == ti.n_columns(3)
+    dist, idx = cKDTree(xyz).query(v["xyz"])
+    assert len(set(idx)) == len(idx)                       # one-to-one
+    assert dist.max() < 2e-6                               # both converged to the same equilibrium
+    # same topology under that matching
+    for i in range(0, v["n_cols"], 3):
+        mine = {idx[j] for j in v["nbr"][i] if j >= 0}
+        theirs = {j for j in nbr[idx[i]] if j >= 0}
+        assert mine == theirs
+    # control-volume vertices agree too (triangle centroids of the pre-move grid)
+    dC, _ = cKDTree(C[:, :5].reshape(-1, 3)).query(v["cv_vertex"][:, :5].reshape(-1, 3))
+    assert dC.max() < 2e-6
+
+
+def test_exported_geometry_matches_the_oracle_recomputation(lib_grid3):
+    v = lib_grid3.view
+    G = oracle.Geometry(v["xyz"], v["nbr"], 4, ti.EARTH, v["cv_vertex"])
+    assert np.abs(G.Ac - v["area"]).max() < 1e-15
+    assert np.abs(G.len - v["edge_len"]).max() < 1e-15
+    assert np.abs(G.nrm - v["edge_nrm"]).max() < 1e-14
+    assert abs(v["area"].sum() - 4 * math.pi) < 1e-12
+    # L120: every point is the Eq. 13 centroid of its control volume
+    deg = (v["nbr"] >= 0).sum(axis=1)
+    d = [np.linalg.norm(np.cross(oracle.centroid_eq13(v["cv_vertex"][i, : deg[i]]), v["xyz"][i])) for i in range(v["n_cols"])]
+    assert max(d) < 1e-13
+
+
+@pytest.mark.parametrize("level", [0, 1, 5])
+def test_topology_and_device_order(level):
+    g = thor.Grid(level, 2, ti.EARTH)
+    v = g.view
+    N = v["n_cols"]
+    assert N == ti.n_columns(level)
+    deg = (v["nbr"] >= 0).sum(axis=1)
+    assert (deg == 5).sum() == 12 and deg.sum() == 2 * (3 * N - 6)
+    assert sorted(v["device_order"]) == list(range(N))                      # a permutation
+    assert np.allclose(np.linalg.norm(v["xyz"], axis=1), 1.0, atol=1e-15)
+    if level >= 5:
+        # locality: neighbours sit close in device order (quadtree order of the leaf triangles)
+        rank = np.empty(N, dtype=np.int64)
+        rank[v["device_order"]] = np.arange(N)
+        gaps = [abs(rank[i] - rank[j]) for i in range(N) for j in v["nbr"][i] if j >= 0]
+        assert np.median(gaps) < 64
+
+
+def test_operator_accuracy_on_library_grids():
+    """P5 on the library's own grids, through the oracle's operators: second order 4 -> 5."""
+    e = {}
+    for lvl in (4, 5):
+        v = thor.Grid(lvl, 2, ti.EARTH).view
+        G = oracle.Geometry(v["xyz"], v["nbr"], 2, ti.EARTH, v["cv_vertex"])
+        hr = ti.heikes_randall_fields(v["xyz"], 1, 1)
+        d = G.hdiv(np.repeat(hr["v"][:, None, :], 2, axis=1)) * G.r_c[None, :]
+        err = d[:, 0] - hr["div_v"]
+        e[lvl] = (math.sqrt(np.sum(G.Ac * err ** 2) / G.Ac.sum()), np.abs(err).max())
+    assert 1.8 < math.log2(e[4][0] / e[5][0]) < 2.2
+    assert 1.7 < math.log2(e[4][1] / e[5][1]) < 2.3
