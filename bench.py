@@ -1,0 +1,273 @@
+"""bench.py -- cell-updates/s of the THOR HE-VI large step on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]            the CUDA path (default N = 1)
+  python bench.py --impl reference [--steps K] [--warmup W]      the oracle on the host cores
+
+A "step" is one large time step (all rows of DESIGN.md's hot-path table: three Runge-Kutta stages
+of slow terms + 1 + n/2 + n acoustic substeps + forcing) of config 3 of BASELINE.json
+(level 6 x 32 layers, hot-Jupiter constants, n = 8): 40962 x 32 cells x 13 substeps per step.
+One JSON line on stdout (rank 0).  Multi-GPU: the path is fixed to one GPU by north_star
+("replicas only"): every rank runs an independent replica, no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import thor_inputs as ti  # noqa: E402
+
+WORKLOAD = 3
+METRIC = "cell-updates/s (cols x layers x acoustic substeps) FP64"
+UNIT = "cell-updates/s"
+
+# algorithmic bytes per cell per launch; geometry bytes are per column
+K2_MIN_DOUBLES = 18      # SURVEY 8(d) split: 14 reads (V*'(3) re-read, p*, W*, rho*, rho-theta, 4 slow terms,
+                         # rho^t, p^t, theta^t) + 4 writes
+K2_DESIGN_DOUBLES = 21   # what this design's kernel touches once: 17 reads (LU factors instead of rho^t) + 4 writes
+K1_DOUBLES = 10          # p*, V*(3), slowV(3) read; V*'(3) written
+SUBSTEP_SURVEY_DOUBLES = 27   # B_dep of SURVEY 8(d)
+K2_GEOM_BYTES = 6 * 4 + 21 * 8
+K1_GEOM_BYTES = 6 * 4 + 18 * 8
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.samples.append(parts)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[3 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm), "power_w_max": max(float(s[2]) for s in self.samples)}
+
+
+def sample_config(level):
+    """config 3's constants and forcing on a coarser grid (used only by the CPU legs)."""
+    cfg = dict(ti.CONFIGS[WORKLOAD])
+    cfg["dt"] = cfg["dt"] * 2 ** (cfg["level"] - level)
+    cfg["level"] = level
+    return cfg
+
+
+def time_oracle(level, n_steps, warmup):
+    """The oracle as it stands on the host cores.  Grid description from the oracle's own generator
+    up to level 4 is too slow beyond that, so the library's host generator supplies positions."""
+    import oracle
+    import paper_1607_05535_b200 as thor
+    cfg = sample_config(level)
+    g = thor.Grid(level, cfg["nv"], cfg["planet"])          # host-only call
+    v = g.view
+    G = oracle.Geometry(v["xyz"], v["nbr"], cfg["nv"], cfg["planet"], v["cv_vertex"])
+    ti.CONFIGS["_sample"] = cfg
+    state = ti.initial_state(WORKLOAD, v["xyz"])
+    F = ti.forcing_tables(WORKLOAD, v["xyz"])
+    for _ in range(warmup):
+        state = G.step(*state, 1, cfg["dt"], cfg["n_sub"], F)
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        state = G.step(*state, 1, cfg["dt"], cfg["n_sub"], F)
+    dt = time.perf_counter() - t0
+    cells = v["n_cols"] * cfg["nv"] * ti.substeps_per_large_step(cfg["n_sub"])
+    return cells * n_steps / dt, dt / max(n_steps, 1), oracle.num_threads(), \
+        "config-3 constants and forcing at level %d x %d layers (%d columns), %d large steps" % (
+            level, cfg["nv"], v["n_cols"], n_steps)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    value, per_step, cores, sample = time_oracle(5, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config 3 (hot Jupiter, n=8) sampled: " + sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1607_05535_b200 as thor
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback (use --impl reference)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = ti.CONFIGS[WORKLOAD]
+    nv, dt, n = cfg["nv"], cfg["dt"], cfg["n_sub"]
+    grid = thor.Grid(cfg["level"], nv, cfg["planet"])
+    N = grid.n_cols
+    xyz = grid.view["xyz"]
+    host = ti.initial_state(WORKLOAD, xyz)
+    forcing = ti.forcing_tables(WORKLOAD, xyz)
+    stream = torch.cuda.Stream()
+    state = thor.State(grid, *host, cuda_stream=stream.cuda_stream)
+    substeps = ti.substeps_per_large_step(n)
+    cells_per_step = N * nv * substeps
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            state.step(1, dt, n, forcing)
+        barrier()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        time.sleep(0.3)
+        l0 = thor.thor_launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record(stream)
+        for _ in range(args.steps):
+            state.step(1, dt, n, forcing)
+        ev1.record(stream)
+        barrier()
+        launches = thor.thor_launch_count() - l0
+        ms = ev0.elapsed_time(ev1)
+
+        # dominant kernel alone (K2 = divergences + column solve) and K1, CUDA events on the same stream
+        def time_kernels(which, reps=60):
+            state.acoustic_substeps(5, dt / n, which)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record(stream)
+            state.acoustic_substeps(reps, dt / n, which)
+            b.record(stream)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        k2_ms = time_kernels(2)
+        k1_ms = time_kernels(1)
+        sub_ms = time_kernels(3)
+        sampler.stop_flag.set()
+        sampler.join()
+
+        # end to end through the public API with host buffers: upload, step, download every step
+        state.set(*host)
+        pinned = [torch.from_numpy(a).pin_memory() for a in host]
+        h_in = [t.numpy() for t in pinned]
+        h_out = tuple(torch.empty_like(t).pin_memory().numpy() for t in pinned)
+        state.set(*h_in)
+        state.step(1, dt, n, forcing)
+        state.get(h_out)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            state.set(*h_in)
+            state.step(1, dt, n, forcing)
+            state.get(h_out)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        barrier()
+
+    io_bytes = int(sum(a.nbytes for a in h_in))
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+    value = cells_per_step * args.steps * world / (ms * 1e-3)
+    e2e_value = cells_per_step * args.steps * world / e2e_s
+
+    peak, peak_kind = measured_peak()
+    cells = N * nv
+    k2_bytes = cells * K2_MIN_DOUBLES * 8 + N * K2_GEOM_BYTES
+    achieved = k2_bytes / (k2_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_vertical (a5-a9: divergences + column solve + rho, rho-theta, p*)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "peak_kind": peak_kind, "ms_per_launch": k2_ms, "bytes_per_launch": k2_bytes,
+                "achieved_design_bytes": (cells * K2_DESIGN_DOUBLES * 8 + N * K2_GEOM_BYTES) / (k2_ms * 1e-3) / 1e9,
+                "k1_ms_per_launch": k1_ms,
+                "k1_achieved": (cells * K1_DOUBLES * 8 + N * K1_GEOM_BYTES) / (k1_ms * 1e-3) / 1e9,
+                "substep_ms": sub_ms,
+                "substep_frac_survey_budget": (cells * SUBSTEP_SURVEY_DOUBLES * 8 + N * 336) / (sub_ms * 1e-3) / 1e9 / peak,
+                "substep_frac_of_8TBs": (cells * SUBSTEP_SURVEY_DOUBLES * 8 + N * 336) / (sub_ms * 1e-3) / 1e9 / 8000.0,
+                "substep_cell_updates_per_s": cells / (sub_ms * 1e-3)}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config 3: level 6 (40962 columns) x 32 layers, hot-Jupiter constants, dt=300 s, "
+                                   "n=8 (13 substeps per large step), Newtonian relaxation forcing",
+                       "cells": cells, "substeps_per_step": substeps, "parallelism": "replicas x%d" % world,
+                       "l2": "working set 35 arrays x 10.5 MB = 367 MB > 126 MB L2, no flush"},
+            "clocks": sampler.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
+                    "ms_per_step": e2e_s / args.steps * 1e3},
+            "gpu_launches": int(launches), "roofline": roofline}
+    if world == 1 and not args.no_cpu_baseline:
+        v, per, cores, sample = time_oracle(5, 4, 1)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
