@@ -34,14 +34,27 @@ int fail(int code, const std::string& msg) {
             return fail(THOR_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
     } while (0)
 
+constexpr int kMaxLayers = 128;
+
 struct DeviceGeom {
     bool ready = false;
     int device = -1;
+    int Npad = 0;
     int* nbr = nullptr;
     int* order = nullptr;
     double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr;
 };
+
+// lane-group width G and layers per lane E of the record kernels; NVP = G*E padded layers
+struct Shape { int G, E; };
+Shape shape_for(int nv) {
+    if (nv <= 8) return {4, 2};
+    if (nv <= 16) return {8, 2};
+    if (nv <= 32) return {16, 2};
+    if (nv <= 64) return {32, 2};
+    return {32, 4};
+}
 
 }  // namespace
 
@@ -53,13 +66,12 @@ struct thor_grid {
 struct thor_state {
     const thor_grid* grid = nullptr;
     cudaStream_t stream = nullptr;
-    Fields f{};
-    std::vector<double*> owned;      // every cudaMalloc'ed field
+    int NVP = 0;
+    double* S = nullptr;             // the slab of column records [Npad][NF][NVP]
     double* stage_buf = nullptr;     // canonical-order staging, max(N*nv*3, N*(nv+1)) doubles
-    double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;
+    double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;   // [Npad][NVP]
     bool has_Teq = false, has_kT = false, has_kv = false;
     double *col_mass = nullptr, *col_energy = nullptr;
-    double last_delta = 0.0;
     bool stepped = false;
 };
 
@@ -72,6 +84,8 @@ int upload(T** dst, const std::vector<T>& src) {
     return THOR_OK;
 }
 
+// device copy of the geometry, padded to Npad columns (pad columns: own neighbour, zero weights)
+// and to kMaxLayers layers (pad layers: 0)
 int ensure_device_geom(const thor_grid* grid) {
     DeviceGeom& d = grid->d;
     if (d.ready) return THOR_OK;
@@ -81,18 +95,36 @@ int ensure_device_geom(const thor_grid* grid) {
         return fail(THOR_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
     CU(cudaGetDevice(&d.device));
     const HostGrid& h = grid->h;
+    const int N = h.N, Npad = (N + kColPad - 1) / kColPad * kColPad;
+    d.Npad = Npad;
+    std::vector<int> nbr(size_t(Npad) * 8);
+    std::vector<double> wdiv(size_t(Npad) * 24, 0.0), wgrad(size_t(Npad) * 18, 0.0), rhat(size_t(Npad) * 4, 0.0),
+        area(Npad, 0.0);
+    for (int c = 0; c < Npad; ++c) {
+        for (int k = 0; k < 8; ++k) nbr[size_t(c) * 8 + k] = (c < N && k < 6) ? h.d_nbr[size_t(c) * 6 + k] : c;
+        if (c >= N) { rhat[size_t(c) * 4 + 2] = 1.0; continue; }
+        std::copy_n(&h.d_wdiv[size_t(c) * 21], 21, &wdiv[size_t(c) * 24]);
+        std::copy_n(&h.d_wgrad[size_t(c) * 18], 18, &wgrad[size_t(c) * 18]);
+        std::copy_n(&h.d_rhat[size_t(c) * 3], 3, &rhat[size_t(c) * 4]);
+        area[c] = h.d_area[c];
+    }
+    auto padded = [&](const std::vector<double>& v) {
+        std::vector<double> o(kMaxLayers, 0.0);
+        std::copy(v.begin(), v.end(), o.begin());
+        return o;
+    };
     int rc;
-    if ((rc = upload(&d.nbr, h.d_nbr))) return rc;
+    if ((rc = upload(&d.nbr, nbr))) return rc;
     if ((rc = upload(&d.order, h.order))) return rc;
-    if ((rc = upload(&d.wdiv, h.d_wdiv))) return rc;
-    if ((rc = upload(&d.wgrad, h.d_wgrad))) return rc;
-    if ((rc = upload(&d.rhat, h.d_rhat))) return rc;
-    if ((rc = upload(&d.area, h.d_area))) return rc;
-    if ((rc = upload(&d.rinv, h.rinv))) return rc;
-    if ((rc = upload(&d.dlo, h.dlo))) return rc;
-    if ((rc = upload(&d.dhi, h.dhi))) return rc;
-    if ((rc = upload(&d.vol, h.vol))) return rc;
-    if ((rc = upload(&d.zc, h.zc))) return rc;
+    if ((rc = upload(&d.wdiv, wdiv))) return rc;
+    if ((rc = upload(&d.wgrad, wgrad))) return rc;
+    if ((rc = upload(&d.rhat, rhat))) return rc;
+    if ((rc = upload(&d.area, area))) return rc;
+    if ((rc = upload(&d.rinv, padded(h.rinv)))) return rc;
+    if ((rc = upload(&d.dlo, padded(h.dlo)))) return rc;
+    if ((rc = upload(&d.dhi, padded(h.dhi)))) return rc;
+    if ((rc = upload(&d.vol, padded(h.vol)))) return rc;
+    if ((rc = upload(&d.zc, padded(h.zc)))) return rc;
     d.ready = true;
     return THOR_OK;
 }
@@ -101,79 +133,88 @@ Geom make_geom(const thor_grid* grid) {
     const HostGrid& h = grid->h;
     const DeviceGeom& d = grid->d;
     Geom g;
-    g.N = h.N; g.nv = h.nv;
+    g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
     g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc;
     g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
+    // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
+    const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
+    g.eosq[0] = 1.0;
+    for (int k = 1; k <= kEosTerms; ++k) g.eosq[k] = g.eosq[k - 1] * (gam - k) / (k + 1);
     return g;
 }
 
-// lane-group width G and layers per lane E for a given layer count
-struct Shape { int G, E; };
-Shape shape_for(int nv) {
-    if (nv <= 8) return {8, 1};
-    if (nv <= 16) return {16, 1};
-    if (nv <= 32) return {32, 1};
-    if (nv <= 64) return {32, 2};
-    if (nv <= 96) return {32, 3};
-    return {32, 4};
-}
-int column_blocks(int N, int G) {
-    const int cols_per_block = kWarpsPerBlock * (32 / G);
-    return (N + cols_per_block - 1) / cols_per_block;
-}
-
-// dispatch a column kernel template over the supported (G, E) shapes
-#define THOR_DISPATCH(KERNEL, nv, N, stream, ...)                                                  \
+// dispatch a record kernel template over the supported (G, E) shapes; Npad is a multiple of the
+// columns per block of every shape
+#define THOR_DISPATCH(KERNEL, nv, Npad, stream, ...)                                               \
     do {                                                                                           \
         const Shape sh_ = shape_for(nv);                                                           \
-        const dim3 grid_(column_blocks(N, sh_.G)), block_(kWarpsPerBlock * 32);                    \
-        if (sh_.G == 8) KERNEL<8, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                   \
-        else if (sh_.G == 16) KERNEL<16, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);            \
-        else if (sh_.E == 1) KERNEL<32, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
+        const dim3 grid_((Npad) / (kWarpsPerBlock * (32 / sh_.G))), block_(kWarpsPerBlock * 32);   \
+        if (sh_.G == 4) KERNEL<4, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                   \
+        else if (sh_.G == 8) KERNEL<8, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);              \
+        else if (sh_.G == 16) KERNEL<16, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);            \
         else if (sh_.E == 2) KERNEL<32, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
-        else if (sh_.E == 3) KERNEL<32, 3><<<grid_, block_, 0, stream>>>(__VA_ARGS__);             \
+        else KERNEL<32, 4><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                             \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                                        \
+    } while (0)
+
+// config-1 operators on plain [N][nv] arrays: G lanes per column, E = ceil(nv/G) strided layers per lane
+#define THOR_DISPATCH_OP(KERNEL, nv, N, stream, ...)                                               \
+    do {                                                                                           \
+        const int G_ = (nv) <= 8 ? 8 : ((nv) <= 16 ? 16 : 32);                                     \
+        const int E_ = ((nv) + G_ - 1) / G_;                                                       \
+        const int cpb_ = kWarpsPerBlock * (32 / G_);                                               \
+        const dim3 grid_(((N) + cpb_ - 1) / cpb_), block_(kWarpsPerBlock * 32);                    \
+        if (G_ == 8) KERNEL<8, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                      \
+        else if (G_ == 16) KERNEL<16, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);               \
+        else if (E_ == 1) KERNEL<32, 1><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                \
+        else if (E_ == 2) KERNEL<32, 2><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                \
+        else if (E_ == 3) KERNEL<32, 3><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                \
         else KERNEL<32, 4><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                             \
         g_launches.fetch_add(1, std::memory_order_relaxed);                                        \
     } while (0)
 
 int flat_blocks(size_t n) { return int((n + 255) / 256); }
 
-// host canonical arrays -> device fields (through the staging buffer, permuted on the device)
+// one canonical host array (or a component of it) -> one row of every column record
+int put_row(thor_state* s, const double* host, size_t count, int row_len, int cs, int c0, int field, double pad,
+            int zero_k0) {
+    const HostGrid& h = s->grid->h;
+    const int Npad = s->grid->d.Npad;
+    if (host) CU(cudaMemcpyAsync(s->stage_buf, host, count * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    k_rows_from_canonical<<<flat_blocks(size_t(Npad) * s->NVP), 256, 0, s->stream>>>(
+        h.N, Npad, h.nv, s->NVP, s->grid->d.order, s->stage_buf, row_len, cs, c0,
+        s->S + size_t(field) * s->NVP, size_t(NF) * s->NVP, pad, zero_k0);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return THOR_OK;
+}
+
+// host canonical arrays -> Phi^n rows (through the staging buffer, permuted and padded on the device)
 int upload_state(thor_state* s, const double* rho, const double* mom_h, const double* W, const double* p) {
     const HostGrid& h = s->grid->h;
     const int N = h.N, nv = h.nv;
     const size_t nc = size_t(N) * nv;
-    const int* order = s->grid->d.order;
-    cudaStream_t st = s->stream;
-    auto gather = [&](const double* host, size_t count, int row_len, int cs, int c0, double* dst) -> int {
-        if (host) CU(cudaMemcpyAsync(s->stage_buf, host, count * sizeof(double), cudaMemcpyHostToDevice, st));
-        k_gather_rows<<<flat_blocks(nc), 256, 0, st>>>(N, nv, order, s->stage_buf, row_len, cs, c0, dst);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
-        return THOR_OK;
-    };
     int rc;
-    if ((rc = gather(rho, nc, nv, 1, 0, s->f.rho_n))) return rc;
-    if ((rc = gather(p, nc, nv, 1, 0, s->f.p_n))) return rc;
-    if ((rc = gather(mom_h, nc * 3, nv * 3, 3, 0, s->f.Vx_n))) return rc;
-    if ((rc = gather(nullptr, 0, nv * 3, 3, 1, s->f.Vy_n))) return rc;
-    if ((rc = gather(nullptr, 0, nv * 3, 3, 2, s->f.Vz_n))) return rc;
-    if ((rc = gather(W, size_t(N) * (nv + 1), nv + 1, 1, 0, s->f.W_n))) return rc;   // lower interfaces 0..nv-1
-    k_zero_ground<<<(N + 255) / 256, 256, 0, st>>>(N, nv, s->f.W_n);                 // rigid lid (L339)
-    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if ((rc = put_row(s, rho, nc, nv, 1, 0, F_RHON, 1.0, 0))) return rc;
+    if ((rc = put_row(s, p, nc, nv, 1, 0, F_PN, h.P.p_ref, 0))) return rc;
+    if ((rc = put_row(s, mom_h, nc * 3, nv * 3, 3, 0, F_VXN, 0.0, 0))) return rc;
+    if ((rc = put_row(s, nullptr, 0, nv * 3, 3, 1, F_VYN, 0.0, 0))) return rc;
+    if ((rc = put_row(s, nullptr, 0, nv * 3, 3, 2, F_VZN, 0.0, 0))) return rc;
+    // W: lower interfaces 0..nv-1 of the canonical [nv+1]; ground forced to 0 (rigid lid, L339)
+    if ((rc = put_row(s, W, size_t(N) * (nv + 1), nv + 1, 1, 0, F_WN, 0.0, 1))) return rc;
     CU(cudaGetLastError());
-    CU(cudaStreamSynchronize(st));
+    CU(cudaStreamSynchronize(s->stream));
     return THOR_OK;
 }
 
 int upload_table(thor_state* s, const double* host, double** dev) {
     const HostGrid& h = s->grid->h;
+    const int Npad = s->grid->d.Npad;
     const size_t nc = size_t(h.N) * h.nv;
-    if (!*dev) {
-        CU(cudaMalloc(reinterpret_cast<void**>(dev), nc * sizeof(double)));
-    }
+    if (!*dev) CU(cudaMalloc(reinterpret_cast<void**>(dev), size_t(Npad) * s->NVP * sizeof(double)));
     CU(cudaMemcpyAsync(s->stage_buf, host, nc * sizeof(double), cudaMemcpyHostToDevice, s->stream));
-    k_gather_rows<<<flat_blocks(nc), 256, 0, s->stream>>>(h.N, h.nv, s->grid->d.order, s->stage_buf, h.nv, 1, 0, *dev);
+    k_rows_from_canonical<<<flat_blocks(size_t(Npad) * s->NVP), 256, 0, s->stream>>>(
+        h.N, Npad, h.nv, s->NVP, s->grid->d.order, s->stage_buf, h.nv, 1, 0, *dev, size_t(s->NVP), 0.0, 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CU(cudaGetLastError());
     return THOR_OK;
@@ -228,8 +269,7 @@ void thor_grid_destroy(thor_grid* grid) {
 
 void thor_state_destroy(thor_state* s) {
     if (!s) return;
-    for (double* p : s->owned) cudaFree(p);
-    cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
+    cudaFree(s->S); cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
     cudaFree(s->col_mass); cudaFree(s->col_energy);
     delete s;
 }
@@ -244,28 +284,19 @@ int thor_state_init(const thor_grid* grid, const double* rho, const double* mom_
     s->grid = grid;
     s->stream = static_cast<cudaStream_t>(cuda_stream);
     const HostGrid& h = grid->h;
-    const size_t nc = size_t(h.N) * h.nv;
-    double** slots[] = {&s->f.rho_n, &s->f.Vx_n, &s->f.Vy_n, &s->f.Vz_n, &s->f.W_n, &s->f.p_n, &s->f.rt_n,
-                        &s->f.rho_t, &s->f.Vx_t, &s->f.Vy_t, &s->f.Vz_t, &s->f.W_t, &s->f.p_t,
-                        &s->f.h, &s->f.th, &s->f.ux, &s->f.uy, &s->f.uz, &s->f.fa, &s->f.fi, &s->f.fc,
-                        &s->f.sVx, &s->f.sVy, &s->f.sVz, &s->f.srho, &s->f.sW, &s->f.sp, &s->f.srt,
-                        &s->f.rho_s, &s->f.Vx_s, &s->f.Vy_s, &s->f.Vz_s, &s->f.W_s, &s->f.p_s, &s->f.rt};
-    for (double** slot : slots) {
-        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(slot), nc * sizeof(double));
-        if (e == cudaSuccess) e = cudaMemsetAsync(*slot, 0, nc * sizeof(double), s->stream);
-        if (e != cudaSuccess) {
-            thor_state_destroy(s);
-            return fail(e == cudaErrorMemoryAllocation ? THOR_ENOMEM : THOR_ECUDA,
-                        std::string("thor_state_init: ") + cudaGetErrorString(e));
-        }
-        s->owned.push_back(*slot);
-    }
-    const size_t stage_n = std::max(nc * 3, size_t(h.N) * (h.nv + 1));
-    if (cudaMalloc(reinterpret_cast<void**>(&s->stage_buf), stage_n * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&s->col_mass), h.N * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(reinterpret_cast<void**>(&s->col_energy), h.N * sizeof(double)) != cudaSuccess) {
+    const Shape sh = shape_for(h.nv);
+    s->NVP = sh.G * sh.E;
+    const size_t slab = size_t(grid->d.Npad) * NF * s->NVP;
+    const size_t stage_n = std::max(size_t(h.N) * h.nv * 3, size_t(h.N) * (h.nv + 1));
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&s->S), slab * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->S, 0, slab * sizeof(double), s->stream);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&s->stage_buf), stage_n * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&s->col_mass), h.N * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&s->col_energy), h.N * sizeof(double));
+    if (e != cudaSuccess) {
         thor_state_destroy(s);
-        return fail(THOR_ENOMEM, "thor_state_init: out of device memory");
+        return fail(e == cudaErrorMemoryAllocation ? THOR_ENOMEM : THOR_ECUDA,
+                    std::string("thor_state_init: ") + cudaGetErrorString(e));
     }
     rc = upload_state(s, rho, mom_h, W, p);
     if (rc) {
@@ -288,21 +319,22 @@ int thor_state_get(const thor_state* s, double* rho, double* mom_h, double* W, d
     const size_t nc = size_t(N) * nv;
     const int* order = s->grid->d.order;
     cudaStream_t st = s->stream;
-    auto scatter = [&](const double* src, int row_len, int cs, int c0) {
-        k_scatter_rows<<<flat_blocks(nc), 256, 0, st>>>(N, nv, order, src, row_len, cs, c0, s->stage_buf);
+    auto scatter = [&](int field, int row_len, int cs, int c0) {
+        k_rows_to_canonical<<<flat_blocks(nc), 256, 0, st>>>(N, nv, s->NVP, order, s->S + size_t(field) * s->NVP,
+                                                             size_t(NF) * s->NVP, row_len, cs, c0, s->stage_buf);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     };
-    scatter(s->f.rho_n, nv, 1, 0);
+    scatter(F_RHON, nv, 1, 0);
     CU(cudaMemcpyAsync(rho, s->stage_buf, nc * sizeof(double), cudaMemcpyDeviceToHost, st));
-    scatter(s->f.p_n, nv, 1, 0);
+    scatter(F_PN, nv, 1, 0);
     CU(cudaMemcpyAsync(p, s->stage_buf, nc * sizeof(double), cudaMemcpyDeviceToHost, st));
-    scatter(s->f.Vx_n, nv * 3, 3, 0);
-    scatter(s->f.Vy_n, nv * 3, 3, 1);
-    scatter(s->f.Vz_n, nv * 3, 3, 2);
+    scatter(F_VXN, nv * 3, 3, 0);
+    scatter(F_VYN, nv * 3, 3, 1);
+    scatter(F_VZN, nv * 3, 3, 2);
     CU(cudaMemcpyAsync(mom_h, s->stage_buf, nc * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
     k_fill<<<flat_blocks(size_t(N) * (nv + 1)), 256, 0, st>>>(size_t(N) * (nv + 1), s->stage_buf, 0.0);   // lid = 0
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    scatter(s->f.W_n, nv + 1, 1, 0);
+    scatter(F_WN, nv + 1, 1, 0);
     CU(cudaMemcpyAsync(W, s->stage_buf, size_t(N) * (nv + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(st));
@@ -313,8 +345,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (!s) return fail(THOR_EINVAL, "thor_step: null state");
     if (n_large < 0 || !(dt > 0) || n < 2 || (n & 1)) return fail(THOR_EINVAL, "thor_step: need n_large >= 0, dt > 0, even n >= 2");
     const HostGrid& h = s->grid->h;
-    const int N = h.N, nv = h.nv;
-    const size_t nc = size_t(N) * nv;
+    const int nv = h.nv, Npad = s->grid->d.Npad;
     cudaStream_t st = s->stream;
     if (forcing && !forcing->resident) {
         int rc;
@@ -323,25 +354,24 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
         if (s->has_kT && (rc = upload_table(s, forcing->k_T, &s->tab_kT))) return rc;
         if (s->has_kv && (rc = upload_table(s, forcing->k_v, &s->tab_kv))) return rc;
     }
-    Fields f = s->f;
-    f.T_eq = (forcing && s->has_Teq) ? s->tab_Teq : nullptr;
-    f.k_T = (forcing && s->has_kT) ? s->tab_kT : nullptr;
-    f.k_v = (forcing && s->has_kv) ? s->tab_kv : nullptr;
+    Forcing F;
+    F.T_eq = (forcing && s->has_Teq) ? s->tab_Teq : nullptr;
+    F.k_T = (forcing && s->has_kT) ? s->tab_kT : nullptr;
+    F.k_v = (forcing && s->has_kv) ? s->tab_kv : nullptr;
     const Geom g = make_geom(s->grid);
+    double* S = s->S;
     for (int step = 0; step < n_large; ++step) {
         for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
             const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
             const double delta = stage == 1 ? dt / 3.0 : dt / n;
-            THOR_DISPATCH(k_stage_prepare, nv, N, st, g, f, stage, delta);
-            THOR_DISPATCH(k_slow_terms, nv, N, st, g, f);
+            THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta);
+            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S);
             for (int sub = 0; sub < ns; ++sub) {
-                THOR_DISPATCH(k_momentum, nv, N, st, g, f, delta);
-                THOR_DISPATCH(k_vertical, nv, N, st, g, f, delta);
+                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta);
+                THOR_DISPATCH(k_vertical, nv, Npad, st, g, S, delta, sub == 0 ? 1 : 0);
             }
-            s->last_delta = delta;
         }
-        k_finish<<<flat_blocks(nc), 256, 0, st>>>(nc, f, dt, g.Rd);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
+        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt);
     }
     CU(cudaGetLastError());
     s->stepped = s->stepped || n_large > 0;
@@ -353,11 +383,11 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     if (n_substeps < 0 || !(delta > 0) || which < 1 || which > 3) return fail(THOR_EINVAL, "thor_acoustic_substeps: bad argument");
     if (!s->stepped) return fail(THOR_EINVAL, "thor_acoustic_substeps: call thor_step first (no stage data yet)");
     const HostGrid& h = s->grid->h;
+    const int Npad = s->grid->d.Npad;
     const Geom g = make_geom(s->grid);
-    Fields f = s->f;
     for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, h.N, s->stream, g, f, delta);
-        if (which & 2) THOR_DISPATCH(k_vertical, h.nv, h.N, s->stream, g, f, delta);
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta);
+        if (which & 2) THOR_DISPATCH(k_vertical, h.nv, Npad, s->stream, g, s->S, delta, 0);
     }
     CU(cudaGetLastError());
     return THOR_OK;
@@ -367,7 +397,7 @@ int thor_diagnostics(const thor_state* s, thor_diag* out) {
     if (!s || !out) return fail(THOR_EINVAL, "thor_diagnostics: null argument");
     const HostGrid& h = s->grid->h;
     const Geom g = make_geom(s->grid);
-    THOR_DISPATCH(k_diag, h.nv, h.N, s->stream, g, s->f, s->col_mass, s->col_energy);
+    THOR_DISPATCH(k_diag, h.nv, s->grid->d.Npad, s->stream, g, s->S, s->col_mass, s->col_energy);
     CU(cudaGetLastError());
     std::vector<double> m(h.N), e(h.N);
     CU(cudaMemcpyAsync(m.data(), s->col_mass, h.N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
@@ -395,7 +425,7 @@ int thor_apply_div_device(const thor_grid* grid, const double* vx, const double*
     if (rc) return rc;
     const Geom g = make_geom(grid);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    THOR_DISPATCH(k_div, g.nv, g.N, st, g, vx, vy, vz, out);
+    THOR_DISPATCH_OP(k_div, g.nv, g.N, st, g, vx, vy, vz, out);
     CU(cudaGetLastError());
     return THOR_OK;
 }
@@ -407,7 +437,7 @@ int thor_apply_grad_device(const thor_grid* grid, const double* sfield, double* 
     if (rc) return rc;
     const Geom g = make_geom(grid);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    THOR_DISPATCH(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
+    THOR_DISPATCH_OP(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
     CU(cudaGetLastError());
     return THOR_OK;
 }

@@ -1,12 +1,21 @@
 // sm_100a kernels of the THOR HE-VI large step (Fig. 6).
 //
-// Data layout: every field is its own [column][layer] FP64 array, layer
-// fastest, columns in the locality-preserving device order.  A column is owned by a group of G
-// lanes (G = 8, 16 or 32); each lane holds E consecutive layers (layer = lane_in_group*E + e), so a
-// neighbour-column read is one contiguous row (256 B at 32 layers, 512 B at 64) and vertical
-// neighbours are either in the same lane or one shuffle away.  W (= rho v_r) is stored on the LOWER
-// interface of each layer (slot 0 = ground = 0; the lid above the top layer is an implicit 0), so
-// every array has the same stride.
+// Data layout in HBM: ONE slab of column records, columns in the
+// locality-preserving device order, padded to a whole number of thread blocks:
+//
+//     S[column][field][layer]     field = one of the NF rows below, layer fastest, NVP doubles per row
+//
+// NVP = G*E is the layer count rounded up to 8/16/32/64/128.  A column is owned by a group of G
+// lanes; each lane holds E (even) CONSECUTIVE layers, so every row access is a 128-bit load/store,
+// a neighbour column's row is one contiguous 8*NVP-byte segment, every field of a column sits at a
+// compile-time offset from one base address, and vertical neighbours are in the same lane or one
+// shuffle away.  The rows a kernel reads together are adjacent in the record (the acoustic
+// column-solve kernel reads rows 0..16 of its own column: one contiguous 17*NVP*8-byte block).
+//
+// W (= rho v_r) is stored on the LOWER interface of each layer (slot 0 = ground = 0; the lid above
+// the top layer is an implicit 0).  Pad layers (k >= n_layers) and pad columns hold exact zeros in
+// every deviation / slow-term / LU-factor row and harmless finite values elsewhere, so they never
+// need a branch and never leak into real layers (see "pad invariant" in DESIGN.md).
 //
 // The path is an HBM-bound 7-point gather plus a per-column recurrence: no tensor cores.
 #pragma once
@@ -16,58 +25,97 @@ namespace thor {
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kWarpsPerBlock = 8;
+constexpr int kColPad = 64;      // columns are padded to a multiple of this (>= columns per block of any shape)
+constexpr int kEosTerms = 11;    // degree of the binomial series of Eq. 36 in deviation form
+constexpr double kEosSmall = 0.03125;   // |x| <= 2^-5: series; beyond: expm1/log1p
 
-struct Geom {                 // device pointers, device column order
-    int N, nv;
-    const int* nbr;           // [N][6]
-    const double* wdiv;       // [N][7][3]
-    const double* wgrad;      // [N][6][3]
-    const double* rhat;       // [N][3]
-    const double* area;       // [N]
-    const double* rinv;       // [nv]
-    const double* dlo;        // [nv]
-    const double* dhi;        // [nv]
-    const double* vol;        // [nv]
-    const double* zc;         // [nv]
-    double dz, omega, gravity, Rd, Cp, p_ref;
+// rows of a column record
+enum Field : int {
+    // --- acoustic substep, gathered from the 6 neighbours by the column-solve kernel
+    F_VXS = 0, F_VYS, F_VZS,     // V* = (rho v_h)*, Cartesian                     (Eq. 31, 33)
+    F_H, F_TH,                   // h = Cp T, theta of the stage reference state   (Eq. 38)
+    // --- acoustic substep, column-local
+    F_PS,                        // p*        (gathered by the momentum kernel)
+    F_RHOS, F_WS, F_RTS,         // rho*, W* = (rho v_r)*, (rho theta)*
+    F_SRHO, F_SP, F_SW, F_SRT,   // slow terms of Eq. 32, 40, 42, 35
+    F_FA, F_FI, F_FC,            // LU factors of the tridiagonal matrix of Eq. 37
+    F_PT, F_IRT,                 // p^[t], 1/(rho theta)^[t]
+    F_SVX, F_SVY, F_SVZ,         // slow term of Eq. 33
+    // --- stage reference state Phi^[t] (R1) and the un-projected velocity (L268)
+    F_VXT, F_VYT, F_VZT, F_UX, F_UY, F_UZ, F_RHOT, F_WT,
+    // --- Phi^n (the prognostic state between large steps) and (rho theta)^n
+    F_RHON, F_VXN, F_VYN, F_VZN, F_WN, F_PN, F_RTN,
+    NF
 };
 
-struct Fields {               // device pointers, each [N][nv]
-    // Phi^n (the prognostic state between large steps)
-    double *rho_n, *Vx_n, *Vy_n, *Vz_n, *W_n, *p_n, *rt_n;
-    // Phi^[t] (reference state of the current Runge-Kutta stage, R1)
-    double *rho_t, *Vx_t, *Vy_t, *Vz_t, *W_t, *p_t;
-    // stage coefficients (Eq. 38-39) and the factorised tridiagonal matrix of Eq. 37
-    double *h, *th, *ux, *uy, *uz, *fa, *fi, *fc;
-    // slow terms (RHS of Eq. 32-35, Eq. 42)
-    double *sVx, *sVy, *sVz, *srho, *sW, *sp, *srt;
-    // deviations Phi* (Eq. 31) and the full rho*theta
-    double *rho_s, *Vx_s, *Vy_s, *Vz_s, *W_s, *p_s, *rt;
-    // forcing tables (Eq. 51-52), may be null
+struct Geom {                 // device pointers, device column order, padded to Npad columns
+    int N, Npad, nv;
+    const int* nbr;           // [Npad][8]   6 neighbours (pentagons, pad columns: self), 2 x self
+    const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad
+    const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)
+    const double* rhat;       // [Npad][4]   unit vector of the column, 1 pad
+    const double* area;       // [Npad]
+    const double* rinv;       // [128] 1/r_k              (pad layers: 0)
+    const double* dlo;        // [128] r_h,k^2/(r_k^2 dz)
+    const double* dhi;        // [128] r_h,k+1^2/(r_k^2 dz)
+    const double* vol;        // [128] r_k^2 dz
+    const double* zc;         // [128]
+    double dz, omega, gravity, Rd, Cp, p_ref;
+    double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
+};
+
+struct Forcing {              // [Npad][NVP] each, may be null (Eq. 51-52)
     const double *T_eq, *k_T, *k_v;
 };
 
 // ---------------------------------------------------------------------------------------------
-// lane <-> (column, layer) mapping and vertical neighbour access
+// lane <-> (column, layers) mapping of the record kernels
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
-struct Lanes {
-    int col;        // device column (clamped to N-1 so that every lane takes part in the shuffles)
-    bool live;      // col < N
-    int gl;         // lane within the group
-    int k0;         // first layer of this lane
-    __device__ Lanes(int N) {
+struct Map {
+    static_assert(E % 2 == 0, "two layers per 128-bit access");
+    static constexpr int NVP = G * E;
+    static constexpr int CPW = 32 / G;                 // columns per warp
+    static constexpr size_t REC = size_t(NF) * NVP;    // doubles per column record
+    int col, gl, k0;
+    __device__ Map() {
         const int lane = threadIdx.x & 31;
         const int warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-        const int c = warp * (32 / G) + lane / G;
-        live = c < N;
-        col = live ? c : N - 1;
+        col = warp * CPW + lane / G;                   // < Npad by construction of the grid
         gl = lane & (G - 1);
         k0 = gl * E;
     }
 };
 
-// value at layer k-1 (fill at the bottom)
+template <int E>
+__device__ __forceinline__ void ld_nc(const double* p, double (&v)[E]) {     // rows nobody writes in this kernel
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+        const double2 t = __ldg(reinterpret_cast<const double2*>(p) + i);
+        v[2 * i] = t.x; v[2 * i + 1] = t.y;
+    }
+}
+template <int E>
+__device__ __forceinline__ void ld_rw(const double* p, double (&v)[E]) {
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+        const double2 t = reinterpret_cast<const double2*>(p)[i];
+        v[2 * i] = t.x; v[2 * i + 1] = t.y;
+    }
+}
+template <int E>
+__device__ __forceinline__ void st_row(double* p, const double (&v)[E]) {
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) reinterpret_cast<double2*>(p)[i] = make_double2(v[2 * i], v[2 * i + 1]);
+}
+
+__device__ __forceinline__ double3 ld_rhat(const double* rhat, int col) {   // [Npad][4]
+    const double2 a = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col));
+    const double2 b = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col) + 1);
+    return make_double3(a.x, a.y, b.x);
+}
+
+// value at layer k-1 (fill below the ground)
 template <int G, int E>
 __device__ __forceinline__ void below(const double (&v)[E], double (&out)[E], int gl, double fill) {
     double prev = __shfl_up_sync(kFull, v[E - 1], 1, G);
@@ -76,7 +124,7 @@ __device__ __forceinline__ void below(const double (&v)[E], double (&out)[E], in
 #pragma unroll
     for (int e = 1; e < E; ++e) out[e] = v[e - 1];
 }
-// value at layer k+1 (fill above the last lane; masked layers must already hold the fill value)
+// value at layer k+1 (fill above the last lane)
 template <int G, int E>
 __device__ __forceinline__ void above(const double (&v)[E], double (&out)[E], int gl, double fill) {
     double next = __shfl_down_sync(kFull, v[0], 1, G);
@@ -86,29 +134,24 @@ __device__ __forceinline__ void above(const double (&v)[E], double (&out)[E], in
     out[E - 1] = next;
 }
 
-template <int E>
-__device__ __forceinline__ void load_row(const double* __restrict__ base, int k0, int nv, double (&v)[E]) {
-#pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = (k0 + e < nv) ? __ldg(base + k0 + e) : 0.0;
-}
-template <int E>
-__device__ __forceinline__ void load_row_rw(const double* base, int k0, int nv, double (&v)[E]) {
-#pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = (k0 + e < nv) ? base[k0 + e] : 0.0;
-}
-template <int E>
-__device__ __forceinline__ void store_row(double* base, int k0, int nv, bool live, const double (&v)[E]) {
-#pragma unroll
-    for (int e = 0; e < E; ++e)
-        if (live && k0 + e < nv) base[k0 + e] = v[e];
-}
-
 // Eq. 24 (L210) and its inverse
-__device__ __forceinline__ double eos_p(double rt, double Rd, double p_ref, double gam) {
-    return p_ref * pow(Rd * rt / p_ref, gam);
-}
 __device__ __forceinline__ double eos_rt(double p, double Rd, double p_ref, double inv_gam) {
     return p_ref / Rd * pow(p / p_ref, inv_gam);
+}
+
+// Eq. 36 (L270) in deviation form: with x = (rho theta)* / (rho theta)^[t],
+//   p* = p_ref (Rd (rho theta)/p_ref)^gamma - p^[t] = p^[t] ((1 + x)^gamma - 1)
+//      = p^[t] gamma x (1 + q_1 x + q_2 x^2 + ...),   q_k = C(gamma, k+1)/gamma.
+// Free of the cancellation of the printed form.  |x| <= 2^-5: the series is
+// below 2^-57 relative after kEosTerms terms; beyond, expm1(gamma log1p x).
+__device__ __forceinline__ double eos_dev(double x, double pt, double gam, const Geom& g) {
+    if (fabs(x) <= kEosSmall) {
+        double q = g.eosq[kEosTerms];
+#pragma unroll
+        for (int k = kEosTerms - 1; k >= 0; --k) q = fma(q, x, g.eosq[k]);
+        return (pt * gam) * x * q;
+    }
+    return pt * expm1(gam * log1p(x));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -118,7 +161,6 @@ __device__ __forceinline__ double eos_rt(double p, double Rd, double p_ref, doub
 // ---------------------------------------------------------------------------------------------
 template <int G, int E, bool DOWN>
 __device__ __forceinline__ void affine_scan(const double (&A)[E], const double (&B)[E], double (&y)[E], int gl) {
-    // compose this lane's E maps into one: y_out = a * y_in + b
     double a = 1.0, b = 0.0;
     if (!DOWN) {
 #pragma unroll
@@ -134,7 +176,6 @@ __device__ __forceinline__ void affine_scan(const double (&A)[E], const double (
         const bool has = DOWN ? (gl + s < G) : (gl >= s);
         if (has) { b = fma(a, bp, b); a = a * ap; }
     }
-    // carry entering this lane = inclusive result of the previous lane
     double carry = DOWN ? __shfl_down_sync(kFull, b, 1, G) : __shfl_up_sync(kFull, b, 1, G);
     if (DOWN ? (gl == G - 1) : (gl == 0)) carry = 0.0;
     if (!DOWN) {
@@ -147,34 +188,48 @@ __device__ __forceinline__ void affine_scan(const double (&A)[E], const double (
 }
 
 // ---------------------------------------------------------------------------------------------
-// Config-1 operators (Eq. 6 and Eq. 7), one row per (column, lane group)
+// Config-1 operators (Eq. 6 and Eq. 7) on caller-owned [column][layer] arrays (row length nv, no
+// padding): G lanes per column, E layers per lane with stride G (coalesced scalar accesses).
 // ---------------------------------------------------------------------------------------------
+template <int G, int E>
+struct Lanes {
+    int col; bool live; int gl;
+    __device__ Lanes(int N) {
+        const int lane = threadIdx.x & 31;
+        const int warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+        const int c = warp * (32 / G) + lane / G;
+        live = c < N;
+        col = live ? c : N - 1;
+        gl = lane & (G - 1);
+    }
+};
+
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_div(Geom g, const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
       double* __restrict__ out) {
     Lanes<G, E> L(g.N);
     const int nv = g.nv;
-    const double* w = g.wdiv + size_t(L.col) * 21;
+    const double* w = g.wdiv + size_t(L.col) * 24;
     double acc[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) acc[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
-        const int c = j == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 6 + j - 1);
+        const int c = j == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 8 + j - 1);
         const double wx = __ldg(w + 3 * j), wy = __ldg(w + 3 * j + 1), wz = __ldg(w + 3 * j + 2);
-        double x[E], y[E], z[E];
-        load_row<E>(vx + size_t(c) * nv, L.k0, nv, x);
-        load_row<E>(vy + size_t(c) * nv, L.k0, nv, y);
-        load_row<E>(vz + size_t(c) * nv, L.k0, nv, z);
+        const size_t o = size_t(c) * nv;
 #pragma unroll
-        for (int e = 0; e < E; ++e) acc[e] = fma(wx, x[e], fma(wy, y[e], fma(wz, z[e], acc[e])));
+        for (int e = 0; e < E; ++e) {
+            const int k = L.gl + e * G;
+            if (k < nv) acc[e] = fma(wx, __ldg(vx + o + k), fma(wy, __ldg(vy + o + k), fma(wz, __ldg(vz + o + k), acc[e])));
+        }
     }
-    double ri[E];
-    load_row<E>(g.rinv, L.k0, nv, ri);
 #pragma unroll
-    for (int e = 0; e < E; ++e) acc[e] *= ri[e];
-    store_row<E>(out + size_t(L.col) * nv, L.k0, nv, L.live, acc);
+    for (int e = 0; e < E; ++e) {
+        const int k = L.gl + e * G;
+        if (L.live && k < nv) out[size_t(L.col) * nv + k] = acc[e] * __ldg(g.rinv + k);
+    }
 }
 
 template <int G, int E>
@@ -185,91 +240,88 @@ k_grad(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* __
     const int nv = g.nv;
     const double* w = g.wgrad + size_t(L.col) * 18;
     double s0[E], ax[E], ay[E], az[E];
-    load_row<E>(s + size_t(L.col) * nv, L.k0, nv, s0);
 #pragma unroll
-    for (int e = 0; e < E; ++e) ax[e] = ay[e] = az[e] = 0.0;
+    for (int e = 0; e < E; ++e) {
+        const int k = L.gl + e * G;
+        s0[e] = k < nv ? __ldg(s + size_t(L.col) * nv + k) : 0.0;
+        ax[e] = ay[e] = az[e] = 0.0;
+    }
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const int c = __ldg(g.nbr + size_t(L.col) * 6 + j);
+        const int c = __ldg(g.nbr + size_t(L.col) * 8 + j);
         const double wx = __ldg(w + 3 * j), wy = __ldg(w + 3 * j + 1), wz = __ldg(w + 3 * j + 2);
-        double sj[E];
-        load_row<E>(s + size_t(c) * nv, L.k0, nv, sj);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double d = sj[e] - s0[e];
+            const int k = L.gl + e * G;
+            const double d = (k < nv ? __ldg(s + size_t(c) * nv + k) : 0.0) - s0[e];
             ax[e] = fma(wx, d, ax[e]); ay[e] = fma(wy, d, ay[e]); az[e] = fma(wz, d, az[e]);
         }
     }
-    double ri[E];
-    load_row<E>(g.rinv, L.k0, nv, ri);
 #pragma unroll
-    for (int e = 0; e < E; ++e) { ax[e] *= ri[e]; ay[e] *= ri[e]; az[e] *= ri[e]; }
-    store_row<E>(gx + size_t(L.col) * nv, L.k0, nv, L.live, ax);
-    store_row<E>(gy + size_t(L.col) * nv, L.k0, nv, L.live, ay);
-    store_row<E>(gz + size_t(L.col) * nv, L.k0, nv, L.live, az);
+    for (int e = 0; e < E; ++e) {
+        const int k = L.gl + e * G;
+        if (L.live && k < nv) {
+            const double ri = __ldg(g.rinv + k);
+            const size_t o = size_t(L.col) * nv + k;
+            gx[o] = ax[e] * ri; gy[o] = ay[e] * ri; gz[o] = az[e] * ri;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
 // S1: stage preparation (column-local).  Fig. 6 large-step 4 of the previous stage and
 // large-step 1 of this one:  Phi^[t] <- Phi^n (stage 1) or Phi^[t] + Phi* (stages 2, 3);
-// h = Cp p/(Rd rho) (Eq. 38, G9), theta, u = (V + I_c[W] r)/rho (L268), g~ (Eq. 39) and the
-// LU factors of the tridiagonal matrix of Eq. 37 (coefficients: DESIGN.md "tridiagonal", R8) for
-// this stage's substep length delta.  The matrix does not change between the substeps of a
-// stage, so its factorisation is done once here and the substeps only run the two sweeps.
+// h = Cp p/(Rd rho) (Eq. 38, G9), theta, u = (V + I_c[W] r)/rho (L268), the LU factors of the
+// tridiagonal matrix of Eq. 37 (g~ of Eq. 39 inside; coefficients: DESIGN.md "tridiagonal", R8) for
+// this stage's substep length delta, and the initial deviations of Eq. 31 (R1: every stage starts
+// from t_n).  The matrix does not change between the substeps of a stage, so it is factorised
+// once here and the substeps only run the two sweeps.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_stage_prepare(Geom g, Fields f, int stage, double delta) {
-    Lanes<G, E> L(g.N);
+k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
     const int nv = g.nv;
-    const size_t o = size_t(L.col) * nv;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
-    double rho[E], Vx[E], Vy[E], Vz[E], W[E], p[E];
+    bool real[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) real[e] = (L.k0 + e < nv) && (L.col < g.N);
+
+    double rho[E], Vx[E], Vy[E], Vz[E], W[E], p[E], d[E];
     if (stage == 1) {
-        load_row_rw<E>(f.rho_n + o, L.k0, nv, rho); load_row_rw<E>(f.Vx_n + o, L.k0, nv, Vx);
-        load_row_rw<E>(f.Vy_n + o, L.k0, nv, Vy);   load_row_rw<E>(f.Vz_n + o, L.k0, nv, Vz);
-        load_row_rw<E>(f.W_n + o, L.k0, nv, W);     load_row_rw<E>(f.p_n + o, L.k0, nv, p);
+        ld_rw<E>(me + F_RHON * NVP, rho); ld_rw<E>(me + F_VXN * NVP, Vx); ld_rw<E>(me + F_VYN * NVP, Vy);
+        ld_rw<E>(me + F_VZN * NVP, Vz);   ld_rw<E>(me + F_WN * NVP, W);   ld_rw<E>(me + F_PN * NVP, p);
     } else {
-        double d[E];
-        load_row_rw<E>(f.rho_t + o, L.k0, nv, rho); load_row_rw<E>(f.rho_s + o, L.k0, nv, d);
+        auto add = [&](int ft, int fs, double (&out)[E]) {
+            ld_rw<E>(me + ft * NVP, out); ld_rw<E>(me + fs * NVP, d);
 #pragma unroll
-        for (int e = 0; e < E; ++e) rho[e] += d[e];
-        load_row_rw<E>(f.Vx_t + o, L.k0, nv, Vx); load_row_rw<E>(f.Vx_s + o, L.k0, nv, d);
-#pragma unroll
-        for (int e = 0; e < E; ++e) Vx[e] += d[e];
-        load_row_rw<E>(f.Vy_t + o, L.k0, nv, Vy); load_row_rw<E>(f.Vy_s + o, L.k0, nv, d);
-#pragma unroll
-        for (int e = 0; e < E; ++e) Vy[e] += d[e];
-        load_row_rw<E>(f.Vz_t + o, L.k0, nv, Vz); load_row_rw<E>(f.Vz_s + o, L.k0, nv, d);
-#pragma unroll
-        for (int e = 0; e < E; ++e) Vz[e] += d[e];
-        load_row_rw<E>(f.W_t + o, L.k0, nv, W); load_row_rw<E>(f.W_s + o, L.k0, nv, d);
-#pragma unroll
-        for (int e = 0; e < E; ++e) W[e] += d[e];
-        load_row_rw<E>(f.p_t + o, L.k0, nv, p); load_row_rw<E>(f.p_s + o, L.k0, nv, d);
-#pragma unroll
-        for (int e = 0; e < E; ++e) p[e] += d[e];
+            for (int e = 0; e < E; ++e) out[e] += d[e];
+        };
+        add(F_RHOT, F_RHOS, rho); add(F_VXT, F_VXS, Vx); add(F_VYT, F_VYS, Vy); add(F_VZT, F_VZS, Vz);
+        add(F_WT, F_WS, W);       add(F_PT, F_PS, p);
     }
-    // masked layers: harmless non-zero values so that nothing divides by zero
 #pragma unroll
     for (int e = 0; e < E; ++e)
-        if (L.k0 + e >= nv) { rho[e] = 1.0; p[e] = g.p_ref; }
+        if (!real[e]) { rho[e] = 1.0; p[e] = g.p_ref; Vx[e] = Vy[e] = Vz[e] = W[e] = 0.0; }
 
-    const double rx = __ldg(g.rhat + 3 * L.col), ry = __ldg(g.rhat + 3 * L.col + 1), rz = __ldg(g.rhat + 3 * L.col + 2);
-    double h[E], th[E], rtt[E], Wup[E], ux[E], uy[E], uz[E];
+    const double3 rh = ld_rhat(g.rhat, L.col);
+    double h[E], th[E], rtt[E], irt[E], Wup[E], ux[E], uy[E], uz[E];
     above<G, E>(W, Wup, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         h[e] = g.Cp * p[e] / (g.Rd * rho[e]);
         rtt[e] = eos_rt(p[e], g.Rd, g.p_ref, 1.0 / gam);
         th[e] = rtt[e] / rho[e];
-        const double wc = (L.k0 + e == nv - 1) ? 0.5 * W[e] : 0.5 * (W[e] + Wup[e]);   // I_c[W]
+        irt[e] = 1.0 / rtt[e];
+        const double wc = 0.5 * (W[e] + Wup[e]);                            // I_c[W]; the lid's W is the pad's 0
         const double ir = 1.0 / rho[e];
-        ux[e] = (Vx[e] + wc * rx) * ir; uy[e] = (Vy[e] + wc * ry) * ir; uz[e] = (Vz[e] + wc * rz) * ir;
+        ux[e] = (Vx[e] + wc * rh.x) * ir; uy[e] = (Vy[e] + wc * rh.y) * ir; uz[e] = (Vz[e] + wc * rh.z) * ir;
     }
     // interface quantities on the lower interface of each layer
     double pb[E], rb[E], hb[E], hh[E], gt[E];
-    below<G, E>(p, pb, L.gl, 0.0); below<G, E>(rho, rb, L.gl, 0.0); below<G, E>(h, hb, L.gl, 0.0);
+    below<G, E>(p, pb, L.gl, 0.0); below<G, E>(rho, rb, L.gl, 1.0); below<G, E>(h, hb, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
@@ -280,80 +332,98 @@ k_stage_prepare(Geom g, Fields f, int stage, double delta) {
     double hhb[E], hha[E], gtb[E], gta[E], dlo[E], dhi[E], dlob[E], dhib[E];
     below<G, E>(hh, hhb, L.gl, 0.0); above<G, E>(hh, hha, L.gl, 0.0);
     below<G, E>(gt, gtb, L.gl, 0.0); above<G, E>(gt, gta, L.gl, 0.0);
-    load_row<E>(g.dlo, L.k0, nv, dlo); load_row<E>(g.dhi, L.k0, nv, dhi);
+    ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
     below<G, E>(dlo, dlob, L.gl, 0.0); below<G, E>(dhi, dhib, L.gl, 0.0);
     double ta[E], tb[E], tc[E];
     const double d2 = delta * delta, ck = d2 * kv / g.dz, cg = 0.5 * d2 * g.gravity;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-        const int k = L.k0 + e;
-        // the top interior interface (k = nv-1) has no unknown above it: hh, g~ there are the lid's 0
-        const double hu = (k + 1 < nv) ? hha[e] : 0.0, gu = (k + 1 < nv) ? gta[e] : 0.0;
-        tc[e] = -ck * (dhi[e] * hu - 0.5 * gu) - cg * dhi[e];
+        // hh, g~ are 0 on the lid and on the ground: a_1 and c_(nv-1) multiply the zero boundary values
+        tc[e] = -ck * (dhi[e] * hha[e] - 0.5 * gta[e]) - cg * dhi[e];
         ta[e] = -ck * (dlob[e] * hhb[e] + 0.5 * gtb[e]) + cg * dlob[e];
         tb[e] = 1.0 + ck * hh[e] * (dlo[e] + dhib[e]) - cg * (dhib[e] - dlo[e]);
     }
-    // Thomas forward elimination of the matrix (L339), serial over the interfaces; every lane of the
-    // group follows the same recurrence and keeps the factors of its own interfaces.
+    // Thomas forward elimination of the matrix (L339): c'_k = c_k/(b_k - a_k c'_(k-1)), serial over the
+    // interfaces.  Lane by lane: in phase l every lane runs its own E steps from the carry it holds,
+    // only lane l's carry-in is the true c'_(k0-1); its carry-out is then handed to the whole group.
+    // fi = 1/b'_k, fa = a_k/b'_k, fc = c'_k; all three stay 0 on the ground, on pads and in pad columns.
     double fa[E], fi[E], fc[E];
+    double carry = 0.0;
+    for (int l = 0; l < G; ++l) {
+        double cp = carry;
 #pragma unroll
-    for (int e = 0; e < E; ++e) fa[e] = fi[e] = fc[e] = 0.0;
-    double cprev = 0.0;
-    const int gbase = (threadIdx.x & 31) & ~(G - 1);
-    for (int kk = 1; kk < nv; ++kk) {
-        const int src = kk / E, ee = kk % E;
-        double a_ = 0.0, b_ = 0.0, c_ = 0.0;
-#pragma unroll
-        for (int e = 0; e < E; ++e)
-            if (e == ee) { a_ = ta[e]; b_ = tb[e]; c_ = tc[e]; }
-        a_ = __shfl_sync(kFull, a_, gbase + src);
-        b_ = __shfl_sync(kFull, b_, gbase + src);
-        c_ = __shfl_sync(kFull, c_, gbase + src);
-        const double inv = 1.0 / (b_ - a_ * cprev);
-        cprev = c_ * inv;
-#pragma unroll
-        for (int e = 0; e < E; ++e)
-            if (L.k0 + e == kk) { fi[e] = inv; fa[e] = a_ * inv; fc[e] = cprev; }
+        for (int e = 0; e < E; ++e) {
+            const int k = L.k0 + e;
+            const bool in = k >= 1 && k < nv && L.col < g.N;
+            const double inv = 1.0 / (tb[e] - ta[e] * cp);
+            cp = in ? tc[e] * inv : 0.0;
+            if (L.gl == l) { fi[e] = in ? inv : 0.0; fa[e] = in ? ta[e] * inv : 0.0; fc[e] = cp; }
+        }
+        carry = __shfl_sync(kFull, cp, l, G);
     }
-    store_row<E>(f.rho_t + o, L.k0, nv, L.live, rho); store_row<E>(f.Vx_t + o, L.k0, nv, L.live, Vx);
-    store_row<E>(f.Vy_t + o, L.k0, nv, L.live, Vy);   store_row<E>(f.Vz_t + o, L.k0, nv, L.live, Vz);
-    store_row<E>(f.W_t + o, L.k0, nv, L.live, W);     store_row<E>(f.p_t + o, L.k0, nv, L.live, p);
-    store_row<E>(f.h + o, L.k0, nv, L.live, h);       store_row<E>(f.th + o, L.k0, nv, L.live, th);
-    store_row<E>(f.ux + o, L.k0, nv, L.live, ux);     store_row<E>(f.uy + o, L.k0, nv, L.live, uy);
-    store_row<E>(f.uz + o, L.k0, nv, L.live, uz);
-    store_row<E>(f.fa + o, L.k0, nv, L.live, fa);     store_row<E>(f.fi + o, L.k0, nv, L.live, fi);
-    store_row<E>(f.fc + o, L.k0, nv, L.live, fc);
-    if (stage == 1) store_row<E>(f.rt_n + o, L.k0, nv, L.live, rtt);   // (rho theta)^n, start of every stage
+    st_row<E>(me + F_RHOT * NVP, rho); st_row<E>(me + F_VXT * NVP, Vx); st_row<E>(me + F_VYT * NVP, Vy);
+    st_row<E>(me + F_VZT * NVP, Vz);   st_row<E>(me + F_WT * NVP, W);   st_row<E>(me + F_PT * NVP, p);
+    st_row<E>(me + F_H * NVP, h);      st_row<E>(me + F_TH * NVP, th);  st_row<E>(me + F_IRT * NVP, irt);
+    st_row<E>(me + F_UX * NVP, ux);    st_row<E>(me + F_UY * NVP, uy);  st_row<E>(me + F_UZ * NVP, uz);
+    st_row<E>(me + F_FA * NVP, fa);    st_row<E>(me + F_FI * NVP, fi);  st_row<E>(me + F_FC * NVP, fc);
+
+    // Eq. 31: Phi*(0) = Phi^n - Phi^[t]; (rho theta)*(0) = (rho theta)^n - (rho theta)^[t]
+    if (stage == 1) {
+        st_row<E>(me + F_RTN * NVP, rtt);
+#pragma unroll
+        for (int e = 0; e < E; ++e) d[e] = 0.0;
+        st_row<E>(me + F_RHOS * NVP, d); st_row<E>(me + F_VXS * NVP, d); st_row<E>(me + F_VYS * NVP, d);
+        st_row<E>(me + F_VZS * NVP, d);  st_row<E>(me + F_WS * NVP, d);  st_row<E>(me + F_PS * NVP, d);
+        st_row<E>(me + F_RTS * NVP, d);
+    } else {
+        auto dev = [&](int fn, int fs, const double (&t)[E]) {
+            ld_rw<E>(me + fn * NVP, d);
+#pragma unroll
+            for (int e = 0; e < E; ++e) d[e] = real[e] ? d[e] - t[e] : 0.0;
+            st_row<E>(me + fs * NVP, d);
+        };
+        dev(F_RHON, F_RHOS, rho); dev(F_VXN, F_VXS, Vx); dev(F_VYN, F_VYS, Vy); dev(F_VZN, F_VZS, Vz);
+        dev(F_WN, F_WS, W);       dev(F_PN, F_PS, p);    dev(F_RTN, F_RTS, rtt);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
-// S2: slow terms of the stage (Fig. 6 large-step 3; RHS of Eq. 32-35 and Eq. 42; O4 with R7) and
-// the initial deviations of Eq. 31 (R1: every stage starts from t_n).
+// S2: slow terms of the stage (Fig. 6 large-step 3; RHS of Eq. 32-35 and Eq. 42; O4 with R7).
+// Gathers V^[t](3), h, theta, u(3), p^[t] from the 6 neighbours.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_slow_terms(Geom g, Fields f) {
-    Lanes<G, E> L(g.N);
+k_slow_terms(Geom g, double* __restrict__ S) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC;
+    double* me = S + size_t(L.col) * REC + L.k0;
     const int nv = g.nv;
-    const size_t o = size_t(L.col) * nv;
     const double kv = g.Rd / (g.Cp - g.Rd);
-    const double* wd = g.wdiv + size_t(L.col) * 21;
-    const double* wg = g.wgrad + size_t(L.col) * 18;
+    const double2* wd = reinterpret_cast<const double2*>(g.wdiv + size_t(L.col) * 24);
+    const double2* wg = reinterpret_cast<const double2*>(g.wgrad + size_t(L.col) * 18);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    double wdv[24], wgv[18];
+#pragma unroll
+    for (int i = 0; i < 12; ++i) { const double2 t = __ldg(wd + i); wdv[2 * i] = t.x; wdv[2 * i + 1] = t.y; }
+#pragma unroll
+    for (int i = 0; i < 9; ++i) { const double2 t = __ldg(wg + i); wgv[2 * i] = t.x; wgv[2 * i + 1] = t.y; }
 
-    double p0[E], h0[E], th0[E], rho[E], V0x[E], V0y[E], V0z[E], u0x[E], u0y[E], u0z[E];
-    load_row<E>(f.p_t + o, L.k0, nv, p0);
+    double p0[E], h0[E], th0[E], V0x[E], V0y[E], V0z[E], u0x[E], u0y[E], u0z[E];
+    ld_nc<E>(me + F_PT * NVP, p0);
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], gpx[E], gpy[E], gpz[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = Ax[e] = Ay[e] = Az[e] = gpx[e] = gpy[e] = gpz[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
-        const int c = j == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 6 + j - 1);
-        const size_t oc = size_t(c) * nv;
-        const double wx = __ldg(wd + 3 * j), wy = __ldg(wd + 3 * j + 1), wz = __ldg(wd + 3 * j + 2);
+        const double* q = S + size_t(nb[j]) * REC + L.k0;
+        const double wx = wdv[3 * j], wy = wdv[3 * j + 1], wz = wdv[3 * j + 2];
         double x[E], y[E], z[E], hj[E], tj[E], ujx[E], ujy[E], ujz[E], pj[E];
-        load_row<E>(f.Vx_t + oc, L.k0, nv, x); load_row<E>(f.Vy_t + oc, L.k0, nv, y); load_row<E>(f.Vz_t + oc, L.k0, nv, z);
-        load_row<E>(f.h + oc, L.k0, nv, hj);   load_row<E>(f.th + oc, L.k0, nv, tj);
-        load_row<E>(f.ux + oc, L.k0, nv, ujx); load_row<E>(f.uy + oc, L.k0, nv, ujy); load_row<E>(f.uz + oc, L.k0, nv, ujz);
+        ld_nc<E>(q + F_VXT * NVP, x); ld_nc<E>(q + F_VYT * NVP, y); ld_nc<E>(q + F_VZT * NVP, z);
+        ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
+        ld_nc<E>(q + F_UX * NVP, ujx); ld_nc<E>(q + F_UY * NVP, ujy); ld_nc<E>(q + F_UZ * NVP, ujz);
         if (j == 0) {
 #pragma unroll
             for (int e = 0; e < E; ++e) {
@@ -361,8 +431,8 @@ k_slow_terms(Geom g, Fields f) {
                 u0x[e] = ujx[e]; u0y[e] = ujy[e]; u0z[e] = ujz[e];
             }
         } else {
-            load_row<E>(f.p_t + oc, L.k0, nv, pj);
-            const double gx = __ldg(wg + 3 * (j - 1)), gy = __ldg(wg + 3 * (j - 1) + 1), gz = __ldg(wg + 3 * (j - 1) + 2);
+            ld_nc<E>(q + F_PT * NVP, pj);
+            const double gx = wgv[3 * (j - 1)], gy = wgv[3 * (j - 1) + 1], gz = wgv[3 * (j - 1) + 2];
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const double d = pj[e] - p0[e];
@@ -378,20 +448,16 @@ k_slow_terms(Geom g, Fields f) {
             Ax[e] = fma(ujx[e], d, Ax[e]); Ay[e] = fma(ujy[e], d, Ay[e]); Az[e] = fma(ujz[e], d, Az[e]);
         }
     }
-    double ri[E], dlo[E], dhi[E];
-    load_row<E>(g.rinv, L.k0, nv, ri); load_row<E>(g.dlo, L.k0, nv, dlo); load_row<E>(g.dhi, L.k0, nv, dhi);
+    double ri[E], dlo[E], dhi[E], rho[E], W[E], Wup[E];
+    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         divV[e] *= ri[e]; divhV[e] *= ri[e]; divtV[e] *= ri[e];
         Ax[e] *= ri[e]; Ay[e] *= ri[e]; Az[e] *= ri[e];
         gpx[e] *= ri[e]; gpy[e] *= ri[e]; gpz[e] *= ri[e];
     }
-    load_row<E>(f.rho_t + o, L.k0, nv, rho);
-#pragma unroll
-    for (int e = 0; e < E; ++e)
-        if (L.k0 + e >= nv) rho[e] = 1.0;
-    double W[E], Wup[E];
-    load_row<E>(f.W_t + o, L.k0, nv, W);
+    ld_nc<E>(me + F_RHOT * NVP, rho);
+    ld_nc<E>(me + F_WT * NVP, W);
     above<G, E>(W, Wup, L.gl, 0.0);
 
     // vertical flux divergences D_c[W I_h[q]] for q = u_x, u_y, u_z, h, theta, and D_c[W]
@@ -399,7 +465,7 @@ k_slow_terms(Geom g, Fields f) {
     auto vflux = [&](const double (&q)[E], double (&out)[E]) {
         below<G, E>(q, qb, L.gl, 0.0);
 #pragma unroll
-        for (int e = 0; e < E; ++e) X[e] = W[e] * 0.5 * (qb[e] + q[e]);    // W = 0 on the ground
+        for (int e = 0; e < E; ++e) X[e] = W[e] * 0.5 * (qb[e] + q[e]);    // W = 0 on the ground and on the lid
         above<G, E>(X, Xup, L.gl, 0.0);
 #pragma unroll
         for (int e = 0; e < E; ++e) out[e] = dhi[e] * Xup[e] - dlo[e] * X[e];
@@ -420,7 +486,8 @@ k_slow_terms(Geom g, Fields f) {
 #pragma unroll
     for (int e = 0; e < E; ++e) DW[e] = dhi[e] * Wup[e] - dlo[e] * W[e];
 
-    const double rx = __ldg(g.rhat + 3 * L.col), ry = __ldg(g.rhat + 3 * L.col + 1), rz = __ldg(g.rhat + 3 * L.col + 2);
+    const double3 rh = ld_rhat(g.rhat, L.col);
+    const double rx = rh.x, ry = rh.y, rz = rh.z;
     double sVx[E], sVy[E], sVz[E], Fr[E], srho[E], sp[E], srt[E];
     // g~ W on interfaces, then I_c
     double pb[E], rb[E], Z[E], Zup[E];
@@ -434,62 +501,33 @@ k_slow_terms(Geom g, Fields f) {
     above<G, E>(Z, Zup, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
+        const bool real = (L.k0 + e < nv) && (L.col < g.N);
         const double wc = 0.5 * (W[e] + Wup[e]);
         const double Mx = V0x[e] + wc * rx, My = V0y[e] + wc * ry;
         const double Cx = -2.0 * g.omega * My, Cy = 2.0 * g.omega * Mx;       // 2 Omega z x M
         const double Ar = Ax[e] * rx + Ay[e] * ry + Az[e] * rz;
         const double Cr = Cx * rx + Cy * ry;
         Fr[e] = Ar + Cr;
-        sVx[e] = -gpx[e] - (Ax[e] - Ar * rx) - (Cx - Cr * rx);
-        sVy[e] = -gpy[e] - (Ay[e] - Ar * ry) - (Cy - Cr * ry);
-        sVz[e] = -gpz[e] - (Az[e] - Ar * rz) - (0.0 - Cr * rz);
-        srho[e] = -divV[e] - DW[e];
+        sVx[e] = real ? -gpx[e] - (Ax[e] - Ar * rx) - (Cx - Cr * rx) : 0.0;
+        sVy[e] = real ? -gpy[e] - (Ay[e] - Ar * ry) - (Cy - Cr * ry) : 0.0;
+        sVz[e] = real ? -gpz[e] - (Az[e] - Ar * rz) - (0.0 - Cr * rz) : 0.0;
+        srho[e] = real ? -divV[e] - DW[e] : 0.0;
         const double vgp = (V0x[e] * gpx[e] + V0y[e] * gpy[e] + V0z[e] * gpz[e]) / rho[e];
-        sp[e] = -kv * (divhV[e] + DhW[e] - vgp - 0.5 * (Z[e] + Zup[e]));
-        srt[e] = -divtV[e] - DtW[e];
+        sp[e] = real ? -kv * (divhV[e] + DhW[e] - vgp - 0.5 * (Z[e] + Zup[e])) : 0.0;
+        srt[e] = real ? -divtV[e] - DtW[e] : 0.0;
     }
     double Frb[E], sW[E];
     below<G, E>(Fr, Frb, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
-        sW[e] = (k >= 1 && k < nv)
+        sW[e] = (k >= 1 && k < nv && L.col < g.N)
                     ? -(p0[e] - pb[e]) / g.dz - g.gravity * 0.5 * (rb[e] + rho[e]) - 0.5 * (Frb[e] + Fr[e])
                     : 0.0;                                                    // Eq. 42
     }
-    store_row<E>(f.sVx + o, L.k0, nv, L.live, sVx); store_row<E>(f.sVy + o, L.k0, nv, L.live, sVy);
-    store_row<E>(f.sVz + o, L.k0, nv, L.live, sVz); store_row<E>(f.srho + o, L.k0, nv, L.live, srho);
-    store_row<E>(f.sW + o, L.k0, nv, L.live, sW);   store_row<E>(f.sp + o, L.k0, nv, L.live, sp);
-    store_row<E>(f.srt + o, L.k0, nv, L.live, srt);
-
-    // Eq. 31: Phi*(0) = Phi^n - Phi^[t]; (rho theta)(0) = (rho theta)^n
-    double a[E], d[E];
-    load_row<E>(f.rho_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - ((L.k0 + e < nv) ? rho[e] : 0.0);
-    store_row<E>(f.rho_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.Vx_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - V0x[e];
-    store_row<E>(f.Vx_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.Vy_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - V0y[e];
-    store_row<E>(f.Vy_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.Vz_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - V0z[e];
-    store_row<E>(f.Vz_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.W_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - W[e];
-    store_row<E>(f.W_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.p_n + o, L.k0, nv, a);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = a[e] - p0[e];
-    store_row<E>(f.p_s + o, L.k0, nv, L.live, d);
-    load_row<E>(f.rt_n + o, L.k0, nv, a);
-    store_row<E>(f.rt + o, L.k0, nv, L.live, a);
+    st_row<E>(me + F_SVX * NVP, sVx); st_row<E>(me + F_SVY * NVP, sVy); st_row<E>(me + F_SVZ * NVP, sVz);
+    st_row<E>(me + F_SRHO * NVP, srho); st_row<E>(me + F_SW * NVP, sW); st_row<E>(me + F_SP * NVP, sp);
+    st_row<E>(me + F_SRT * NVP, srt);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -498,69 +536,79 @@ k_slow_terms(Geom g, Fields f) {
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum(Geom g, Fields f, double delta) {
-    Lanes<G, E> L(g.N);
-    const int nv = g.nv;
-    const size_t o = size_t(L.col) * nv;
-    const double* wg = g.wgrad + size_t(L.col) * 18;
-    double p0[E], gx[E], gy[E], gz[E];
-    load_row<E>(f.p_s + o, L.k0, nv, p0);
+k_momentum(Geom g, double* __restrict__ S, double delta) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC;
+    double* me = S + size_t(L.col) * REC + L.k0;
+    const double2* wg = reinterpret_cast<const double2*>(g.wgrad + size_t(L.col) * 18);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    double wgv[18];
+#pragma unroll
+    for (int i = 0; i < 9; ++i) { const double2 t = __ldg(wg + i); wgv[2 * i] = t.x; wgv[2 * i + 1] = t.y; }
+    double p0[E], pj[6][E], gx[E], gy[E], gz[E];
+    ld_nc<E>(me + F_PS * NVP, p0);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) ld_nc<E>(S + size_t(nb[j]) * REC + L.k0 + F_PS * NVP, pj[j]);
+    double ri[E], vx[E], vy[E], vz[E], sx[E], sy[E], sz[E];
+    ld_nc<E>(g.rinv + L.k0, ri);
+    ld_rw<E>(me + F_VXS * NVP, vx); ld_rw<E>(me + F_VYS * NVP, vy); ld_rw<E>(me + F_VZS * NVP, vz);
+    ld_nc<E>(me + F_SVX * NVP, sx); ld_nc<E>(me + F_SVY * NVP, sy); ld_nc<E>(me + F_SVZ * NVP, sz);
 #pragma unroll
     for (int e = 0; e < E; ++e) gx[e] = gy[e] = gz[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const int c = __ldg(g.nbr + size_t(L.col) * 6 + j);
-        const double wx = __ldg(wg + 3 * j), wy = __ldg(wg + 3 * j + 1), wz = __ldg(wg + 3 * j + 2);
-        double pj[E];
-        load_row<E>(f.p_s + size_t(c) * nv, L.k0, nv, pj);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double d = pj[e] - p0[e];
-            gx[e] = fma(wx, d, gx[e]); gy[e] = fma(wy, d, gy[e]); gz[e] = fma(wz, d, gz[e]);
+            const double d = pj[j][e] - p0[e];
+            gx[e] = fma(wgv[3 * j], d, gx[e]); gy[e] = fma(wgv[3 * j + 1], d, gy[e]); gz[e] = fma(wgv[3 * j + 2], d, gz[e]);
         }
     }
-    double ri[E], v[E], s[E];
-    load_row<E>(g.rinv, L.k0, nv, ri);
-    load_row_rw<E>(f.Vx_s + o, L.k0, nv, v); load_row<E>(f.sVx + o, L.k0, nv, s);
 #pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = fma(delta, s[e] - gx[e] * ri[e], v[e]);
-    store_row<E>(f.Vx_s + o, L.k0, nv, L.live, v);
-    load_row_rw<E>(f.Vy_s + o, L.k0, nv, v); load_row<E>(f.sVy + o, L.k0, nv, s);
-#pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = fma(delta, s[e] - gy[e] * ri[e], v[e]);
-    store_row<E>(f.Vy_s + o, L.k0, nv, L.live, v);
-    load_row_rw<E>(f.Vz_s + o, L.k0, nv, v); load_row<E>(f.sVz + o, L.k0, nv, s);
-#pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = fma(delta, s[e] - gz[e] * ri[e], v[e]);
-    store_row<E>(f.Vz_s + o, L.k0, nv, L.live, v);
+    for (int e = 0; e < E; ++e) {
+        vx[e] = fma(delta, sx[e] - gx[e] * ri[e], vx[e]);
+        vy[e] = fma(delta, sy[e] - gy[e] * ri[e], vy[e]);
+        vz[e] = fma(delta, sz[e] - gz[e] * ri[e], vz[e]);
+    }
+    st_row<E>(me + F_VXS * NVP, vx); st_row<E>(me + F_VYS * NVP, vy); st_row<E>(me + F_VZS * NVP, vz);
 }
 
 // ---------------------------------------------------------------------------------------------
 // K2 (a5-a9): horizontal divergences of the new momentum, the implicit vertical momentum
 // (Eq. 37; two sweeps with the stage's LU factors), density (Eq. 32), rho*theta (Eq. 35, G7) and
 // the pressure deviation (Eq. 36).  Fig. 6 small-steps 3-6.  Gathers V*', h, theta from the 6
-// neighbours; everything else is column-local.
+// neighbours; everything else is column-local.  `first`: p*(tau) is read (first substep of a
+// stage, p* = p^n - p^[t]); otherwise it is re-evaluated from (rho theta)* exactly as the previous
+// substep stored it, which saves one row of HBM reads.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_vertical(Geom g, Fields f, double delta) {
-    Lanes<G, E> L(g.N);
-    const int nv = g.nv;
-    const size_t o = size_t(L.col) * nv;
+k_vertical(Geom g, double* __restrict__ S, double delta, int first) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC;
+    double* me = S + size_t(L.col) * REC + L.k0;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
-    const double* wd = g.wdiv + size_t(L.col) * 21;
+    const double2* wd = reinterpret_cast<const double2*>(g.wdiv + size_t(L.col) * 24);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    double wdv[24];
+#pragma unroll
+    for (int i = 0; i < 12; ++i) { const double2 t = __ldg(wd + i); wdv[2 * i] = t.x; wdv[2 * i + 1] = t.y; }
 
     double divV[E], divhV[E], divtV[E], th0[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
-        const int c = j == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 6 + j - 1);
-        const size_t oc = size_t(c) * nv;
-        const double wx = __ldg(wd + 3 * j), wy = __ldg(wd + 3 * j + 1), wz = __ldg(wd + 3 * j + 2);
+        const double* q = S + size_t(nb[j]) * REC + L.k0;
+        const double wx = wdv[3 * j], wy = wdv[3 * j + 1], wz = wdv[3 * j + 2];
         double x[E], y[E], z[E], hj[E], tj[E];
-        load_row<E>(f.Vx_s + oc, L.k0, nv, x); load_row<E>(f.Vy_s + oc, L.k0, nv, y); load_row<E>(f.Vz_s + oc, L.k0, nv, z);
-        load_row<E>(f.h + oc, L.k0, nv, hj);   load_row<E>(f.th + oc, L.k0, nv, tj);
+        ld_nc<E>(q + F_VXS * NVP, x); ld_nc<E>(q + F_VYS * NVP, y); ld_nc<E>(q + F_VZS * NVP, z);
+        ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double d = fma(wx, x[e], fma(wy, y[e], wz * z[e]));
@@ -571,12 +619,18 @@ k_vertical(Geom g, Fields f, double delta) {
         }
     }
     double ri[E], dlo[E], dhi[E];
-    load_row<E>(g.rinv, L.k0, nv, ri); load_row<E>(g.dlo, L.k0, nv, dlo); load_row<E>(g.dhi, L.k0, nv, dhi);
+    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
 
-    double rho_s[E], p_s[E], W_s[E], srho[E], sp[E], sW[E];
-    load_row_rw<E>(f.rho_s + o, L.k0, nv, rho_s); load_row_rw<E>(f.p_s + o, L.k0, nv, p_s);
-    load_row_rw<E>(f.W_s + o, L.k0, nv, W_s);
-    load_row<E>(f.srho + o, L.k0, nv, srho); load_row<E>(f.sp + o, L.k0, nv, sp); load_row<E>(f.sW + o, L.k0, nv, sW);
+    double rho_s[E], p_s[E], W_s[E], rts[E], srho[E], sp[E], sW[E], srt[E], pt[E], irt[E];
+    ld_rw<E>(me + F_RHOS * NVP, rho_s); ld_rw<E>(me + F_WS * NVP, W_s); ld_rw<E>(me + F_RTS * NVP, rts);
+    ld_nc<E>(me + F_SRHO * NVP, srho); ld_nc<E>(me + F_SP * NVP, sp); ld_nc<E>(me + F_SW * NVP, sW);
+    ld_nc<E>(me + F_SRT * NVP, srt);   ld_nc<E>(me + F_PT * NVP, pt); ld_nc<E>(me + F_IRT * NVP, irt);
+    if (first) {
+        ld_rw<E>(me + F_PS * NVP, p_s);
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) p_s[e] = eos_dev(rts[e] * irt[e], pt[e], gam, g);
+    }
     double pq[E], rq[E], pqb[E], rqb[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -586,82 +640,98 @@ k_vertical(Geom g, Fields f, double delta) {
         rq[e] = fma(delta, Srho, rho_s[e]);
     }
     below<G, E>(pq, pqb, L.gl, 0.0); below<G, E>(rq, rqb, L.gl, 0.0);
-    // right-hand side d_k on interior interfaces (0 on the ground), already scaled by 1/b'_k
+    // right-hand side d_k on interior interfaces, already scaled by 1/b'_k (fi = 0 on the ground and on pads)
     double fa[E], fi[E], fc[E], A[E], B[E], zf[E], Wn[E];
-    load_row<E>(f.fa + o, L.k0, nv, fa); load_row<E>(f.fi + o, L.k0, nv, fi); load_row<E>(f.fc + o, L.k0, nv, fc);
+    ld_nc<E>(me + F_FA * NVP, fa); ld_nc<E>(me + F_FI * NVP, fi); ld_nc<E>(me + F_FC * NVP, fc);
     const double cdz = delta / g.dz, cg = 0.5 * delta * g.gravity;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const double d = W_s[e] + delta * sW[e] - cdz * (pq[e] - pqb[e]) - cg * (rqb[e] + rq[e]);
         A[e] = -fa[e];            // z_k = d_k/b'_k - (a_k/b'_k) z_(k-1)
-        B[e] = fi[e] * d;         // fi = 0 on the ground and on masked layers
+        B[e] = fi[e] * d;
     }
     affine_scan<G, E, false>(A, B, zf, L.gl);
 #pragma unroll
     for (int e = 0; e < E; ++e) A[e] = -fc[e];                          // x_k = z_k - c'_k x_(k+1)
     affine_scan<G, E, true>(A, zf, Wn, L.gl);
 
-    double Wup[E], thb[E], X[E], Xup[E], rt[E], srt[E], p_t[E];
+    double Wup[E], thb[E], X[E], Xup[E];
     above<G, E>(Wn, Wup, L.gl, 0.0);
     below<G, E>(th0, thb, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) X[e] = 0.5 * (thb[e] + th0[e]) * Wn[e];  // I_h[theta] W'
     above<G, E>(X, Xup, L.gl, 0.0);
-    load_row_rw<E>(f.rt + o, L.k0, nv, rt); load_row<E>(f.srt + o, L.k0, nv, srt); load_row<E>(f.p_t + o, L.k0, nv, p_t);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-        rho_s[e] = rq[e] - delta * (dhi[e] * Wup[e] - dlo[e] * Wn[e]);                             // Eq. 32
-        rt[e] = rt[e] + delta * (srt[e] - divtV[e] * ri[e] - (dhi[e] * Xup[e] - dlo[e] * X[e]));  // Eq. 35
-        if (L.k0 + e >= nv) rt[e] = g.p_ref / g.Rd;
-        p_s[e] = eos_p(rt[e], g.Rd, g.p_ref, gam) - p_t[e];                                        // Eq. 36
+        rho_s[e] = rq[e] - delta * (dhi[e] * Wup[e] - dlo[e] * Wn[e]);                               // Eq. 32
+        rts[e] = rts[e] + delta * (srt[e] - divtV[e] * ri[e] - (dhi[e] * Xup[e] - dlo[e] * X[e]));  // Eq. 35
+        p_s[e] = eos_dev(rts[e] * irt[e], pt[e], gam, g);                                            // Eq. 36
     }
-    store_row<E>(f.W_s + o, L.k0, nv, L.live, Wn);   store_row<E>(f.rho_s + o, L.k0, nv, L.live, rho_s);
-    store_row<E>(f.rt + o, L.k0, nv, L.live, rt);    store_row<E>(f.p_s + o, L.k0, nv, L.live, p_s);
+    st_row<E>(me + F_WS * NVP, Wn);   st_row<E>(me + F_RHOS * NVP, rho_s);
+    st_row<E>(me + F_RTS * NVP, rts); st_row<E>(me + F_PS * NVP, p_s);
 }
 
 // ---------------------------------------------------------------------------------------------
 // End of the large step: Phi^(n+1) = Phi^[t] + Phi* (Fig. 6 large-step 4), then the PROFX forcing
 // (Eq. 51-52, backward Euler with the large step, R9).
 // ---------------------------------------------------------------------------------------------
-__global__ void k_finish(size_t n, Fields f, double dt, double Rd) {
-    size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    double rho = f.rho_t[i] + f.rho_s[i];
-    double vx = f.Vx_t[i] + f.Vx_s[i], vy = f.Vy_t[i] + f.Vy_s[i], vz = f.Vz_t[i] + f.Vz_s[i];
-    double w = f.W_t[i] + f.W_s[i];
-    double p = f.p_t[i] + f.p_s[i];
-    if (f.k_v) {
-        const double s = 1.0 + f.k_v[i] * dt;
-        vx /= s; vy /= s; vz /= s;                                           // Eq. 51
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_finish(Geom g, double* __restrict__ S, Forcing F, double dt) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
+    const size_t to = size_t(L.col) * NVP + L.k0;
+    double a[E], d[E], rho[E], p[E], vx[E], vy[E], vz[E];
+    auto sum = [&](int ft, int fs, double (&out)[E]) {
+        ld_rw<E>(me + ft * NVP, out); ld_rw<E>(me + fs * NVP, d);
+#pragma unroll
+        for (int e = 0; e < E; ++e) out[e] += d[e];
+    };
+    sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p); sum(F_VXT, F_VXS, vx); sum(F_VYT, F_VYS, vy); sum(F_VZT, F_VZS, vz);
+    sum(F_WT, F_WS, a);
+    st_row<E>(me + F_WN * NVP, a);
+    if (F.k_v) {
+        ld_nc<E>(F.k_v + to, a);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double s = 1.0 + a[e] * dt;
+            vx[e] /= s; vy[e] /= s; vz[e] /= s;                               // Eq. 51
+        }
     }
-    if (f.k_T && f.T_eq) {
-        double T = p / (rho * Rd);                                           // Eq. 25
-        T = (T + f.k_T[i] * dt * f.T_eq[i]) / (1.0 + f.k_T[i] * dt);         // Eq. 52
-        p = rho * Rd * T;
+    if (F.k_T && F.T_eq) {
+        double te[E];
+        ld_nc<E>(F.k_T + to, a); ld_nc<E>(F.T_eq + to, te);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            double T = p[e] / (rho[e] * g.Rd);                                // Eq. 25
+            T = (T + a[e] * dt * te[e]) / (1.0 + a[e] * dt);                  // Eq. 52
+            p[e] = (L.k0 + e < g.nv && L.col < g.N) ? rho[e] * g.Rd * T : p[e];
+        }
     }
-    f.rho_n[i] = rho; f.Vx_n[i] = vx; f.Vy_n[i] = vy; f.Vz_n[i] = vz; f.W_n[i] = w; f.p_n[i] = p;
+    st_row<E>(me + F_RHON * NVP, rho); st_row<E>(me + F_PN * NVP, p);
+    st_row<E>(me + F_VXN * NVP, vx);   st_row<E>(me + F_VYN * NVP, vy); st_row<E>(me + F_VZN * NVP, vz);
 }
 
 // ---------------------------------------------------------------------------------------------
-// Diagnostics (a12, R10): per-column partial sums of mass and energy; host finishes the sum.
+// Diagnostics (a12, R10): per-column partial sums of mass and energy; the host finishes the sum.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_diag(Geom g, Fields f, double* __restrict__ col_mass, double* __restrict__ col_energy) {
-    Lanes<G, E> L(g.N);
-    const int nv = g.nv;
-    const size_t o = size_t(L.col) * nv;
+k_diag(Geom g, const double* __restrict__ S, double* __restrict__ col_mass, double* __restrict__ col_energy) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    const double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
     const double Cv = g.Cp - g.Rd;
     double rho[E], Vx[E], Vy[E], Vz[E], W[E], Wup[E], p[E], vol[E], zc[E];
-    load_row_rw<E>(f.rho_n + o, L.k0, nv, rho); load_row_rw<E>(f.Vx_n + o, L.k0, nv, Vx);
-    load_row_rw<E>(f.Vy_n + o, L.k0, nv, Vy);   load_row_rw<E>(f.Vz_n + o, L.k0, nv, Vz);
-    load_row_rw<E>(f.W_n + o, L.k0, nv, W);     load_row_rw<E>(f.p_n + o, L.k0, nv, p);
-    load_row<E>(g.vol, L.k0, nv, vol);          load_row<E>(g.zc, L.k0, nv, zc);
+    ld_nc<E>(me + F_RHON * NVP, rho); ld_nc<E>(me + F_VXN * NVP, Vx); ld_nc<E>(me + F_VYN * NVP, Vy);
+    ld_nc<E>(me + F_VZN * NVP, Vz);   ld_nc<E>(me + F_WN * NVP, W);   ld_nc<E>(me + F_PN * NVP, p);
+    ld_nc<E>(g.vol + L.k0, vol);      ld_nc<E>(g.zc + L.k0, zc);
     above<G, E>(W, Wup, L.gl, 0.0);
     double m = 0.0, en = 0.0;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-        if (L.k0 + e < nv) {
+        if (L.k0 + e < g.nv) {
             const double wc = 0.5 * (W[e] + Wup[e]);
             const double ke = 0.5 * (Vx[e] * Vx[e] + Vy[e] * Vy[e] + Vz[e] * Vz[e] + wc * wc) / rho[e];
             m += rho[e] * vol[e];
@@ -673,7 +743,7 @@ k_diag(Geom g, Fields f, double* __restrict__ col_mass, double* __restrict__ col
         m += __shfl_xor_sync(kFull, m, s, G);
         en += __shfl_xor_sync(kFull, en, s, G);
     }
-    if (L.live && L.gl == 0) {
+    if (L.col < g.N && L.gl == 0) {
         const double a = __ldg(g.area + L.col);
         col_mass[L.col] = m * a;
         col_energy[L.col] = en * a;
@@ -681,9 +751,29 @@ k_diag(Geom g, Fields f, double* __restrict__ col_mass, double* __restrict__ col
 }
 
 // ---------------------------------------------------------------------------------------------
-// Canonical (host order, as uploaded) <-> device order
+// Canonical (host order, as uploaded) <-> device rows.  One thread per (device column, layer).
+//   rows:   dst[d*dst_col + k] for d < Npad, k < NVP  (a record row: dst_col = NF*NVP; a table: NVP)
+//   canon:  src[order[d]*row_len + k*cs + c0]         (real columns and layers only; pads get `pad`)
 // ---------------------------------------------------------------------------------------------
-// in: canonical [N][nv*stride_in + off...] ; generic row gather: out[d][k] = in[order[d]][k*cs + c0]
+__global__ void k_rows_from_canonical(int N, int Npad, int nv, int NVP, const int* __restrict__ order,
+                                      const double* __restrict__ src, int row_len, int cs, int c0,
+                                      double* __restrict__ dst, size_t dst_col, double pad, int zero_k0) {
+    const size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= size_t(Npad) * NVP) return;
+    const int d = int(i / NVP), k = int(i % NVP);
+    double v = pad;
+    if (d < N && k < nv) v = (zero_k0 && k == 0) ? 0.0 : src[size_t(order[d]) * row_len + size_t(k) * cs + c0];
+    dst[size_t(d) * dst_col + k] = v;
+}
+__global__ void k_rows_to_canonical(int N, int nv, int NVP, const int* __restrict__ order,
+                                    const double* __restrict__ src, size_t src_col,
+                                    int row_len, int cs, int c0, double* __restrict__ dst) {
+    const size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= size_t(N) * nv) return;
+    const int d = int(i / nv), k = int(i % nv);
+    dst[size_t(order[d]) * row_len + size_t(k) * cs + c0] = src[size_t(d) * src_col + k];
+}
+// plain [N][nv] arrays in canonical <-> device column order (config-1 host wrappers)
 __global__ void k_gather_rows(int N, int nv, const int* __restrict__ order, const double* __restrict__ in,
                               int row_len, int cs, int c0, double* __restrict__ out) {
     size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
@@ -691,17 +781,12 @@ __global__ void k_gather_rows(int N, int nv, const int* __restrict__ order, cons
     const int d = int(i / nv), k = int(i % nv);
     out[i] = in[size_t(order[d]) * row_len + size_t(k) * cs + c0];
 }
-// out: canonical; out[order[d]][k*cs + c0] = in[d][k]
 __global__ void k_scatter_rows(int N, int nv, const int* __restrict__ order, const double* __restrict__ in,
                                int row_len, int cs, int c0, double* __restrict__ out) {
     size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= size_t(N) * nv) return;
     const int d = int(i / nv), k = int(i % nv);
     out[size_t(order[d]) * row_len + size_t(k) * cs + c0] = in[i];
-}
-__global__ void k_zero_ground(int N, int nv, double* W) {
-    int d = blockIdx.x * blockDim.x + threadIdx.x;
-    if (d < N) W[size_t(d) * nv] = 0.0;
 }
 __global__ void k_fill(size_t n, double* p, double v) {
     size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x;
