@@ -7,6 +7,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -176,6 +177,21 @@ Geom make_geom(const thor_grid* grid) {
 
 int flat_blocks(size_t n) { return int((n + 255) / 256); }
 
+// L2 schedule of the two acoustic kernels; THOR_B200_TUNE="rev,k1_ahead,k2_ahead,tail"
+// overrides the defaults for measurement.
+struct TunePair { Tune k1, k2; int tma_stages, tma_ctas; };
+TunePair tune() {
+    int v[6] = {1, 0, 148, 148, 2, 3};
+    if (const char* e = std::getenv("THOR_B200_TUNE"))
+        std::sscanf(e, "%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5]);
+    TunePair p;
+    p.k1 = Tune{v[0], v[1], v[3]};
+    p.k2 = Tune{v[0], v[2], v[3]};
+    p.tma_stages = v[4];      // 0: direct-load column-solve kernel; 2 or 3: TMA-staged, that many stages
+    p.tma_ctas = v[5];        // persistent blocks per SM of the TMA-staged kernel
+    return p;
+}
+
 // one canonical host array (or a component of it) -> one row of every column record
 int put_row(thor_state* s, const double* host, size_t count, int row_len, int cs, int c0, int field, double pad,
             int zero_k0) {
@@ -217,6 +233,38 @@ int upload_table(thor_state* s, const double* host, double** dev) {
         h.N, Npad, h.nv, s->NVP, s->grid->d.order, s->stage_buf, h.nv, 1, 0, *dev, size_t(s->NVP), 0.0, 0);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+// a5-a9: TMA-staged persistent kernel where the shape has one (NVP = 32, 64), else the direct-load kernel
+template <int G, int E, int NS>
+int launch_vertical_tma(const Geom& g, double* S, double delta, int first, const TunePair& tn, cudaStream_t st) {
+    constexpr int NVP = G * E, TCOL = kTmaWarps * (32 / G);
+    const size_t smem = (size_t(NS) * TCOL * kOwnRows * NVP + TCOL * 24) * sizeof(double) + NS * sizeof(unsigned long long);
+    static bool configured = false;
+    static int n_sm = 0;
+    if (!configured) {
+        CU(cudaFuncSetAttribute(k_vertical_tma<G, E, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+        int dev = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        configured = true;
+    }
+    const int ntiles = g.Npad / TCOL;
+    const int grid = std::min(ntiles, n_sm * tn.tma_ctas);
+    k_vertical_tma<G, E, NS><<<grid, kTmaWarps * 32, smem, st>>>(g, S, delta, first, ntiles, tn.k2.rev);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return THOR_OK;
+}
+int launch_vertical(const Geom& g, double* S, double delta, int first, const TunePair& tn, cudaStream_t st) {
+    const Shape sh = shape_for(g.nv);
+    if (tn.tma_stages >= 2 && sh.E == 2 && sh.G == 16)
+        return tn.tma_stages == 2 ? launch_vertical_tma<16, 2, 2>(g, S, delta, first, tn, st)
+                                  : launch_vertical_tma<16, 2, 3>(g, S, delta, first, tn, st);
+    if (tn.tma_stages >= 2 && sh.E == 2 && sh.G == 32)
+        return tn.tma_stages == 2 ? launch_vertical_tma<32, 2, 2>(g, S, delta, first, tn, st)
+                                  : launch_vertical_tma<32, 2, 3>(g, S, delta, first, tn, st);
+    THOR_DISPATCH(k_vertical, g.nv, g.Npad, st, g, S, delta, first, tn.k2);
     return THOR_OK;
 }
 
@@ -359,6 +407,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     F.k_T = (forcing && s->has_kT) ? s->tab_kT : nullptr;
     F.k_v = (forcing && s->has_kv) ? s->tab_kv : nullptr;
     const Geom g = make_geom(s->grid);
+    const TunePair tn = tune();
     double* S = s->S;
     for (int step = 0; step < n_large; ++step) {
         for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
@@ -367,8 +416,8 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
             THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta);
             THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S);
             for (int sub = 0; sub < ns; ++sub) {
-                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta);
-                THOR_DISPATCH(k_vertical, nv, Npad, st, g, S, delta, sub == 0 ? 1 : 0);
+                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, tn.k1);
+                if (int rc = launch_vertical(g, S, delta, sub == 0 ? 1 : 0, tn, st)) return rc;
             }
         }
         THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt);
@@ -385,9 +434,11 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     const HostGrid& h = s->grid->h;
     const int Npad = s->grid->d.Npad;
     const Geom g = make_geom(s->grid);
+    const TunePair tn = tune();
     for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta);
-        if (which & 2) THOR_DISPATCH(k_vertical, h.nv, Npad, s->stream, g, s->S, delta, 0);
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, tn.k1);
+        if (which & 2)
+            if (int rc = launch_vertical(g, s->S, delta, 0, tn, s->stream)) return rc;
     }
     CU(cudaGetLastError());
     return THOR_OK;

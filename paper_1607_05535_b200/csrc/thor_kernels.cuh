@@ -68,6 +68,27 @@ struct Forcing {              // [Npad][NVP] each, may be null (Eq. 51-52)
     const double *T_eq, *k_T, *k_v;
 };
 
+// Launch-time knobs of the two acoustic kernels (defaults in thor_api.cu).
+struct Tune {
+    int rev;    // 1: the column-solve kernel walks the blocks in descending order, so that each kernel starts
+                //    on the columns the previous one has just left in L2
+    int ahead;  // blocks of look-ahead of the in-kernel bulk L2 prefetch (0 = off)
+    int tail;   // the last `tail` blocks of a kernel prefetch the rows the NEXT kernel reads first (0 = off)
+};
+
+// TMA bulk prefetch of a contiguous global range into L2 (no shared memory, no registers held)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+// rows [f0, f0 + nf) of every column of block `bid`, issued by the first warp of the calling block
+template <int G, int E>
+__device__ __forceinline__ void prefetch_block_rows(const double* S, int bid, int f0, int nf) {
+    constexpr int NVP = G * E, CPB = kWarpsPerBlock * (32 / G);
+    if (threadIdx.x < 32)
+        for (int c = threadIdx.x; c < CPB; c += 32)
+            bulk_prefetch_l2(S + (size_t(bid) * CPB + c) * (size_t(NF) * NVP) + size_t(f0) * NVP, unsigned(nf) * NVP * 8u);
+}
+
 // ---------------------------------------------------------------------------------------------
 // lane <-> (column, layers) mapping of the record kernels
 // ---------------------------------------------------------------------------------------------
@@ -78,9 +99,9 @@ struct Map {
     static constexpr int CPW = 32 / G;                 // columns per warp
     static constexpr size_t REC = size_t(NF) * NVP;    // doubles per column record
     int col, gl, k0;
-    __device__ Map() {
+    __device__ explicit Map(int bid = blockIdx.x) {
         const int lane = threadIdx.x & 31;
-        const int warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+        const int warp = bid * (blockDim.x >> 5) + (threadIdx.x >> 5);
         col = warp * CPW + lane / G;                   // < Npad by construction of the grid
         gl = lane & (G - 1);
         k0 = gl * E;
@@ -113,6 +134,15 @@ __device__ __forceinline__ double3 ld_rhat(const double* rhat, int col) {   // [
     const double2 a = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col));
     const double2 b = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col) + 1);
     return make_double3(a.x, a.y, b.x);
+}
+
+// Per-column stencil weights staged once per warp in shared memory (every lane of a column group
+// would otherwise hold the same 21-39 doubles in registers): the G lanes of a group copy `n2`
+// double2's from `src` to `dst`; the caller reads them back as broadcast LDS.
+template <int G>
+__device__ __forceinline__ void stage_weights(const double* src, double* dst, int n2, int gl) {
+    for (int i = gl; i < n2; i += G)
+        reinterpret_cast<double2*>(dst)[i] = __ldg(reinterpret_cast<const double2*>(src) + i);
 }
 
 // value at layer k-1 (fill below the ground)
@@ -400,16 +430,15 @@ k_slow_terms(Geom g, double* __restrict__ S) {
     double* me = S + size_t(L.col) * REC + L.k0;
     const int nv = g.nv;
     const double kv = g.Rd / (g.Cp - g.Rd);
-    const double2* wd = reinterpret_cast<const double2*>(g.wdiv + size_t(L.col) * 24);
-    const double2* wg = reinterpret_cast<const double2*>(g.wgrad + size_t(L.col) * 18);
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][24 + 18];
+    double* wdv = wsm[threadIdx.x / G];
+    double* wgv = wdv + 24;
+    stage_weights<G>(g.wdiv + size_t(L.col) * 24, wdv, 12, L.gl);
+    stage_weights<G>(g.wgrad + size_t(L.col) * 18, wgv, 9, L.gl);
     const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
     const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    double wdv[24], wgv[18];
-#pragma unroll
-    for (int i = 0; i < 12; ++i) { const double2 t = __ldg(wd + i); wdv[2 * i] = t.x; wdv[2 * i + 1] = t.y; }
-#pragma unroll
-    for (int i = 0; i < 9; ++i) { const double2 t = __ldg(wg + i); wgv[2 * i] = t.x; wgv[2 * i + 1] = t.y; }
+    __syncwarp();
 
     double p0[E], h0[E], th0[E], V0x[E], V0y[E], V0z[E], u0x[E], u0y[E], u0z[E];
     ld_nc<E>(me + F_PT * NVP, p0);
@@ -536,18 +565,30 @@ k_slow_terms(Geom g, double* __restrict__ S) {
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum(Geom g, double* __restrict__ S, double delta) {
+k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
     Map<G, E> L;
+    {   // L2 schedule: own look-ahead (ascending), and hand-over to the column-solve kernel
+        const int nblk = gridDim.x, b = blockIdx.x;
+        if (tn.ahead > 0 && b + tn.ahead < nblk) {
+            prefetch_block_rows<G, E>(S, b + tn.ahead, F_VXS, 3);
+            prefetch_block_rows<G, E>(S, b + tn.ahead, F_PS, 1);
+            prefetch_block_rows<G, E>(S, b + tn.ahead, F_SVX, 3);
+        }
+        if (tn.tail > 0 && b >= nblk - tn.tail) {
+            const int t = tn.rev ? b : nblk - 1 - b;      // the block of columns k_vertical reaches at the same rank
+            prefetch_block_rows<G, E>(S, t, F_H, F_IRT - F_H + 1);
+        }
+    }
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
-    const double2* wg = reinterpret_cast<const double2*>(g.wgrad + size_t(L.col) * 18);
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][18];
+    double* wgv = wsm[threadIdx.x / G];
+    stage_weights<G>(g.wgrad + size_t(L.col) * 18, wgv, 9, L.gl);
     const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
     const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    double wgv[18];
-#pragma unroll
-    for (int i = 0; i < 9; ++i) { const double2 t = __ldg(wg + i); wgv[2 * i] = t.x; wgv[2 * i + 1] = t.y; }
+    __syncwarp();
     double p0[E], pj[6][E], gx[E], gy[E], gz[E];
     ld_nc<E>(me + F_PS * NVP, p0);
 #pragma unroll
@@ -582,30 +623,38 @@ k_momentum(Geom g, double* __restrict__ S, double delta) {
 // neighbours; everything else is column-local.  `first`: p*(tau) is read (first substep of a
 // stage, p* = p^n - p^[t]); otherwise it is re-evaluated from (rho theta)* exactly as the previous
 // substep stored it, which saves one row of HBM reads.
+//
+// vertical_column is the work of one lane group on one column.  `own` points at row 0 (layer k0)
+// of the column's own rows F_VXS..F_IRT -- in global memory (k_vertical) or in the shared-memory
+// stage a TMA bulk copy has filled (k_vertical_tma); neighbours are always gathered from global
+// memory (L1/L2 hits).  wdv: the column's 21 divergence weights in shared memory.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_vertical(Geom g, double* __restrict__ S, double delta, int first) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t REC = Map<G, E>::REC;
-    double* me = S + size_t(L.col) * REC + L.k0;
+__device__ __forceinline__ void vertical_column(const Geom& g, double* __restrict__ S, const double* own, const double* wdv,
+                                                int col, int gl, int k0, double delta, int first) {
+    constexpr int NVP = G * E;
+    constexpr size_t REC = size_t(NF) * NVP;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
-    const double2* wd = reinterpret_cast<const double2*>(g.wdiv + size_t(L.col) * 24);
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    double wdv[24];
-#pragma unroll
-    for (int i = 0; i < 12; ++i) { const double2 t = __ldg(wd + i); wdv[2 * i] = t.x; wdv[2 * i + 1] = t.y; }
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
 
     double divV[E], divhV[E], divtV[E], th0[E];
+    {
+        double x[E], y[E], z[E], hj[E];
+        ld_rw<E>(own + F_VXS * NVP, x); ld_rw<E>(own + F_VYS * NVP, y); ld_rw<E>(own + F_VZS * NVP, z);
+        ld_rw<E>(own + F_H * NVP, hj);  ld_rw<E>(own + F_TH * NVP, th0);
+        const double wx = wdv[0], wy = wdv[1], wz = wdv[2];
 #pragma unroll
-    for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = 0.0;
+        for (int e = 0; e < E; ++e) {
+            const double d = fma(wx, x[e], fma(wy, y[e], wz * z[e]));
+            divV[e] = d; divhV[e] = hj[e] * d; divtV[e] = th0[e] * d;
+        }
+    }
 #pragma unroll
-    for (int j = 0; j < 7; ++j) {
-        const double* q = S + size_t(nb[j]) * REC + L.k0;
-        const double wx = wdv[3 * j], wy = wdv[3 * j + 1], wz = wdv[3 * j + 2];
+    for (int j = 0; j < 6; ++j) {
+        const double* q = S + size_t(nb[j]) * REC + k0;
+        const double wx = wdv[3 * j + 3], wy = wdv[3 * j + 4], wz = wdv[3 * j + 5];
         double x[E], y[E], z[E], hj[E], tj[E];
         ld_nc<E>(q + F_VXS * NVP, x); ld_nc<E>(q + F_VYS * NVP, y); ld_nc<E>(q + F_VZS * NVP, z);
         ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
@@ -615,18 +664,17 @@ k_vertical(Geom g, double* __restrict__ S, double delta, int first) {
             divV[e] += d;
             divhV[e] = fma(hj[e], d, divhV[e]);
             divtV[e] = fma(tj[e], d, divtV[e]);
-            if (j == 0) th0[e] = tj[e];
         }
     }
     double ri[E], dlo[E], dhi[E];
-    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
+    ld_nc<E>(g.rinv + k0, ri); ld_nc<E>(g.dlo + k0, dlo); ld_nc<E>(g.dhi + k0, dhi);
 
     double rho_s[E], p_s[E], W_s[E], rts[E], srho[E], sp[E], sW[E], srt[E], pt[E], irt[E];
-    ld_rw<E>(me + F_RHOS * NVP, rho_s); ld_rw<E>(me + F_WS * NVP, W_s); ld_rw<E>(me + F_RTS * NVP, rts);
-    ld_nc<E>(me + F_SRHO * NVP, srho); ld_nc<E>(me + F_SP * NVP, sp); ld_nc<E>(me + F_SW * NVP, sW);
-    ld_nc<E>(me + F_SRT * NVP, srt);   ld_nc<E>(me + F_PT * NVP, pt); ld_nc<E>(me + F_IRT * NVP, irt);
+    ld_rw<E>(own + F_RHOS * NVP, rho_s); ld_rw<E>(own + F_WS * NVP, W_s); ld_rw<E>(own + F_RTS * NVP, rts);
+    ld_rw<E>(own + F_SRHO * NVP, srho);  ld_rw<E>(own + F_SP * NVP, sp);  ld_rw<E>(own + F_SW * NVP, sW);
+    ld_rw<E>(own + F_SRT * NVP, srt);    ld_rw<E>(own + F_PT * NVP, pt);  ld_rw<E>(own + F_IRT * NVP, irt);
     if (first) {
-        ld_rw<E>(me + F_PS * NVP, p_s);
+        ld_rw<E>(own + F_PS * NVP, p_s);
     } else {
 #pragma unroll
         for (int e = 0; e < E; ++e) p_s[e] = eos_dev(rts[e] * irt[e], pt[e], gam, g);
@@ -639,10 +687,10 @@ k_vertical(Geom g, double* __restrict__ S, double delta, int first) {
         pq[e] = fma(delta, Sp, p_s[e]);
         rq[e] = fma(delta, Srho, rho_s[e]);
     }
-    below<G, E>(pq, pqb, L.gl, 0.0); below<G, E>(rq, rqb, L.gl, 0.0);
+    below<G, E>(pq, pqb, gl, 0.0); below<G, E>(rq, rqb, gl, 0.0);
     // right-hand side d_k on interior interfaces, already scaled by 1/b'_k (fi = 0 on the ground and on pads)
     double fa[E], fi[E], fc[E], A[E], B[E], zf[E], Wn[E];
-    ld_nc<E>(me + F_FA * NVP, fa); ld_nc<E>(me + F_FI * NVP, fi); ld_nc<E>(me + F_FC * NVP, fc);
+    ld_rw<E>(own + F_FA * NVP, fa); ld_rw<E>(own + F_FI * NVP, fi); ld_rw<E>(own + F_FC * NVP, fc);
     const double cdz = delta / g.dz, cg = 0.5 * delta * g.gravity;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -650,25 +698,132 @@ k_vertical(Geom g, double* __restrict__ S, double delta, int first) {
         A[e] = -fa[e];            // z_k = d_k/b'_k - (a_k/b'_k) z_(k-1)
         B[e] = fi[e] * d;
     }
-    affine_scan<G, E, false>(A, B, zf, L.gl);
+    affine_scan<G, E, false>(A, B, zf, gl);
 #pragma unroll
     for (int e = 0; e < E; ++e) A[e] = -fc[e];                          // x_k = z_k - c'_k x_(k+1)
-    affine_scan<G, E, true>(A, zf, Wn, L.gl);
+    affine_scan<G, E, true>(A, zf, Wn, gl);
 
     double Wup[E], thb[E], X[E], Xup[E];
-    above<G, E>(Wn, Wup, L.gl, 0.0);
-    below<G, E>(th0, thb, L.gl, 0.0);
+    above<G, E>(Wn, Wup, gl, 0.0);
+    below<G, E>(th0, thb, gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) X[e] = 0.5 * (thb[e] + th0[e]) * Wn[e];  // I_h[theta] W'
-    above<G, E>(X, Xup, L.gl, 0.0);
+    above<G, E>(X, Xup, gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         rho_s[e] = rq[e] - delta * (dhi[e] * Wup[e] - dlo[e] * Wn[e]);                               // Eq. 32
         rts[e] = rts[e] + delta * (srt[e] - divtV[e] * ri[e] - (dhi[e] * Xup[e] - dlo[e] * X[e]));  // Eq. 35
         p_s[e] = eos_dev(rts[e] * irt[e], pt[e], gam, g);                                            // Eq. 36
     }
+    double* me = S + size_t(col) * REC + k0;
     st_row<E>(me + F_WS * NVP, Wn);   st_row<E>(me + F_RHOS * NVP, rho_s);
     st_row<E>(me + F_RTS * NVP, rts); st_row<E>(me + F_PS * NVP, p_s);
+}
+
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
+    const int nblk = gridDim.x;
+    const int bid = tn.rev ? nblk - 1 - int(blockIdx.x) : int(blockIdx.x);
+    Map<G, E> L(bid);
+    {   // L2 schedule: own look-ahead in walking order, and hand-over to the next momentum kernel
+        const int b = blockIdx.x;
+        if (tn.ahead > 0 && b + tn.ahead < nblk)
+            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - (b + tn.ahead) : b + tn.ahead, F_VXS, F_IRT + 1);
+        if (tn.tail > 0 && b >= nblk - tn.tail)
+            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - b : b - (nblk - tn.tail), F_SVX, 3);
+    }
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][24];
+    double* wdv = wsm[threadIdx.x / G];
+    stage_weights<G>(g.wdiv + size_t(L.col) * 24, wdv, 12, L.gl);
+    __syncwarp();
+    vertical_column<G, E>(g, S, S + size_t(L.col) * Map<G, E>::REC + L.k0, wdv, L.col, L.gl, L.k0, delta, first);
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2, TMA-staged: persistent blocks of kTmaWarps warps walk tiles of TCOL = kTmaWarps*32/G columns.
+// The own rows F_VXS..F_IRT of a tile (the contiguous head of each column record) are brought into
+// shared memory by cp.async.bulk (TMA) NSTAGE tiles ahead of their use and signalled through
+// mbarriers, so HBM requests are in flight without holding registers or stalling warps; only the
+// neighbour gathers (L1/L2 hits) are ordinary loads.
+// ---------------------------------------------------------------------------------------------
+constexpr int kTmaWarps = 4;
+constexpr int kOwnRows = F_IRT + 1;     // 17
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int G, int E, int NSTAGE>
+__global__ void __launch_bounds__(kTmaWarps * 32)
+k_vertical_tma(Geom g, double* __restrict__ S, double delta, int first, int ntiles, int rev) {
+    constexpr int NVP = G * E, CPW = 32 / G, TCOL = kTmaWarps * CPW;
+    constexpr size_t REC = size_t(NF) * NVP;
+    constexpr int STAGE_DOUBLES = TCOL * kOwnRows * NVP;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* stage = reinterpret_cast<double*>(smem_raw);                       // [NSTAGE][TCOL][17][NVP]
+    double* wsm = stage + size_t(NSTAGE) * STAGE_DOUBLES;                       // [TCOL][24]
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(wsm + TCOL * 24);   // [NSTAGE]
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int slot = warp * CPW + lane / G;       // column of the tile this lane group owns
+    const int gl = lane & (G - 1), k0 = gl * E;
+    // tile i of this block = tile blockIdx.x + i*gridDim.x in walking order
+    const int my_tiles = (ntiles - int(blockIdx.x) + int(gridDim.x) - 1) / int(gridDim.x);
+    auto tile_of = [&](int i) { const int t = int(blockIdx.x) + i * int(gridDim.x); return rev ? ntiles - 1 - t : t; };
+    // producer: the first warp; lane 0 arms the barrier, lane c copies column c of the tile
+    auto issue = [&](int i) {
+        if (warp != 0) return;
+        const int s = i % NSTAGE;
+        const unsigned row = NVP * 8u;
+        const unsigned bytes = TCOL * (first ? kOwnRows : kOwnRows - 1) * row;
+        if (lane == 0) mbar_expect_tx(full + s, bytes);
+        __syncwarp();
+        for (int c = lane; c < TCOL; c += 32) {
+            const double* src = S + (size_t(tile_of(i)) * TCOL + c) * REC;
+            double* dst = stage + size_t(s) * STAGE_DOUBLES + size_t(c) * kOwnRows * NVP;
+            if (first) {
+                bulk_g2s(dst, src, kOwnRows * row, full + s);
+            } else {                                     // skip the p* row: it is re-evaluated from (rho theta)*
+                bulk_g2s(dst, src, F_PS * row, full + s);
+                bulk_g2s(dst + (F_PS + 1) * NVP, src + (F_PS + 1) * NVP, (kOwnRows - F_PS - 1) * row, full + s);
+            }
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(full + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    for (int i = 0; i < NSTAGE && i < my_tiles; ++i) issue(i);
+
+    for (int i = 0; i < my_tiles; ++i) {
+        const int s = i % NSTAGE;
+        const int col = tile_of(i) * TCOL + slot;
+        double* wdv = wsm + slot * 24;
+        stage_weights<G>(g.wdiv + size_t(col) * 24, wdv, 12, gl);
+        __syncwarp();
+        mbar_wait(full + s, (i / NSTAGE) & 1);
+        vertical_column<G, E>(g, S, stage + size_t(s) * STAGE_DOUBLES + size_t(slot) * kOwnRows * NVP + k0, wdv,
+                              col, gl, k0, delta, first);
+        __syncthreads();                                  // every warp has read stage s (and its weights)
+        if (i + NSTAGE < my_tiles) issue(i + NSTAGE);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
