@@ -47,11 +47,17 @@ inline double norm(V3 a) { return std::sqrt(dot(a, a)); }
 inline V3 unit(V3 a) { return (1.0 / norm(a)) * a; }
 inline double arc(V3 a, V3 b) { return std::atan2(norm(cross(a, b)), dot(a, b)); }
 
+// A triangle and, for the device column order, the position of its corners on the lattice of the
+// rhombus it belongs to: the 20 faces pair into 10 rhombi (L45 "ten rhombuses"), each an n x n
+// lattice (n = 2^level) with corners (0,0), (n,0), (0,n), (n,n) and the shared face edge on the
+// short diagonal (n,0)-(0,n).
 struct Tri {
     int a, b, c;
+    int r = 0;                       // rhombus 0..9
+    int ia = 0, ja = 0, ib = 0, jb = 0, ic = 0, jc = 0;
 };
 
-void icosahedron(std::vector<V3>& pts, std::vector<Tri>& tris) {
+void icosahedron(std::vector<V3>& pts, std::vector<Tri>& tris, int n) {
     const double lat = std::atan(0.5);
     pts.clear();
     tris.clear();
@@ -68,10 +74,10 @@ void icosahedron(std::vector<V3>& pts, std::vector<Tri>& tris) {
     // five north-to-south strips of four faces; counter-clockwise seen from outside
     for (int j = 0; j < 5; ++j) {
         int u0 = 1 + j, u1 = 1 + (j + 1) % 5, l0 = 6 + j, l1 = 6 + (j + 1) % 5;
-        tris.push_back({0, u0, u1});
-        tris.push_back({u0, l0, u1});
-        tris.push_back({u1, l0, l1});
-        tris.push_back({11, l1, l0});
+        tris.push_back({0, u0, u1, 2 * j, 0, 0, n, 0, 0, n});
+        tris.push_back({u0, l0, u1, 2 * j, n, 0, n, n, 0, n});
+        tris.push_back({u1, l0, l1, 2 * j + 1, 0, 0, n, 0, 0, n});
+        tris.push_back({11, l1, l0, 2 * j + 1, n, n, 0, n, n, 0});
     }
 }
 
@@ -93,10 +99,12 @@ void bisect(std::vector<V3>& pts, std::vector<Tri>& tris) {
     out.reserve(tris.size() * 4);
     for (const Tri& t : tris) {
         int ab = midpoint(t.a, t.b), bc = midpoint(t.b, t.c), ca = midpoint(t.c, t.a);
-        out.push_back({t.a, ab, ca});
-        out.push_back({ab, bc, ca});   // centre child second: keeps consecutive children adjacent
-        out.push_back({ab, t.b, bc});
-        out.push_back({ca, bc, t.c});
+        const int iab = (t.ia + t.ib) / 2, jab = (t.ja + t.jb) / 2, ibc = (t.ib + t.ic) / 2, jbc = (t.jb + t.jc) / 2;
+        const int ica = (t.ic + t.ia) / 2, jca = (t.jc + t.ja) / 2;
+        out.push_back({t.a, ab, ca, t.r, t.ia, t.ja, iab, jab, ica, jca});
+        out.push_back({ab, bc, ca, t.r, iab, jab, ibc, jbc, ica, jca});
+        out.push_back({ab, t.b, bc, t.r, iab, jab, t.ib, t.jb, ibc, jbc});
+        out.push_back({ca, bc, t.c, t.r, ica, jca, ibc, jbc, t.ic, t.jc});
     }
     tris.swap(out);
 }
@@ -203,7 +211,7 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
     std::vector<V3> pts;
     std::vector<Tri> tris;
     std::vector<int> nbr, deg;
-    icosahedron(pts, tris);
+    icosahedron(pts, tris, 1 << level);
     g.spring_iterations = 0;
     for (int l = 1; l <= level; ++l) {
         bisect(pts, tris);
@@ -271,16 +279,37 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
         return bary[size_t(t) * 3 + 2];
     };
 
-    // --- device column order: first touch in quadtree order of the leaf triangles
+    // --- device column order.  Every rhombus owns the lattice points 0 <= I < n, 0 < J <= n (the ten
+    // half-open rhombi tile the sphere; the two poles are left over), and its columns are laid out
+    // along the Morton (Z-order) curve of (I, J-1): every aligned run of 4 / 8 / 16 columns is a
+    // 2x2 / 2x4 / 4x4 lattice patch, so the tiles the kernels stage in shared memory have the
+    // smallest possible halo (10 / 14 / 18 columns) and neighbours sit close in memory.
     g.order.assign(N, -1);
     g.rank.assign(N, -1);
     {
-        int next = 0;
-        auto touch = [&](int v) {
-            if (g.rank[v] < 0) { g.rank[v] = next; g.order[next] = v; ++next; }
+        const long long n = 1LL << level;
+        auto morton = [](unsigned x, unsigned y) {
+            unsigned long long m = 0;
+            for (int b = 0; b < 16; ++b) m |= ((unsigned long long)((x >> b) & 1u) << (2 * b + 1)) | ((unsigned long long)((y >> b) & 1u) << (2 * b));
+            return m;
         };
-        for (const Tri& t : tris) { touch(t.a); touch(t.b); touch(t.c); }
-        if (next != N) return THOR_EINVAL;
+        std::vector<long long> key(N, -1);
+        auto claim = [&](int v, int r, int I, int J) {
+            if (I >= 0 && I < n && J > 0 && J <= n) key[v] = (long long)r * n * n + (long long)morton(unsigned(I), unsigned(J - 1));
+        };
+        for (const Tri& t : tris) { claim(t.a, t.r, t.ia, t.ja); claim(t.b, t.r, t.ib, t.jb); claim(t.c, t.r, t.ic, t.jc); }
+        int poles = 0;
+        for (int v = 0; v < N; ++v)
+            if (key[v] < 0) key[v] = 10 * n * n + poles++;
+        if (poles != 2) return THOR_EINVAL;
+        std::vector<int> idx(N);
+        for (int v = 0; v < N; ++v) idx[v] = v;
+        std::sort(idx.begin(), idx.end(), [&](int x, int y) { return key[x] < key[y]; });
+        for (int d = 0; d < N; ++d) {
+            if (d > 0 && key[idx[d]] == key[idx[d - 1]]) return THOR_EINVAL;    // every column has one owner
+            g.order[d] = idx[d];
+            g.rank[idx[d]] = d;
+        }
     }
 
     // --- l_k, n_k, A_c (Eq. 4, 6) and the expanded stencil weights
@@ -341,6 +370,33 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
         g.d_rhat[size_t(d) * 3 + 1] = p0.y;
         g.d_rhat[size_t(d) * 3 + 2] = p0.z;
         g.d_area[d] = area;
+    }
+
+    // --- tangent basis per column and the stencils contracted with it.  e1 = z x r (x x r next to the
+    // poles), e2 = r x e1: no smoothness is needed, the weights absorb the basis of every neighbour.
+    g.d_basis.assign(size_t(N) * 6, 0.0);
+    g.d_wdiv2.assign(size_t(N) * 14, 0.0);
+    g.d_wgrad2.assign(size_t(N) * 12, 0.0);
+    for (int d = 0; d < N; ++d) {
+        const V3 r{g.d_rhat[size_t(d) * 3], g.d_rhat[size_t(d) * 3 + 1], g.d_rhat[size_t(d) * 3 + 2]};
+        const V3 axis = std::fabs(r.z) < 0.9 ? V3{0, 0, 1} : V3{1, 0, 0};
+        const V3 e1 = unit(cross(axis, r)), e2 = cross(r, e1);
+        double* b = &g.d_basis[size_t(d) * 6];
+        b[0] = e1.x; b[1] = e1.y; b[2] = e1.z; b[3] = e2.x; b[4] = e2.y; b[5] = e2.z;
+    }
+    for (int d = 0; d < N; ++d) {
+        auto vec = [](const double* p) { return V3{p[0], p[1], p[2]}; };
+        for (int j = 0; j < 7; ++j) {
+            const int c = j == 0 ? d : g.d_nbr[size_t(d) * 6 + j - 1];
+            const V3 w = vec(&g.d_wdiv[size_t(d) * 21 + 3 * j]);
+            g.d_wdiv2[size_t(d) * 14 + 2 * j] = dot(w, vec(&g.d_basis[size_t(c) * 6]));
+            g.d_wdiv2[size_t(d) * 14 + 2 * j + 1] = dot(w, vec(&g.d_basis[size_t(c) * 6 + 3]));
+        }
+        for (int j = 0; j < 6; ++j) {
+            const V3 w = vec(&g.d_wgrad[size_t(d) * 18 + 3 * j]);
+            g.d_wgrad2[size_t(d) * 12 + 2 * j] = dot(w, vec(&g.d_basis[size_t(d) * 6]));
+            g.d_wgrad2[size_t(d) * 12 + 2 * j + 1] = dot(w, vec(&g.d_basis[size_t(d) * 6 + 3]));
+        }
     }
 
     // --- vertical tables (R6: uniform dz; Eq. 27's radial operator)

@@ -44,7 +44,12 @@ struct DeviceGeom {
     int* nbr = nullptr;
     int* order = nullptr;
     double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
+    double *basis = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr;
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr;
+    // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
+    int tcol = 0, hmax = 0;
+    int* tile_halo = nullptr;
+    unsigned char* tile_slots = nullptr;
 };
 
 // lane-group width G and layers per lane E of the record kernels; NVP = G*E padded layers
@@ -100,10 +105,13 @@ int ensure_device_geom(const thor_grid* grid) {
     d.Npad = Npad;
     std::vector<int> nbr(size_t(Npad) * 8);
     std::vector<double> wdiv(size_t(Npad) * 24, 0.0), wgrad(size_t(Npad) * 18, 0.0), rhat(size_t(Npad) * 4, 0.0),
-        area(Npad, 0.0);
+        area(Npad, 0.0), basis(size_t(Npad) * 8, 0.0), wdiv2(size_t(Npad) * 16, 0.0), wgrad2(size_t(Npad) * 12, 0.0);
     for (int c = 0; c < Npad; ++c) {
         for (int k = 0; k < 8; ++k) nbr[size_t(c) * 8 + k] = (c < N && k < 6) ? h.d_nbr[size_t(c) * 6 + k] : c;
-        if (c >= N) { rhat[size_t(c) * 4 + 2] = 1.0; continue; }
+        if (c >= N) { rhat[size_t(c) * 4 + 2] = 1.0; basis[size_t(c) * 8] = 1.0; basis[size_t(c) * 8 + 4] = 1.0; continue; }
+        std::copy_n(&h.d_basis[size_t(c) * 6], 6, &basis[size_t(c) * 8]);
+        std::copy_n(&h.d_wdiv2[size_t(c) * 14], 14, &wdiv2[size_t(c) * 16]);
+        std::copy_n(&h.d_wgrad2[size_t(c) * 12], 12, &wgrad2[size_t(c) * 12]);
         std::copy_n(&h.d_wdiv[size_t(c) * 21], 21, &wdiv[size_t(c) * 24]);
         std::copy_n(&h.d_wgrad[size_t(c) * 18], 18, &wgrad[size_t(c) * 18]);
         std::copy_n(&h.d_rhat[size_t(c) * 3], 3, &rhat[size_t(c) * 4]);
@@ -121,11 +129,45 @@ int ensure_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.wgrad, wgrad))) return rc;
     if ((rc = upload(&d.rhat, rhat))) return rc;
     if ((rc = upload(&d.area, area))) return rc;
+    if ((rc = upload(&d.basis, basis))) return rc;
+    if ((rc = upload(&d.wdiv2, wdiv2))) return rc;
+    if ((rc = upload(&d.wgrad2, wgrad2))) return rc;
     if ((rc = upload(&d.rinv, padded(h.rinv)))) return rc;
     if ((rc = upload(&d.dlo, padded(h.dlo)))) return rc;
     if ((rc = upload(&d.dhi, padded(h.dhi)))) return rc;
     if ((rc = upload(&d.vol, padded(h.vol)))) return rc;
     if ((rc = upload(&d.zc, padded(h.zc)))) return rc;
+    {   // tile tables: halo columns of every tile and, per column, the slot of each neighbour
+        const Shape sh = shape_for(h.nv);
+        const int TC = kTmaWarps * (32 / sh.G), ntiles = Npad / TC;
+        std::vector<std::vector<int>> halo(ntiles);
+        std::vector<unsigned char> slots(size_t(Npad) * 8, 0);
+        int hmax = 0;
+        for (int t = 0; t < ntiles; ++t) {
+            std::vector<int>& hl = halo[t];
+            for (int c = t * TC; c < (t + 1) * TC; ++c)
+                for (int k = 0; k < 8; ++k) {
+                    const int nb = nbr[size_t(c) * 8 + k];
+                    int slot;
+                    if (nb / TC == t) slot = nb - t * TC;
+                    else {
+                        auto it = std::find(hl.begin(), hl.end(), nb);
+                        if (it == hl.end()) { hl.push_back(nb); it = hl.end() - 1; }
+                        slot = TC + int(it - hl.begin());
+                    }
+                    slots[size_t(c) * 8 + k] = static_cast<unsigned char>(slot);
+                }
+            hmax = std::max(hmax, int(hl.size()));
+        }
+        hmax = std::max(hmax, 1);
+        std::vector<int> flat(size_t(ntiles) * hmax);
+        for (int t = 0; t < ntiles; ++t)
+            for (int i = 0; i < hmax; ++i) flat[size_t(t) * hmax + i] = i < int(halo[t].size()) ? halo[t][i] : t * TC;
+        d.tcol = TC; d.hmax = hmax;
+        if (TC + hmax > 255) d.hmax = 0;                 // slots are bytes; such a grid uses the direct kernel
+        if ((rc = upload(&d.tile_halo, flat))) return rc;
+        if ((rc = upload(&d.tile_slots, slots))) return rc;
+    }
     d.ready = true;
     return THOR_OK;
 }
@@ -136,6 +178,7 @@ Geom make_geom(const thor_grid* grid) {
     Geom g;
     g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
     g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
+    g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc;
     g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
@@ -181,13 +224,13 @@ int flat_blocks(size_t n) { return int((n + 255) / 256); }
 // overrides the defaults for measurement.
 struct TunePair { Tune k1, k2; int tma_stages, tma_ctas; };
 TunePair tune() {
-    int v[6] = {1, 0, 148, 148, 2, 3};
+    int v[6] = {1, 0, 148, 148, 0, 4};
     if (const char* e = std::getenv("THOR_B200_TUNE"))
         std::sscanf(e, "%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5]);
     TunePair p;
     p.k1 = Tune{v[0], v[1], v[3]};
     p.k2 = Tune{v[0], v[2], v[3]};
-    p.tma_stages = v[4];      // 0: direct-load column-solve kernel; 2 or 3: TMA-staged, that many stages
+    p.tma_stages = v[4];      // 0: direct-load column-solve kernel; 1 or 2: TMA-staged, that many stages per block
     p.tma_ctas = v[5];        // persistent blocks per SM of the TMA-staged kernel
     return p;
 }
@@ -236,34 +279,47 @@ int upload_table(thor_state* s, const double* host, double** dev) {
     return THOR_OK;
 }
 
-// a5-a9: TMA-staged persistent kernel where the shape has one (NVP = 32, 64), else the direct-load kernel
-template <int G, int E, int NS>
-int launch_vertical_tma(const Geom& g, double* S, double delta, int first, const TunePair& tn, cudaStream_t st) {
-    constexpr int NVP = G * E, TCOL = kTmaWarps * (32 / G);
-    const size_t smem = (size_t(NS) * TCOL * kOwnRows * NVP + TCOL * 24) * sizeof(double) + NS * sizeof(unsigned long long);
-    static bool configured = false;
+// a5-a9: TMA-staged persistent kernel where a whole stage fits in shared memory, else the direct-load kernel
+constexpr size_t kSmemPerBlockMax = 227 * 1024;
+template <int G, int NS>
+int launch_vertical_staged(const Geom& g, const DeviceGeom& d, double* S, double delta, int first, const TunePair& tn,
+                           cudaStream_t st, bool* done) {
+    constexpr int E = 2, NVP = G * E, TCOL = kTmaWarps * (32 / G);
+    const size_t stage_doubles = size_t(TCOL) * kOwnRows * NVP + size_t(d.hmax) * kHaloRows * NVP + TCOL * 16 + TCOL;
+    const size_t smem = NS * stage_doubles * sizeof(double) + NS * sizeof(unsigned long long);
+    *done = false;
+    if (d.hmax <= 0 || d.tcol != TCOL || smem > kSmemPerBlockMax) return THOR_OK;
+    static size_t configured = 0;
     static int n_sm = 0;
-    if (!configured) {
-        CU(cudaFuncSetAttribute(k_vertical_tma<G, E, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+    if (configured < smem) {
+        CU(cudaFuncSetAttribute(k_vertical_staged<G, E, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
         int dev = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-        configured = true;
+        configured = smem;
     }
     const int ntiles = g.Npad / TCOL;
-    const int grid = std::min(ntiles, n_sm * tn.tma_ctas);
-    k_vertical_tma<G, E, NS><<<grid, kTmaWarps * 32, smem, st>>>(g, S, delta, first, ntiles, tn.k2.rev);
+    const int grid = std::min(ntiles, n_sm * std::max(1, tn.tma_ctas));
+    TileTab tt{d.tile_halo, d.tile_slots, d.hmax};
+    k_vertical_staged<G, E, NS><<<grid, kTmaWarps * 32, smem, st>>>(g, tt, S, delta, first, ntiles, tn.k2.rev);
     g_launches.fetch_add(1, std::memory_order_relaxed);
+    *done = true;
     return THOR_OK;
 }
-int launch_vertical(const Geom& g, double* S, double delta, int first, const TunePair& tn, cudaStream_t st) {
+int launch_vertical(const thor_grid* grid, const Geom& g, double* S, double delta, int first, const TunePair& tn,
+                    cudaStream_t st) {
     const Shape sh = shape_for(g.nv);
-    if (tn.tma_stages >= 2 && sh.E == 2 && sh.G == 16)
-        return tn.tma_stages == 2 ? launch_vertical_tma<16, 2, 2>(g, S, delta, first, tn, st)
-                                  : launch_vertical_tma<16, 2, 3>(g, S, delta, first, tn, st);
-    if (tn.tma_stages >= 2 && sh.E == 2 && sh.G == 32)
-        return tn.tma_stages == 2 ? launch_vertical_tma<32, 2, 2>(g, S, delta, first, tn, st)
-                                  : launch_vertical_tma<32, 2, 3>(g, S, delta, first, tn, st);
+    const DeviceGeom& d = grid->d;
+    bool done = false;
+    int rc = THOR_OK;
+    if (tn.tma_stages >= 1 && sh.E == 2) {
+        const bool two = tn.tma_stages >= 2;
+        if (sh.G == 4) rc = two ? launch_vertical_staged<4, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<4, 1>(g, d, S, delta, first, tn, st, &done);
+        else if (sh.G == 8) rc = two ? launch_vertical_staged<8, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<8, 1>(g, d, S, delta, first, tn, st, &done);
+        else if (sh.G == 16) rc = two ? launch_vertical_staged<16, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<16, 1>(g, d, S, delta, first, tn, st, &done);
+        else rc = two ? launch_vertical_staged<32, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<32, 1>(g, d, S, delta, first, tn, st, &done);
+        if (rc || done) return rc;
+    }
     THOR_DISPATCH(k_vertical, g.nv, g.Npad, st, g, S, delta, first, tn.k2);
     return THOR_OK;
 }
@@ -311,6 +367,7 @@ void thor_grid_destroy(thor_grid* grid) {
     if (d.ready) {
         cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
         cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc);
+        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2);
     }
     delete grid;
 }
@@ -417,7 +474,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
             THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S);
             for (int sub = 0; sub < ns; ++sub) {
                 THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, tn.k1);
-                if (int rc = launch_vertical(g, S, delta, sub == 0 ? 1 : 0, tn, st)) return rc;
+                if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, tn, st)) return rc;
             }
         }
         THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt);
@@ -438,7 +495,7 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     for (int i = 0; i < n_substeps; ++i) {
         if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, tn.k1);
         if (which & 2)
-            if (int rc = launch_vertical(g, s->S, delta, 0, tn, s->stream)) return rc;
+            if (int rc = launch_vertical(s->grid, g, s->S, delta, 0, tn, s->stream)) return rc;
     }
     CU(cudaGetLastError());
     return THOR_OK;

@@ -10,7 +10,7 @@
 // a neighbour column's row is one contiguous 8*NVP-byte segment, every field of a column sits at a
 // compile-time offset from one base address, and vertical neighbours are in the same lane or one
 // shuffle away.  The rows a kernel reads together are adjacent in the record (the acoustic
-// column-solve kernel reads rows 0..16 of its own column: one contiguous 17*NVP*8-byte block).
+// column-solve kernel reads rows 0..15 of its own column: one contiguous 16*NVP*8-byte block).
 //
 // W (= rho v_r) is stored on the LOWER interface of each layer (slot 0 = ground = 0; the lid above
 // the top layer is an implicit 0).  Pad layers (k >= n_layers) and pad columns hold exact zeros in
@@ -24,7 +24,7 @@
 namespace thor {
 
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kWarpsPerBlock = 8;
+constexpr int kWarpsPerBlock = 4;
 constexpr int kColPad = 64;      // columns are padded to a multiple of this (>= columns per block of any shape)
 constexpr int kEosTerms = 11;    // degree of the binomial series of Eq. 36 in deviation form
 constexpr double kEosSmall = 0.03125;   // |x| <= 2^-5: series; beyond: expm1/log1p
@@ -32,16 +32,16 @@ constexpr double kEosSmall = 0.03125;   // |x| <= 2^-5: series; beyond: expm1/lo
 // rows of a column record
 enum Field : int {
     // --- acoustic substep, gathered from the 6 neighbours by the column-solve kernel
-    F_VXS = 0, F_VYS, F_VZS,     // V* = (rho v_h)*, Cartesian                     (Eq. 31, 33)
-    F_H, F_TH,                   // h = Cp T, theta of the stage reference state   (Eq. 38)
+    F_VAS = 0, F_VBS,            // V* = (rho v_h)* = a e1 + b e2 in the column's tangent basis  (Eq. 31, 33)
+    F_H, F_TH,                   // h = Cp T, theta of the stage reference state                (Eq. 38)
     // --- acoustic substep, column-local
     F_PS,                        // p*        (gathered by the momentum kernel)
     F_RHOS, F_WS, F_RTS,         // rho*, W* = (rho v_r)*, (rho theta)*
     F_SRHO, F_SP, F_SW, F_SRT,   // slow terms of Eq. 32, 40, 42, 35
     F_FA, F_FI, F_FC,            // LU factors of the tridiagonal matrix of Eq. 37
-    F_PT, F_IRT,                 // p^[t], 1/(rho theta)^[t]
-    F_SVX, F_SVY, F_SVZ,         // slow term of Eq. 33
-    // --- stage reference state Phi^[t] (R1) and the un-projected velocity (L268)
+    F_PT,                        // p^[t]
+    F_SVA, F_SVB,                // slow term of Eq. 33, tangent basis
+    // --- stage reference state Phi^[t] (R1) and the un-projected velocity (L268), Cartesian
     F_VXT, F_VYT, F_VZT, F_UX, F_UY, F_UZ, F_RHOT, F_WT,
     // --- Phi^n (the prognostic state between large steps) and (rho theta)^n
     F_RHON, F_VXN, F_VYN, F_VZN, F_WN, F_PN, F_RTN,
@@ -54,6 +54,9 @@ struct Geom {                 // device pointers, device column order, padded to
     const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad
     const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)
     const double* rhat;       // [Npad][4]   unit vector of the column, 1 pad
+    const double* basis;      // [Npad][8]   tangent basis e1(3), e2(3), 2 pad
+    const double* wdiv2;      // [Npad][16]  7 x 2 divergence weights contracted with the basis of column j, 2 pad
+    const double* wgrad2;     // [Npad][12]  6 x 2 gradient weights contracted with the column's own basis
     const double* area;       // [Npad]
     const double* rinv;       // [128] 1/r_k              (pad layers: 0)
     const double* dlo;        // [128] r_h,k^2/(r_k^2 dz)
@@ -124,6 +127,14 @@ __device__ __forceinline__ void ld_rw(const double* p, double (&v)[E]) {
         v[2 * i] = t.x; v[2 * i + 1] = t.y;
     }
 }
+// A second read of a row this thread has already loaded (an L1 hit), kept out of the compiler's
+// common-subexpression elimination so that the first copy does not have to stay in registers.
+template <int E>
+__device__ __forceinline__ void ld_again(const double* p, double (&v)[E]) {
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i)
+        asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(v[2 * i]), "=d"(v[2 * i + 1]) : "l"(p + 2 * i));
+}
 template <int E>
 __device__ __forceinline__ void st_row(double* p, const double (&v)[E]) {
 #pragma unroll
@@ -134,6 +145,13 @@ __device__ __forceinline__ double3 ld_rhat(const double* rhat, int col) {   // [
     const double2 a = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col));
     const double2 b = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col) + 1);
     return make_double3(a.x, a.y, b.x);
+}
+
+struct Basis { double3 e1, e2; };
+__device__ __forceinline__ Basis ld_basis(const double* basis, int col) {   // [Npad][8]
+    const double2* p = reinterpret_cast<const double2*>(basis) + 4 * size_t(col);
+    const double2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+    return Basis{make_double3(a.x, a.y, b.x), make_double3(b.y, c.x, c.y)};
 }
 
 // Per-column stencil weights staged once per warp in shared memory (every lane of a column group
@@ -319,6 +337,7 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
 #pragma unroll
     for (int e = 0; e < E; ++e) real[e] = (L.k0 + e < nv) && (L.col < g.N);
 
+    const Basis B = ld_basis(g.basis, L.col);
     double rho[E], Vx[E], Vy[E], Vz[E], W[E], p[E], d[E];
     if (stage == 1) {
         ld_rw<E>(me + F_RHON * NVP, rho); ld_rw<E>(me + F_VXN * NVP, Vx); ld_rw<E>(me + F_VYN * NVP, Vy);
@@ -329,22 +348,29 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
 #pragma unroll
             for (int e = 0; e < E; ++e) out[e] += d[e];
         };
-        add(F_RHOT, F_RHOS, rho); add(F_VXT, F_VXS, Vx); add(F_VYT, F_VYS, Vy); add(F_VZT, F_VZS, Vz);
-        add(F_WT, F_WS, W);       add(F_PT, F_PS, p);
+        add(F_RHOT, F_RHOS, rho); add(F_WT, F_WS, W); add(F_PT, F_PS, p);
+        double va[E], vb[E];                                   // V^[t] += a e1 + b e2
+        ld_rw<E>(me + F_VXT * NVP, Vx); ld_rw<E>(me + F_VYT * NVP, Vy); ld_rw<E>(me + F_VZT * NVP, Vz);
+        ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, vb);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            Vx[e] += va[e] * B.e1.x + vb[e] * B.e2.x;
+            Vy[e] += va[e] * B.e1.y + vb[e] * B.e2.y;
+            Vz[e] += va[e] * B.e1.z + vb[e] * B.e2.z;
+        }
     }
 #pragma unroll
     for (int e = 0; e < E; ++e)
         if (!real[e]) { rho[e] = 1.0; p[e] = g.p_ref; Vx[e] = Vy[e] = Vz[e] = W[e] = 0.0; }
 
     const double3 rh = ld_rhat(g.rhat, L.col);
-    double h[E], th[E], rtt[E], irt[E], Wup[E], ux[E], uy[E], uz[E];
+    double h[E], th[E], rtt[E], Wup[E], ux[E], uy[E], uz[E];
     above<G, E>(W, Wup, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         h[e] = g.Cp * p[e] / (g.Rd * rho[e]);
         rtt[e] = eos_rt(p[e], g.Rd, g.p_ref, 1.0 / gam);
         th[e] = rtt[e] / rho[e];
-        irt[e] = 1.0 / rtt[e];
         const double wc = 0.5 * (W[e] + Wup[e]);                            // I_c[W]; the lid's W is the pad's 0
         const double ir = 1.0 / rho[e];
         ux[e] = (Vx[e] + wc * rh.x) * ir; uy[e] = (Vy[e] + wc * rh.y) * ir; uz[e] = (Vz[e] + wc * rh.z) * ir;
@@ -393,7 +419,7 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
     }
     st_row<E>(me + F_RHOT * NVP, rho); st_row<E>(me + F_VXT * NVP, Vx); st_row<E>(me + F_VYT * NVP, Vy);
     st_row<E>(me + F_VZT * NVP, Vz);   st_row<E>(me + F_WT * NVP, W);   st_row<E>(me + F_PT * NVP, p);
-    st_row<E>(me + F_H * NVP, h);      st_row<E>(me + F_TH * NVP, th);  st_row<E>(me + F_IRT * NVP, irt);
+    st_row<E>(me + F_H * NVP, h);      st_row<E>(me + F_TH * NVP, th);
     st_row<E>(me + F_UX * NVP, ux);    st_row<E>(me + F_UY * NVP, uy);  st_row<E>(me + F_UZ * NVP, uz);
     st_row<E>(me + F_FA * NVP, fa);    st_row<E>(me + F_FI * NVP, fi);  st_row<E>(me + F_FC * NVP, fc);
 
@@ -402,8 +428,8 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
         st_row<E>(me + F_RTN * NVP, rtt);
 #pragma unroll
         for (int e = 0; e < E; ++e) d[e] = 0.0;
-        st_row<E>(me + F_RHOS * NVP, d); st_row<E>(me + F_VXS * NVP, d); st_row<E>(me + F_VYS * NVP, d);
-        st_row<E>(me + F_VZS * NVP, d);  st_row<E>(me + F_WS * NVP, d);  st_row<E>(me + F_PS * NVP, d);
+        st_row<E>(me + F_RHOS * NVP, d); st_row<E>(me + F_VAS * NVP, d); st_row<E>(me + F_VBS * NVP, d);
+        st_row<E>(me + F_WS * NVP, d);   st_row<E>(me + F_PS * NVP, d);
         st_row<E>(me + F_RTS * NVP, d);
     } else {
         auto dev = [&](int fn, int fs, const double (&t)[E]) {
@@ -412,8 +438,16 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
             for (int e = 0; e < E; ++e) d[e] = real[e] ? d[e] - t[e] : 0.0;
             st_row<E>(me + fs * NVP, d);
         };
-        dev(F_RHON, F_RHOS, rho); dev(F_VXN, F_VXS, Vx); dev(F_VYN, F_VYS, Vy); dev(F_VZN, F_VZS, Vz);
-        dev(F_WN, F_WS, W);       dev(F_PN, F_PS, p);    dev(F_RTN, F_RTS, rtt);
+        dev(F_RHON, F_RHOS, rho); dev(F_WN, F_WS, W); dev(F_PN, F_PS, p); dev(F_RTN, F_RTS, rtt);
+        double dx[E], dy[E], dz[E], va[E], vb[E];              // (V^n - V^[t]) in the tangent basis
+        ld_rw<E>(me + F_VXN * NVP, dx); ld_rw<E>(me + F_VYN * NVP, dy); ld_rw<E>(me + F_VZN * NVP, dz);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            dx[e] -= Vx[e]; dy[e] -= Vy[e]; dz[e] -= Vz[e];
+            va[e] = real[e] ? dx[e] * B.e1.x + dy[e] * B.e1.y + dz[e] * B.e1.z : 0.0;
+            vb[e] = real[e] ? dx[e] * B.e2.x + dy[e] * B.e2.y + dz[e] * B.e2.z : 0.0;
+        }
+        st_row<E>(me + F_VAS * NVP, va); st_row<E>(me + F_VBS * NVP, vb);
     }
 }
 
@@ -422,7 +456,7 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
 // Gathers V^[t](3), h, theta, u(3), p^[t] from the 6 neighbours.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
 k_slow_terms(Geom g, double* __restrict__ S) {
     Map<G, E> L;
     constexpr int NVP = Map<G, E>::NVP;
@@ -440,7 +474,7 @@ k_slow_terms(Geom g, double* __restrict__ S) {
     const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
     __syncwarp();
 
-    double p0[E], h0[E], th0[E], V0x[E], V0y[E], V0z[E], u0x[E], u0y[E], u0z[E];
+    double p0[E];
     ld_nc<E>(me + F_PT * NVP, p0);
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], gpx[E], gpy[E], gpz[E];
 #pragma unroll
@@ -453,13 +487,7 @@ k_slow_terms(Geom g, double* __restrict__ S) {
         ld_nc<E>(q + F_VXT * NVP, x); ld_nc<E>(q + F_VYT * NVP, y); ld_nc<E>(q + F_VZT * NVP, z);
         ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
         ld_nc<E>(q + F_UX * NVP, ujx); ld_nc<E>(q + F_UY * NVP, ujy); ld_nc<E>(q + F_UZ * NVP, ujz);
-        if (j == 0) {
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                V0x[e] = x[e]; V0y[e] = y[e]; V0z[e] = z[e]; h0[e] = hj[e]; th0[e] = tj[e];
-                u0x[e] = ujx[e]; u0y[e] = ujy[e]; u0z[e] = ujz[e];
-            }
-        } else {
+        if (j > 0) {
             ld_nc<E>(q + F_PT * NVP, pj);
             const double gx = wgv[3 * (j - 1)], gy = wgv[3 * (j - 1) + 1], gz = wgv[3 * (j - 1) + 2];
 #pragma unroll
@@ -499,19 +527,19 @@ k_slow_terms(Geom g, double* __restrict__ S) {
 #pragma unroll
         for (int e = 0; e < E; ++e) out[e] = dhi[e] * Xup[e] - dlo[e] * X[e];
     };
-    double t[E];
-    vflux(u0x, t);
+    double t[E], q0[E];                 // the column's own rows again (L1 hits), one at a time
+    ld_again<E>(me + F_UX * NVP, q0); vflux(q0, t);
 #pragma unroll
     for (int e = 0; e < E; ++e) Ax[e] += t[e];
-    vflux(u0y, t);
+    ld_again<E>(me + F_UY * NVP, q0); vflux(q0, t);
 #pragma unroll
     for (int e = 0; e < E; ++e) Ay[e] += t[e];
-    vflux(u0z, t);
+    ld_again<E>(me + F_UZ * NVP, q0); vflux(q0, t);
 #pragma unroll
     for (int e = 0; e < E; ++e) Az[e] += t[e];
     double DhW[E], DtW[E], DW[E];
-    vflux(h0, DhW);
-    vflux(th0, DtW);
+    ld_again<E>(me + F_H * NVP, q0);  vflux(q0, DhW);
+    ld_again<E>(me + F_TH * NVP, q0); vflux(q0, DtW);
 #pragma unroll
     for (int e = 0; e < E; ++e) DW[e] = dhi[e] * Wup[e] - dlo[e] * W[e];
 
@@ -528,6 +556,8 @@ k_slow_terms(Geom g, double* __restrict__ S) {
         Z[e] = gt * W[e];
     }
     above<G, E>(Z, Zup, L.gl, 0.0);
+    double V0x[E], V0y[E], V0z[E];
+    ld_again<E>(me + F_VXT * NVP, V0x); ld_again<E>(me + F_VYT * NVP, V0y); ld_again<E>(me + F_VZT * NVP, V0z);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const bool real = (L.k0 + e < nv) && (L.col < g.N);
@@ -554,7 +584,16 @@ k_slow_terms(Geom g, double* __restrict__ S) {
                     ? -(p0[e] - pb[e]) / g.dz - g.gravity * 0.5 * (rb[e] + rho[e]) - 0.5 * (Frb[e] + Fr[e])
                     : 0.0;                                                    // Eq. 42
     }
-    st_row<E>(me + F_SVX * NVP, sVx); st_row<E>(me + F_SVY * NVP, sVy); st_row<E>(me + F_SVZ * NVP, sVz);
+    {
+        const Basis B = ld_basis(g.basis, L.col);
+        double sa[E], sb[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            sa[e] = sVx[e] * B.e1.x + sVy[e] * B.e1.y + sVz[e] * B.e1.z;
+            sb[e] = sVx[e] * B.e2.x + sVy[e] * B.e2.y + sVz[e] * B.e2.z;
+        }
+        st_row<E>(me + F_SVA * NVP, sa); st_row<E>(me + F_SVB * NVP, sb);
+    }
     st_row<E>(me + F_SRHO * NVP, srho); st_row<E>(me + F_SW * NVP, sW); st_row<E>(me + F_SP * NVP, sp);
     st_row<E>(me + F_SRT * NVP, srt);
 }
@@ -570,50 +609,49 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
     {   // L2 schedule: own look-ahead (ascending), and hand-over to the column-solve kernel
         const int nblk = gridDim.x, b = blockIdx.x;
         if (tn.ahead > 0 && b + tn.ahead < nblk) {
-            prefetch_block_rows<G, E>(S, b + tn.ahead, F_VXS, 3);
+            prefetch_block_rows<G, E>(S, b + tn.ahead, F_VAS, 2);
             prefetch_block_rows<G, E>(S, b + tn.ahead, F_PS, 1);
-            prefetch_block_rows<G, E>(S, b + tn.ahead, F_SVX, 3);
+            prefetch_block_rows<G, E>(S, b + tn.ahead, F_SVA, 2);
         }
         if (tn.tail > 0 && b >= nblk - tn.tail) {
             const int t = tn.rev ? b : nblk - 1 - b;      // the block of columns k_vertical reaches at the same rank
-            prefetch_block_rows<G, E>(S, t, F_H, F_IRT - F_H + 1);
+            prefetch_block_rows<G, E>(S, t, F_H, F_PT - F_H + 1);
         }
     }
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
-    __shared__ double wsm[kWarpsPerBlock * 32 / G][18];
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][12];
     double* wgv = wsm[threadIdx.x / G];
-    stage_weights<G>(g.wgrad + size_t(L.col) * 18, wgv, 9, L.gl);
+    stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, wgv, 6, L.gl);
     const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
     const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
     __syncwarp();
-    double p0[E], pj[6][E], gx[E], gy[E], gz[E];
+    double p0[E], pj[6][E], ga[E], gb[E];
     ld_nc<E>(me + F_PS * NVP, p0);
 #pragma unroll
     for (int j = 0; j < 6; ++j) ld_nc<E>(S + size_t(nb[j]) * REC + L.k0 + F_PS * NVP, pj[j]);
-    double ri[E], vx[E], vy[E], vz[E], sx[E], sy[E], sz[E];
+    double ri[E], va[E], vb[E], sa[E], sb[E];
     ld_nc<E>(g.rinv + L.k0, ri);
-    ld_rw<E>(me + F_VXS * NVP, vx); ld_rw<E>(me + F_VYS * NVP, vy); ld_rw<E>(me + F_VZS * NVP, vz);
-    ld_nc<E>(me + F_SVX * NVP, sx); ld_nc<E>(me + F_SVY * NVP, sy); ld_nc<E>(me + F_SVZ * NVP, sz);
+    ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, vb);
+    ld_nc<E>(me + F_SVA * NVP, sa); ld_nc<E>(me + F_SVB * NVP, sb);
 #pragma unroll
-    for (int e = 0; e < E; ++e) gx[e] = gy[e] = gz[e] = 0.0;
+    for (int e = 0; e < E; ++e) ga[e] = gb[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double d = pj[j][e] - p0[e];
-            gx[e] = fma(wgv[3 * j], d, gx[e]); gy[e] = fma(wgv[3 * j + 1], d, gy[e]); gz[e] = fma(wgv[3 * j + 2], d, gz[e]);
+            ga[e] = fma(wgv[2 * j], d, ga[e]); gb[e] = fma(wgv[2 * j + 1], d, gb[e]);
         }
     }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-        vx[e] = fma(delta, sx[e] - gx[e] * ri[e], vx[e]);
-        vy[e] = fma(delta, sy[e] - gy[e] * ri[e], vy[e]);
-        vz[e] = fma(delta, sz[e] - gz[e] * ri[e], vz[e]);
+        va[e] = fma(delta, sa[e] - ga[e] * ri[e], va[e]);
+        vb[e] = fma(delta, sb[e] - gb[e] * ri[e], vb[e]);
     }
-    st_row<E>(me + F_VXS * NVP, vx); st_row<E>(me + F_VYS * NVP, vy); st_row<E>(me + F_VZS * NVP, vz);
+    st_row<E>(me + F_VAS * NVP, va); st_row<E>(me + F_VBS * NVP, vb);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -625,42 +663,39 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
 // substep stored it, which saves one row of HBM reads.
 //
 // vertical_column is the work of one lane group on one column.  `own` points at row 0 (layer k0)
-// of the column's own rows F_VXS..F_IRT -- in global memory (k_vertical) or in the shared-memory
+// of the column's own rows F_VAS..F_PT -- in global memory (k_vertical) or in the shared-memory
 // stage a TMA bulk copy has filled (k_vertical_tma); neighbours are always gathered from global
 // memory (L1/L2 hits).  wdv: the column's 21 divergence weights in shared memory.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
-__device__ __forceinline__ void vertical_column(const Geom& g, double* __restrict__ S, const double* own, const double* wdv,
-                                                int col, int gl, int k0, double delta, int first) {
+__device__ __forceinline__ void vertical_column(const Geom& g, double* __restrict__ me, const double* own,
+                                                const double* const (&nbp)[6], const double* wdv,
+                                                int gl, int k0, double delta, int first) {
     constexpr int NVP = G * E;
-    constexpr size_t REC = size_t(NF) * NVP;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
-    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
 
-    double divV[E], divhV[E], divtV[E], th0[E];
+    double divV[E], divhV[E], divtV[E], th0[E], h0[E];
     {
-        double x[E], y[E], z[E], hj[E];
-        ld_rw<E>(own + F_VXS * NVP, x); ld_rw<E>(own + F_VYS * NVP, y); ld_rw<E>(own + F_VZS * NVP, z);
-        ld_rw<E>(own + F_H * NVP, hj);  ld_rw<E>(own + F_TH * NVP, th0);
-        const double wx = wdv[0], wy = wdv[1], wz = wdv[2];
+        double x[E], y[E];
+        ld_rw<E>(own + F_VAS * NVP, x); ld_rw<E>(own + F_VBS * NVP, y);
+        ld_rw<E>(own + F_H * NVP, h0);  ld_rw<E>(own + F_TH * NVP, th0);
+        const double wa = wdv[0], wb = wdv[1];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double d = fma(wx, x[e], fma(wy, y[e], wz * z[e]));
-            divV[e] = d; divhV[e] = hj[e] * d; divtV[e] = th0[e] * d;
+            const double d = fma(wa, x[e], wb * y[e]);
+            divV[e] = d; divhV[e] = h0[e] * d; divtV[e] = th0[e] * d;
         }
     }
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const double* q = S + size_t(nb[j]) * REC + k0;
-        const double wx = wdv[3 * j + 3], wy = wdv[3 * j + 4], wz = wdv[3 * j + 5];
-        double x[E], y[E], z[E], hj[E], tj[E];
-        ld_nc<E>(q + F_VXS * NVP, x); ld_nc<E>(q + F_VYS * NVP, y); ld_nc<E>(q + F_VZS * NVP, z);
-        ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
+        const double* q = nbp[j];
+        const double wa = wdv[2 * j + 2], wb = wdv[2 * j + 3];
+        double x[E], y[E], hj[E], tj[E];
+        ld_rw<E>(q + F_VAS * NVP, x); ld_rw<E>(q + F_VBS * NVP, y);
+        ld_rw<E>(q + F_H * NVP, hj);  ld_rw<E>(q + F_TH * NVP, tj);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double d = fma(wx, x[e], fma(wy, y[e], wz * z[e]));
+            const double d = fma(wa, x[e], wb * y[e]);
             divV[e] += d;
             divhV[e] = fma(hj[e], d, divhV[e]);
             divtV[e] = fma(tj[e], d, divtV[e]);
@@ -672,7 +707,12 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
     double rho_s[E], p_s[E], W_s[E], rts[E], srho[E], sp[E], sW[E], srt[E], pt[E], irt[E];
     ld_rw<E>(own + F_RHOS * NVP, rho_s); ld_rw<E>(own + F_WS * NVP, W_s); ld_rw<E>(own + F_RTS * NVP, rts);
     ld_rw<E>(own + F_SRHO * NVP, srho);  ld_rw<E>(own + F_SP * NVP, sp);  ld_rw<E>(own + F_SW * NVP, sW);
-    ld_rw<E>(own + F_SRT * NVP, srt);    ld_rw<E>(own + F_PT * NVP, pt);  ld_rw<E>(own + F_IRT * NVP, irt);
+    ld_rw<E>(own + F_SRT * NVP, srt);    ld_rw<E>(own + F_PT * NVP, pt);
+    {   // 1/(rho theta)^[t] from rows already here: h/theta = Cp p/(Rd rho theta)
+        const double kap = g.Rd / g.Cp;
+#pragma unroll
+        for (int e = 0; e < E; ++e) irt[e] = kap * h0[e] / (th0[e] * pt[e]);
+    }
     if (first) {
         ld_rw<E>(own + F_PS * NVP, p_s);
     } else {
@@ -715,7 +755,6 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
         rts[e] = rts[e] + delta * (srt[e] - divtV[e] * ri[e] - (dhi[e] * Xup[e] - dlo[e] * X[e]));  // Eq. 35
         p_s[e] = eos_dev(rts[e] * irt[e], pt[e], gam, g);                                            // Eq. 36
     }
-    double* me = S + size_t(col) * REC + k0;
     st_row<E>(me + F_WS * NVP, Wn);   st_row<E>(me + F_RHOS * NVP, rho_s);
     st_row<E>(me + F_RTS * NVP, rts); st_row<E>(me + F_PS * NVP, p_s);
 }
@@ -729,26 +768,42 @@ k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
     {   // L2 schedule: own look-ahead in walking order, and hand-over to the next momentum kernel
         const int b = blockIdx.x;
         if (tn.ahead > 0 && b + tn.ahead < nblk)
-            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - (b + tn.ahead) : b + tn.ahead, F_VXS, F_IRT + 1);
+            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - (b + tn.ahead) : b + tn.ahead, F_VAS, F_PT + 1);
         if (tn.tail > 0 && b >= nblk - tn.tail)
-            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - b : b - (nblk - tn.tail), F_SVX, 3);
+            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - b : b - (nblk - tn.tail), F_SVA, 2);
     }
-    __shared__ double wsm[kWarpsPerBlock * 32 / G][24];
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][16];
     double* wdv = wsm[threadIdx.x / G];
-    stage_weights<G>(g.wdiv + size_t(L.col) * 24, wdv, 12, L.gl);
+    stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    constexpr size_t REC = Map<G, E>::REC;
+    const double* const nbp[6] = {S + size_t(n03.x) * REC + L.k0, S + size_t(n03.y) * REC + L.k0, S + size_t(n03.z) * REC + L.k0,
+                                  S + size_t(n03.w) * REC + L.k0, S + size_t(n47.x) * REC + L.k0, S + size_t(n47.y) * REC + L.k0};
     __syncwarp();
-    vertical_column<G, E>(g, S, S + size_t(L.col) * Map<G, E>::REC + L.k0, wdv, L.col, L.gl, L.k0, delta, first);
+    double* me = S + size_t(L.col) * REC + L.k0;
+    vertical_column<G, E>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first);
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2, TMA-staged: persistent blocks of kTmaWarps warps walk tiles of TCOL = kTmaWarps*32/G columns.
-// The own rows F_VXS..F_IRT of a tile (the contiguous head of each column record) are brought into
-// shared memory by cp.async.bulk (TMA) NSTAGE tiles ahead of their use and signalled through
-// mbarriers, so HBM requests are in flight without holding registers or stalling warps; only the
-// neighbour gathers (L1/L2 hits) are ordinary loads.
+// K2, TMA-staged (the production path where the shape has one): persistent blocks of kTmaWarps warps
+// walk tiles of TCOL = kTmaWarps*32/G consecutive columns -- 2x2 / 2x4 / 4x4 patches of the rhombus
+// lattice in the Morton device order.  EVERYTHING a tile reads is brought into shared memory by
+// cp.async.bulk (TMA) and signalled through an mbarrier: the own rows F_VAS..F_PT of its columns
+// (the contiguous head of each record), the gathered rows F_VAS..F_TH of its halo columns (host
+// table TileTab::halo, <= hmax per tile), its divergence weights and its neighbour-slot table.
+// HBM and L2 requests are therefore in flight without holding registers or stalling a warp, and the
+// compute phase touches only shared memory; results go straight to global memory.
 // ---------------------------------------------------------------------------------------------
 constexpr int kTmaWarps = 4;
-constexpr int kOwnRows = F_IRT + 1;     // 17
+constexpr int kOwnRows = F_PT + 1;      // 16
+constexpr int kHaloRows = F_TH + 1;     // 4
+
+struct TileTab {
+    const int* halo;              // [ntiles][hmax] device columns of the tile's halo (padded with the tile's first column)
+    const unsigned char* slots;   // [Npad][8] per column: slot of each of the 6 neighbours (own: 0..TCOL-1, halo: TCOL + i), 2 pad
+    int hmax;
+};
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
@@ -771,38 +826,48 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 
 template <int G, int E, int NSTAGE>
 __global__ void __launch_bounds__(kTmaWarps * 32)
-k_vertical_tma(Geom g, double* __restrict__ S, double delta, int first, int ntiles, int rev) {
+k_vertical_staged(Geom g, TileTab tt, double* __restrict__ S, double delta, int first, int ntiles, int rev) {
     constexpr int NVP = G * E, CPW = 32 / G, TCOL = kTmaWarps * CPW;
     constexpr size_t REC = size_t(NF) * NVP;
-    constexpr int STAGE_DOUBLES = TCOL * kOwnRows * NVP;
+    const int HM = tt.hmax;
+    // one stage: own rows [TCOL][16][NVP] | halo rows [HM][4][NVP] | weights [TCOL][16] | slots [TCOL] x 8 bytes
+    const int o_halo = TCOL * kOwnRows * NVP, o_w = o_halo + HM * kHaloRows * NVP, o_sl = o_w + TCOL * 16;
+    const int stage_doubles = o_sl + TCOL;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* stage = reinterpret_cast<double*>(smem_raw);                       // [NSTAGE][TCOL][17][NVP]
-    double* wsm = stage + size_t(NSTAGE) * STAGE_DOUBLES;                       // [TCOL][24]
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(wsm + TCOL * 24);   // [NSTAGE]
+    double* stage0 = reinterpret_cast<double*>(smem_raw);
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(stage0 + size_t(NSTAGE) * stage_doubles);
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int slot = warp * CPW + lane / G;       // column of the tile this lane group owns
     const int gl = lane & (G - 1), k0 = gl * E;
-    // tile i of this block = tile blockIdx.x + i*gridDim.x in walking order
     const int my_tiles = (ntiles - int(blockIdx.x) + int(gridDim.x) - 1) / int(gridDim.x);
     auto tile_of = [&](int i) { const int t = int(blockIdx.x) + i * int(gridDim.x); return rev ? ntiles - 1 - t : t; };
-    // producer: the first warp; lane 0 arms the barrier, lane c copies column c of the tile
+    // producer: the first warp; lane 0 arms the barrier, then the lanes share the copies
     auto issue = [&](int i) {
         if (warp != 0) return;
-        const int s = i % NSTAGE;
+        const int t = tile_of(i);
+        double* st = stage0 + size_t(i % NSTAGE) * stage_doubles;
+        unsigned long long* bar = full + i % NSTAGE;
         const unsigned row = NVP * 8u;
-        const unsigned bytes = TCOL * (first ? kOwnRows : kOwnRows - 1) * row;
-        if (lane == 0) mbar_expect_tx(full + s, bytes);
+        if (lane == 0) {
+            mbar_expect_tx(bar, TCOL * (first ? kOwnRows : kOwnRows - 1) * row + HM * kHaloRows * row + TCOL * 16 * 8u + TCOL * 8u);
+            bulk_g2s(st + o_w, g.wdiv2 + size_t(t) * TCOL * 16, TCOL * 16 * 8u, bar);
+            bulk_g2s(st + o_sl, tt.slots + size_t(t) * TCOL * 8, TCOL * 8u, bar);
+        }
         __syncwarp();
         for (int c = lane; c < TCOL; c += 32) {
-            const double* src = S + (size_t(tile_of(i)) * TCOL + c) * REC;
-            double* dst = stage + size_t(s) * STAGE_DOUBLES + size_t(c) * kOwnRows * NVP;
+            const double* src = S + (size_t(t) * TCOL + c) * REC;
+            double* dst = st + size_t(c) * kOwnRows * NVP;
             if (first) {
-                bulk_g2s(dst, src, kOwnRows * row, full + s);
+                bulk_g2s(dst, src, kOwnRows * row, bar);
             } else {                                     // skip the p* row: it is re-evaluated from (rho theta)*
-                bulk_g2s(dst, src, F_PS * row, full + s);
-                bulk_g2s(dst + (F_PS + 1) * NVP, src + (F_PS + 1) * NVP, (kOwnRows - F_PS - 1) * row, full + s);
+                bulk_g2s(dst, src, F_PS * row, bar);
+                bulk_g2s(dst + (F_PS + 1) * NVP, src + (F_PS + 1) * NVP, (kOwnRows - F_PS - 1) * row, bar);
             }
+        }
+        for (int h = lane; h < HM; h += 32) {
+            const int c = __ldg(tt.halo + size_t(t) * HM + h);
+            bulk_g2s(st + o_halo + size_t(h) * kHaloRows * NVP, S + size_t(c) * REC, kHaloRows * row, bar);
         }
     };
     if (threadIdx.x == 0) {
@@ -813,15 +878,19 @@ k_vertical_tma(Geom g, double* __restrict__ S, double delta, int first, int ntil
     for (int i = 0; i < NSTAGE && i < my_tiles; ++i) issue(i);
 
     for (int i = 0; i < my_tiles; ++i) {
-        const int s = i % NSTAGE;
+        const double* st = stage0 + size_t(i % NSTAGE) * stage_doubles;
+        mbar_wait(full + i % NSTAGE, (i / NSTAGE) & 1);
+        const uint2 sl = *reinterpret_cast<const uint2*>(st + o_sl + slot);
+        auto row0 = [&](unsigned b) -> const double* {      // rows F_VAS.. of the column in slot b, at layer k0
+            return b < unsigned(TCOL) ? st + size_t(b) * kOwnRows * NVP + k0
+                                      : st + o_halo + size_t(b - TCOL) * kHaloRows * NVP + k0;
+        };
+        const double* const nbp[6] = {row0(sl.x & 255u), row0((sl.x >> 8) & 255u), row0((sl.x >> 16) & 255u),
+                                      row0(sl.x >> 24),  row0(sl.y & 255u),        row0((sl.y >> 8) & 255u)};
         const int col = tile_of(i) * TCOL + slot;
-        double* wdv = wsm + slot * 24;
-        stage_weights<G>(g.wdiv + size_t(col) * 24, wdv, 12, gl);
-        __syncwarp();
-        mbar_wait(full + s, (i / NSTAGE) & 1);
-        vertical_column<G, E>(g, S, stage + size_t(s) * STAGE_DOUBLES + size_t(slot) * kOwnRows * NVP + k0, wdv,
-                              col, gl, k0, delta, first);
-        __syncthreads();                                  // every warp has read stage s (and its weights)
+        vertical_column<G, E>(g, S + size_t(col) * REC + k0, st + size_t(slot) * kOwnRows * NVP + k0, nbp,
+                              st + o_w + slot * 16, gl, k0, delta, first);
+        __syncthreads();                                  // every warp has read this stage
         if (i + NSTAGE < my_tiles) issue(i + NSTAGE);
     }
 }
@@ -843,7 +912,19 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, double dt) {
 #pragma unroll
         for (int e = 0; e < E; ++e) out[e] += d[e];
     };
-    sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p); sum(F_VXT, F_VXS, vx); sum(F_VYT, F_VYS, vy); sum(F_VZT, F_VZS, vz);
+    sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p);
+    {
+        const Basis B = ld_basis(g.basis, L.col);
+        double va[E];
+        ld_rw<E>(me + F_VXT * NVP, vx); ld_rw<E>(me + F_VYT * NVP, vy); ld_rw<E>(me + F_VZT * NVP, vz);
+        ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, d);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            vx[e] += va[e] * B.e1.x + d[e] * B.e2.x;
+            vy[e] += va[e] * B.e1.y + d[e] * B.e2.y;
+            vz[e] += va[e] * B.e1.z + d[e] * B.e2.z;
+        }
+    }
     sum(F_WT, F_WS, a);
     st_row<E>(me + F_WN * NVP, a);
     if (F.k_v) {
