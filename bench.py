@@ -29,14 +29,21 @@ WORKLOAD = 3
 METRIC = "cell-updates/s (cols x layers x acoustic substeps) FP64"
 UNIT = "cell-updates/s"
 
-# algorithmic bytes per cell per launch; geometry bytes are per column
-K2_MIN_DOUBLES = 18      # SURVEY 8(d) split: 14 reads (V*'(3) re-read, p*, W*, rho*, rho-theta, 4 slow terms,
-                         # rho^t, p^t, theta^t) + 4 writes
-K2_DESIGN_DOUBLES = 21   # what this design's kernel touches once: 17 reads (LU factors instead of rho^t) + 4 writes
-K1_DOUBLES = 10          # p*, V*(3), slowV(3) read; V*'(3) written
-SUBSTEP_SURVEY_DOUBLES = 27   # B_dep of SURVEY 8(d)
-K2_GEOM_BYTES = 6 * 4 + 21 * 8
-K1_GEOM_BYTES = 6 * 4 + 18 * 8
+# algorithmic bytes per cell per launch (DESIGN.md section 8 "byte budget"); geometry bytes are per column
+K2_SURVEY_DOUBLES = 18   # k_vertical's share of SURVEY 8(d)'s 27 doubles: 14 reads (V*'(3) re-read, p*, W*, rho*,
+                         # rho-theta, 4 slow terms, rho^t, p^t, theta^t) + 4 writes
+K2_DESIGN_DOUBLES = 19   # what this design's kernel moves once per cell: 15 reads (V*' as 2 tangent components, h,
+                         # theta, rho*, W*, (rho theta)*, 4 slow terms, 3 LU factors, p^t) + 4 writes
+K1_SURVEY_DOUBLES = 10   # k_momentum's share: p*, V*(3), slowV(3) read; V*'(3) written
+K1_DESIGN_DOUBLES = 7    # p*, V*(2), slowV(2) read; V*'(2) written
+SUBSTEP_SURVEY_DOUBLES = 27   # B_dep of SURVEY 8(d) = the figure the 60 % target is stated on
+SUBSTEP_DESIGN_DOUBLES = K1_DESIGN_DOUBLES + K2_DESIGN_DOUBLES
+SURVEY_GEOM_BYTES = 336       # per column, SURVEY 8(d)
+K2_GEOM_BYTES = 8 * 4 + 16 * 8    # this design: 8 int32 neighbour slots + 7x2 (+2 pad) contracted divergence weights
+K1_GEOM_BYTES = 8 * 4 + 12 * 8    # 8 int32 + 6x2 contracted gradient weights
+# HBM traffic of one k_vertical launch on config 3 from the committed ncu --set full capture
+# (profiles/r01c_substep_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum)
+K2_NCU_TRAFFIC_BYTES = {3: 200.3e6}
 
 
 def measured_peak():
@@ -77,6 +84,25 @@ class ClockSampler(threading.Thread):
         reasons = [n for i, n in enumerate(names) if any(s[3 + i].lower().startswith("active") for s in self.samples)]
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
                 "samples": len(sm), "power_w_max": max(float(s[2]) for s in self.samples)}
+
+
+def max_over_ranks(values, device="cpu"):
+    """Element-wise MAX of a list of floats over all ranks (the timing rule for N > 1).  Works with
+    any initialised torch.distributed backend (nccl on the GPU box, gloo in the CPU tests); without
+    a process group it is the identity."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def aggregate_value(cells_per_step, steps, world, ms):
+    """Whole-job throughput of `world` independent replicas (weak scaling, no data-path collective):
+    units all ranks processed / the slowest rank's time."""
+    return cells_per_step * steps * world / (ms * 1e-3)
 
 
 def sample_config(level):
@@ -211,27 +237,31 @@ def run_cuda(args):
         barrier()
 
     io_bytes = int(sum(a.nbytes for a in h_in))
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
-    value = cells_per_step * args.steps * world / (ms * 1e-3)
-    e2e_value = cells_per_step * args.steps * world / e2e_s
+    ms, e2e_s = max_over_ranks([ms, e2e_s], device="cuda")
+    value = aggregate_value(cells_per_step, args.steps, world, ms)
+    e2e_value = aggregate_value(cells_per_step, args.steps, world, e2e_s * 1e3)
 
     peak, peak_kind = measured_peak()
     cells = N * nv
-    k2_bytes = cells * K2_MIN_DOUBLES * 8 + N * K2_GEOM_BYTES
+    k2_bytes = cells * K2_SURVEY_DOUBLES * 8 + N * K2_GEOM_BYTES
     achieved = k2_bytes / (k2_ms * 1e-3) / 1e9
+    sub_survey_bytes = cells * SUBSTEP_SURVEY_DOUBLES * 8 + N * SURVEY_GEOM_BYTES
+    sub_design_bytes = cells * SUBSTEP_DESIGN_DOUBLES * 8 + N * (K1_GEOM_BYTES + K2_GEOM_BYTES)
     roofline = {"bound": "hbm", "kernel": "k_vertical (a5-a9: divergences + column solve + rho, rho-theta, p*)",
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": K2_NCU_TRAFFIC_BYTES.get(WORKLOAD),
                 "peak_kind": peak_kind, "ms_per_launch": k2_ms, "bytes_per_launch": k2_bytes,
+                "bytes_per_launch_design": cells * K2_DESIGN_DOUBLES * 8 + N * K2_GEOM_BYTES,
                 "achieved_design_bytes": (cells * K2_DESIGN_DOUBLES * 8 + N * K2_GEOM_BYTES) / (k2_ms * 1e-3) / 1e9,
                 "k1_ms_per_launch": k1_ms,
-                "k1_achieved": (cells * K1_DOUBLES * 8 + N * K1_GEOM_BYTES) / (k1_ms * 1e-3) / 1e9,
+                "k1_achieved_survey_bytes": (cells * K1_SURVEY_DOUBLES * 8 + N * K1_GEOM_BYTES) / (k1_ms * 1e-3) / 1e9,
+                "k1_achieved_design_bytes": (cells * K1_DESIGN_DOUBLES * 8 + N * K1_GEOM_BYTES) / (k1_ms * 1e-3) / 1e9,
+                # the acoustic substep a4-a9 (both kernels back to back): what north_star's 60 % target is stated on
                 "substep_ms": sub_ms,
-                "substep_frac_survey_budget": (cells * SUBSTEP_SURVEY_DOUBLES * 8 + N * 336) / (sub_ms * 1e-3) / 1e9 / peak,
-                "substep_frac_of_8TBs": (cells * SUBSTEP_SURVEY_DOUBLES * 8 + N * 336) / (sub_ms * 1e-3) / 1e9 / 8000.0,
-                "substep_cell_updates_per_s": cells / (sub_ms * 1e-3)}
+                "substep_cell_updates_per_s": cells / (sub_ms * 1e-3),
+                "substep_frac_survey_budget_of_measured_peak": sub_survey_bytes / (sub_ms * 1e-3) / 1e9 / peak,
+                "substep_frac_survey_budget_of_8TBs": sub_survey_bytes / (sub_ms * 1e-3) / 1e9 / 8000.0,
+                "substep_frac_design_bytes_of_measured_peak": sub_design_bytes / (sub_ms * 1e-3) / 1e9 / peak}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -242,7 +272,7 @@ def run_cuda(args):
             "config": {"workload": "config 3: level 6 (40962 columns) x 32 layers, hot-Jupiter constants, dt=300 s, "
                                    "n=8 (13 substeps per large step), Newtonian relaxation forcing",
                        "cells": cells, "substeps_per_step": substeps, "parallelism": "replicas x%d" % world,
-                       "l2": "working set 35 arrays x 10.5 MB = 367 MB > 126 MB L2, no flush"},
+                       "l2": "one large step streams the 33-row column-record slab (346 MB) > 126 MB L2; no flush"},
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
