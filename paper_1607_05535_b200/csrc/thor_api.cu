@@ -79,6 +79,7 @@ struct thor_state {
     bool has_Teq = false, has_kT = false, has_kv = false;
     double *col_mass = nullptr, *col_energy = nullptr;
     bool stepped = false;
+    int walk = 0;                    // direction of the last launch (0 ascending, 1 descending)
 };
 
 namespace {
@@ -222,14 +223,16 @@ int flat_blocks(size_t n) { return int((n + 255) / 256); }
 
 // L2 schedule of the two acoustic kernels; THOR_B200_TUNE="rev,k1_ahead,k2_ahead,tail"
 // overrides the defaults for measurement.
-struct TunePair { Tune k1, k2; int tma_stages, tma_ctas; };
+struct TunePair { Tune k1, k2, ks; int zigzag, tma_stages, tma_ctas; };
 TunePair tune() {
-    int v[6] = {1, 0, 148, 148, 0, 4};
+    int v[7] = {1, 0, 148, 148, 0, 4, 148};
     if (const char* e = std::getenv("THOR_B200_TUNE"))
-        std::sscanf(e, "%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5]);
+        std::sscanf(e, "%d,%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5], &v[6]);
     TunePair p;
-    p.k1 = Tune{v[0], v[1], v[3]};
-    p.k2 = Tune{v[0], v[2], v[3]};
+    p.zigzag = v[0];                 // 1: successive kernels walk the columns in alternating directions
+    p.k1 = Tune{0, v[1], v[3]};      // k_momentum: look-ahead, tail hand-over
+    p.k2 = Tune{0, v[2], v[3]};      // k_vertical
+    p.ks = Tune{0, v[6], 0};         // stage kernels and k_finish: look-ahead only
     p.tma_stages = v[4];      // 0: direct-load column-solve kernel; 1 or 2: TMA-staged, that many stages per block
     p.tma_ctas = v[5];        // persistent blocks per SM of the TMA-staged kernel
     return p;
@@ -466,18 +469,22 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     const Geom g = make_geom(s->grid);
     const TunePair tn = tune();
     double* S = s->S;
+    // every launch walks the columns opposite to the one before it (L2 hand-over)
+    auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
     for (int step = 0; step < n_large; ++step) {
         for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
             const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
             const double delta = stage == 1 ? dt / 3.0 : dt / n;
-            THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta);
-            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S);
+            THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks));
+            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks));
             for (int sub = 0; sub < ns; ++sub) {
-                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, tn.k1);
-                if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, tn, st)) return rc;
+                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
+                TunePair t2 = tn;
+                t2.k2 = dir(tn.k2);
+                if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st)) return rc;
             }
         }
-        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt);
+        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt, dir(tn.ks));
     }
     CU(cudaGetLastError());
     s->stepped = s->stepped || n_large > 0;
@@ -492,10 +499,13 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     const int Npad = s->grid->d.Npad;
     const Geom g = make_geom(s->grid);
     const TunePair tn = tune();
+    auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
     for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, tn.k1);
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1));
+        TunePair t2 = tn;
+        if (which & 2) t2.k2 = dir(tn.k2);
         if (which & 2)
-            if (int rc = launch_vertical(s->grid, g, s->S, delta, 0, tn, s->stream)) return rc;
+            if (int rc = launch_vertical(s->grid, g, s->S, delta, 0, t2, s->stream)) return rc;
     }
     CU(cudaGetLastError());
     return THOR_OK;

@@ -71,12 +71,24 @@ struct Forcing {              // [Npad][NVP] each, may be null (Eq. 51-52)
     const double *T_eq, *k_T, *k_v;
 };
 
-// Launch-time knobs of the two acoustic kernels (defaults in thor_api.cu).
+// L2 schedule of one launch (defaults in thor_api.cu).  Successive kernels of a
+// large step walk the columns in ALTERNATING directions, so each starts on the rows the previous one has
+// just left in the 126 MB L2.
 struct Tune {
-    int rev;    // 1: the column-solve kernel walks the blocks in descending order, so that each kernel starts
-                //    on the columns the previous one has just left in L2
+    int rev;    // 1: this launch walks the blocks in descending column order
     int ahead;  // blocks of look-ahead of the in-kernel bulk L2 prefetch (0 = off)
-    int tail;   // the last `tail` blocks of a kernel prefetch the rows the NEXT kernel reads first (0 = off)
+    int tail;   // the last `tail` blocks (in walking order) prefetch rows the NEXT kernel reads first (0 = off)
+};
+struct Walk {
+    int bid;         // block of columns this thread block works on
+    int ahead_bid;   // block to prefetch for (walking order), -1 = none
+    bool in_tail;
+    __device__ explicit Walk(const Tune& tn) {
+        const int nblk = gridDim.x, b = blockIdx.x;
+        bid = tn.rev ? nblk - 1 - b : b;
+        ahead_bid = (tn.ahead > 0 && b + tn.ahead < nblk) ? (tn.rev ? nblk - 1 - (b + tn.ahead) : b + tn.ahead) : -1;
+        in_tail = tn.tail > 0 && b >= nblk - tn.tail;
+    }
 };
 
 // TMA bulk prefetch of a contiguous global range into L2 (no shared memory, no registers held)
@@ -327,8 +339,17 @@ k_grad(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* __
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
-    Map<G, E> L;
+k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn) {
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) {
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHON, stage == 1 ? 6 : 7);
+        if (stage > 1) {
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 3);
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHOT, 2);
+        }
+    }
     constexpr int NVP = Map<G, E>::NVP;
     double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
     const int nv = g.nv;
@@ -457,8 +478,13 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta) {
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
-k_slow_terms(Geom g, double* __restrict__ S) {
-    Map<G, E> L;
+k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) {
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_H, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 8);
+    }
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
@@ -605,19 +631,14 @@ k_slow_terms(Geom g, double* __restrict__ S) {
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
-    Map<G, E> L;
-    {   // L2 schedule: own look-ahead (ascending), and hand-over to the column-solve kernel
-        const int nblk = gridDim.x, b = blockIdx.x;
-        if (tn.ahead > 0 && b + tn.ahead < nblk) {
-            prefetch_block_rows<G, E>(S, b + tn.ahead, F_VAS, 2);
-            prefetch_block_rows<G, E>(S, b + tn.ahead, F_PS, 1);
-            prefetch_block_rows<G, E>(S, b + tn.ahead, F_SVA, 2);
-        }
-        if (tn.tail > 0 && b >= nblk - tn.tail) {
-            const int t = tn.rev ? b : nblk - 1 - b;      // the block of columns k_vertical reaches at the same rank
-            prefetch_block_rows<G, E>(S, t, F_H, F_PT - F_H + 1);
-        }
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) {
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 1);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_SVA, 2);
     }
+    if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_H, F_PT - F_H + 1);   // the column-solve kernel starts here
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
@@ -762,16 +783,10 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
-    const int nblk = gridDim.x;
-    const int bid = tn.rev ? nblk - 1 - int(blockIdx.x) : int(blockIdx.x);
-    Map<G, E> L(bid);
-    {   // L2 schedule: own look-ahead in walking order, and hand-over to the next momentum kernel
-        const int b = blockIdx.x;
-        if (tn.ahead > 0 && b + tn.ahead < nblk)
-            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - (b + tn.ahead) : b + tn.ahead, F_VAS, F_PT + 1);
-        if (tn.tail > 0 && b >= nblk - tn.tail)
-            prefetch_block_rows<G, E>(S, tn.rev ? nblk - 1 - b : b - (nblk - tn.tail), F_SVA, 2);
-    }
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, F_PT + 1);
+    if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_SVA, 2);               // the next momentum kernel starts here
     __shared__ double wsm[kWarpsPerBlock * 32 / G][16];
     double* wdv = wsm[threadIdx.x / G];
     stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
@@ -901,8 +916,14 @@ k_vertical_staged(Geom g, TileTab tt, double* __restrict__ S, double delta, int 
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_finish(Geom g, double* __restrict__ S, Forcing F, double dt) {
-    Map<G, E> L;
+k_finish(Geom g, double* __restrict__ S, Forcing F, double dt, Tune tn) {
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) {
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 3);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHOT, 2);
+    }
     constexpr int NVP = Map<G, E>::NVP;
     double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
     const size_t to = size_t(L.col) * NVP + L.k0;

@@ -120,6 +120,21 @@ def test_every_layer_shape_one_step(nv):
     _compare(st.get(), ref, 1e-12, "nv=%d" % nv, floor)
 
 
+@pytest.mark.parametrize("tune", ["1,0,0,0,1,4,0", "1,0,0,0,2,2,0", "0,0,0,0,0,4,0", "1,3,5,7,0,4,2"])
+@pytest.mark.parametrize("nv", [32, 64, 8])
+def test_kernel_variants_one_step(tune, nv, monkeypatch):
+    """The launch variants THOR_B200_TUNE selects (TMA-staged column-solve kernel with 1 or 2 stages,
+    no zig-zag walk, odd prefetch distances) compute the same step as the default."""
+    monkeypatch.setenv("THOR_B200_TUNE", tune)
+    planet = dict(ti.EARTH)
+    g, G = _setup(3, nv, planet)
+    s = _random_state(G, planet, 7 + nv)
+    st = thor.State(g, *s)
+    st.step(1, 600.0, 4)
+    ref, floor = _noise_floor(G, s, 1, 600.0, 4)
+    _compare(st.get(), ref, 1e-12, "tune=%s nv=%d" % (tune, nv), floor)
+
+
 def test_config0_parity_1_and_10_steps_and_mass():
     cfg = ti.CONFIGS[0]
     g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
