@@ -212,6 +212,25 @@ def run_cuda(args):
             b.record(stream)
             torch.cuda.synchronize()
             return a.elapsed_time(b) / reps
+        # config 1: the two stencils alone (Eq. 6, Eq. 7) on device arrays of this grid, 32 B/cell + geometry
+        nc = N * nv
+        bufs = [torch.rand(nc, dtype=torch.float64, device="cuda") for _ in range(7)]
+        ptr = [b.data_ptr() for b in bufs]
+
+        def time_op(fn, reps=40):
+            for _ in range(3):
+                fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record(stream)
+            for _ in range(reps):
+                fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        div_ms = time_op(lambda: thor.thor_apply_div_device(grid.handle, ptr[0], ptr[1], ptr[2], ptr[3], stream.cuda_stream))
+        grad_ms = time_op(lambda: thor.thor_apply_grad_device(grid.handle, ptr[0], ptr[4], ptr[5], ptr[6], stream.cuda_stream))
+        del bufs
         k2_ms = time_kernels(2)
         k1_ms = time_kernels(1)
         sub_ms = time_kernels(3)
@@ -276,7 +295,10 @@ def run_cuda(args):
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
-            "gpu_launches": int(launches), "roofline": roofline}
+            "gpu_launches": int(launches), "roofline": roofline,
+            "operators": {"what": "config 1 stencils alone on this grid (level 6 x 32), device arrays, 32 B/cell + geometry",
+                          "div_ms": div_ms, "div_GBs": (cells * 32 + N * 224) / (div_ms * 1e-3) / 1e9,
+                          "grad_ms": grad_ms, "grad_GBs": (cells * 32 + N * 176) / (grad_ms * 1e-3) / 1e9}}
     if world == 1 and not args.no_cpu_baseline:
         v, per, cores, sample = time_oracle(5, 4, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}

@@ -105,6 +105,27 @@ def test_config1_operators_match_oracle_and_closed_form(level):
     assert np.all(g.apply_grad(np.full((G.N, nv), 7.25)) == 0.0)
 
 
+def test_config1_operator_sweep_levels_5_6_7_second_order():
+    """Config 1 of BASELINE.json on the GPU: parity with the oracle at every level and the observed
+    order of the l2 error (Eq. 17) against the analytic result, levels 5 -> 6 -> 7 (pins P5/P8)."""
+    nv = 32
+    l2 = {}
+    for level in (5, 6, 7):
+        g, G = _setup(level, nv, ti.EARTH)
+        f = ti.harmonic_test_fields(G.xyz, ti.EARTH, nv, seed=ti.SEED0 + 1)
+        div, grad = g.apply_div(f["v"]), g.apply_grad(f["s"])
+        assert _rel(div, G.hdiv(f["v"])) <= 1e-12
+        assert _rel(grad, G.hgrad(f["s"])) <= 1e-12
+        w = G.Ac[:, None] / G.Ac.sum()
+        l2[level] = (np.sqrt((w * (div - f["div_exact"]) ** 2).sum() / (w * f["div_exact"] ** 2).sum()),
+                     np.sqrt((w[..., None] * (grad - f["grad_exact"]) ** 2).sum() / (w[..., None] * f["grad_exact"] ** 2).sum()))
+        _CACHE.pop((level, nv, tuple(sorted(ti.EARTH.items()))), None)
+    for k in (0, 1):
+        o56, o67 = np.log2(l2[5][k] / l2[6][k]), np.log2(l2[6][k] / l2[7][k])
+        print("operator %d: l2 %s, order 5->6 %.2f, 6->7 %.2f" % (k, [l2[l][k] for l in (5, 6, 7)], o56, o67))
+        assert o56 > 1.7 and o67 > 1.7
+
+
 @pytest.mark.parametrize("nv", [8, 16, 32, 64, 37, 5, 70, 128])
 def test_every_layer_shape_one_step(nv):
     """All lane-group shapes (G, E) incl. ragged layer counts, one large step with forcing."""
