@@ -80,6 +80,12 @@ struct thor_state {
     double *col_mass = nullptr, *col_energy = nullptr;
     bool stepped = false;
     int walk = 0;                    // direction of the last launch (0 ascending, 1 descending)
+    // one large step captured as a CUDA graph, per starting walk direction (replayed while the key holds)
+    struct GraphKey { double dt = 0; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
+    GraphKey gkey;
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    int gwalk_end[2] = {0, 0};
+    int gkernels = 0;
 };
 
 namespace {
@@ -223,11 +229,11 @@ int flat_blocks(size_t n) { return int((n + 255) / 256); }
 
 // L2 schedule of the two acoustic kernels; THOR_B200_TUNE="rev,k1_ahead,k2_ahead,tail"
 // overrides the defaults for measurement.
-struct TunePair { Tune k1, k2, ks; int zigzag, tma_stages, tma_ctas; };
+struct TunePair { Tune k1, k2, ks; int zigzag, tma_stages, tma_ctas, graph; };
 TunePair tune() {
-    int v[7] = {1, 0, 148, 148, 0, 4, 148};
+    int v[8] = {1, 0, 148, 148, 0, 4, 148, 1};
     if (const char* e = std::getenv("THOR_B200_TUNE"))
-        std::sscanf(e, "%d,%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5], &v[6]);
+        std::sscanf(e, "%d,%d,%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5], &v[6], &v[7]);
     TunePair p;
     p.zigzag = v[0];                 // 1: successive kernels walk the columns in alternating directions
     p.k1 = Tune{0, v[1], v[3]};      // k_momentum: look-ahead, tail hand-over
@@ -235,6 +241,7 @@ TunePair tune() {
     p.ks = Tune{0, v[6], 0};         // stage kernels and k_finish: look-ahead only
     p.tma_stages = v[4];      // 0: direct-load column-solve kernel; 1 or 2: TMA-staged, that many stages per block
     p.tma_ctas = v[5];        // persistent blocks per SM of the TMA-staged kernel
+    p.graph = v[7];           // 1: replay a large step as a CUDA graph (needs a non-default stream)
     return p;
 }
 
@@ -375,10 +382,13 @@ void thor_grid_destroy(thor_grid* grid) {
     delete grid;
 }
 
+static void drop_graphs(thor_state* s);
+
 void thor_state_destroy(thor_state* s) {
     if (!s) return;
     cudaFree(s->S); cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
     cudaFree(s->col_mass); cudaFree(s->col_energy);
+    drop_graphs(s);
     delete s;
 }
 
@@ -449,11 +459,37 @@ int thor_state_get(const thor_state* s, double* rho, double* mom_h, double* W, d
     return THOR_OK;
 }
 
+// the 2 (1 + n/2 + n) + 7 launches of one large step (Fig. 6), on the state's stream
+static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, const Forcing& F, double dt, int n) {
+    const int nv = g.nv, Npad = g.Npad;
+    cudaStream_t st = s->stream;
+    double* S = s->S;
+    // every launch walks the columns opposite to the one before it (L2 hand-over, DESIGN.md "L2 schedule")
+    auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
+    for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
+        const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
+        const double delta = stage == 1 ? dt / 3.0 : dt / n;
+        THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks));
+        THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks));
+        for (int sub = 0; sub < ns; ++sub) {
+            THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
+            TunePair t2 = tn;
+            t2.k2 = dir(tn.k2);
+            if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st)) return rc;
+        }
+    }
+    THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt, dir(tn.ks));
+    return THOR_OK;
+}
+
+static void drop_graphs(thor_state* s) {
+    for (cudaGraphExec_t& e : s->gexec)
+        if (e) { cudaGraphExecDestroy(e); e = nullptr; }
+}
+
 int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* forcing) {
     if (!s) return fail(THOR_EINVAL, "thor_step: null state");
     if (n_large < 0 || !(dt > 0) || n < 2 || (n & 1)) return fail(THOR_EINVAL, "thor_step: need n_large >= 0, dt > 0, even n >= 2");
-    const HostGrid& h = s->grid->h;
-    const int nv = h.nv, Npad = s->grid->d.Npad;
     cudaStream_t st = s->stream;
     if (forcing && !forcing->resident) {
         int rc;
@@ -468,23 +504,45 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     F.k_v = (forcing && s->has_kv) ? s->tab_kv : nullptr;
     const Geom g = make_geom(s->grid);
     const TunePair tn = tune();
-    double* S = s->S;
-    // every launch walks the columns opposite to the one before it (L2 hand-over, DESIGN.md "L2 schedule")
-    auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
-    for (int step = 0; step < n_large; ++step) {
-        for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
-            const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
-            const double delta = stage == 1 ? dt / 3.0 : dt / n;
-            THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks));
-            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks));
-            for (int sub = 0; sub < ns; ++sub) {
-                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
-                TunePair t2 = tn;
-                t2.k2 = dir(tn.k2);
-                if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st)) return rc;
-            }
+    // CUDA graph of one large step: after a first directly launched step (which does every lazy
+    // set-up), capture the launch sequence once per starting walk direction and replay it.  Small
+    // grids are launch-bound (config 0: 33 launches of a few microseconds each).
+    const bool use_graph = tn.graph && st != nullptr && s->stepped;
+    if (use_graph) {
+        thor_state::GraphKey key;
+        std::memset(&key, 0, sizeof(key));
+        key.dt = dt; key.n = n; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
+        if (const char* e = std::getenv("THOR_B200_TUNE")) std::strncpy(key.tune, e, sizeof(key.tune) - 1);
+        if (std::memcmp(&key, &s->gkey, sizeof(key)) != 0) {
+            drop_graphs(s);
+            std::memcpy(&s->gkey, &key, sizeof(key));
         }
-        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt, dir(tn.ks));
+    }
+    for (int step = 0; step < n_large; ++step) {
+        if (!use_graph) {
+            if (int rc = launch_large_step(s, g, tn, F, dt, n)) return rc;
+            continue;
+        }
+        const int w0 = s->walk & 1;
+        if (!s->gexec[w0]) {
+            const long long l0 = g_launches.load();
+            cudaGraph_t graph = nullptr;
+            CU(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int rc = launch_large_step(s, g, tn, F, dt, n);
+            const cudaError_t e = cudaStreamEndCapture(st, &graph);
+            s->gwalk_end[w0] = s->walk;
+            s->walk = w0;                                   // nothing ran yet
+            s->gkernels = int(g_launches.load() - l0);
+            g_launches.store(l0);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_step: graph capture: ") + cudaGetErrorString(e));
+            const cudaError_t ei = cudaGraphInstantiate(&s->gexec[w0], graph, 0);
+            cudaGraphDestroy(graph);
+            if (ei != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_step: graph instantiate: ") + cudaGetErrorString(ei));
+        }
+        CU(cudaGraphLaunch(s->gexec[w0], st));
+        s->walk = s->gwalk_end[w0];
+        g_launches.fetch_add(s->gkernels, std::memory_order_relaxed);
     }
     CU(cudaGetLastError());
     s->stepped = s->stepped || n_large > 0;

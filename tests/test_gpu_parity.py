@@ -156,6 +156,29 @@ def test_kernel_variants_one_step(tune, nv, monkeypatch):
     _compare(st.get(), ref, 1e-12, "tune=%s nv=%d" % (tune, nv), floor)
 
 
+def test_graph_replay_is_bit_identical_to_direct_launches():
+    """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
+    launched step); the state must be bit-identical to direct launches on the default stream."""
+    import torch
+    cfg = ti.CONFIGS[0]
+    g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
+    s = ti.initial_state(0, G.xyz)
+    a = thor.State(g, *s)                                     # default stream: direct launches
+    stream = torch.cuda.Stream()
+    b = thor.State(g, *s, cuda_stream=stream.cuda_stream)     # graph from the second step on
+    n0 = thor.thor_launch_count()
+    for _ in range(5):
+        a.step(1, cfg["dt"], cfg["n_sub"])
+    n1 = thor.thor_launch_count()
+    for _ in range(3):
+        b.step(1, cfg["dt"], cfg["n_sub"])
+    b.step(2, cfg["dt"], cfg["n_sub"])
+    n2 = thor.thor_launch_count()
+    assert n2 - n1 == n1 - n0                                 # replayed kernels are counted like launched ones
+    for x, y in zip(a.get(), b.get()):
+        assert np.array_equal(x, y)
+
+
 def test_config0_parity_1_and_10_steps_and_mass():
     cfg = ti.CONFIGS[0]
     g, G = _setup(cfg["level"], cfg["nv"], cfg["planet"])
