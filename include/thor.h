@@ -24,6 +24,10 @@
  *  - Layers are uniform in altitude: dz = z_top / n_layers, centre k at (k+1/2) dz (R6).
  *  - thor_step and thor_acoustic_substeps are asynchronous on the stream given to thor_state_init;
  *    thor_state_get, thor_state_set and thor_diagnostics synchronise that stream.
+ *  - On a non-default stream thor_step replays a large step as a CUDA graph after the first directly
+ *    launched one (same kernels, same results).  The environment variable THOR_B200_TUNE
+ *    ("zigzag,k1_ahead,k2_ahead,tail,tma_stages,tma_ctas,stage_ahead,graph")
+ *    overrides the launch schedule for measurement; it never changes what is computed.
  *  - The library never falls back to the CPU: without a usable CUDA device every device entry
  *    point returns THOR_ECUDA.  thor_grid_create / thor_grid_get are host-only and need no GPU.
  */
