@@ -9,6 +9,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <cstdint>
+#include <initializer_list>
 #include <new>
 #include <string>
 #include <vector>
@@ -226,6 +228,25 @@ Geom make_geom(const thor_grid* grid) {
     } while (0)
 
 int flat_blocks(size_t n) { return int((n + 255) / 256); }
+
+// fast path of the config-1 operators: even layer count <= 64 and 16-byte aligned arrays
+bool op_fast_path(int nv, std::initializer_list<const void*> ptrs) {
+    if ((nv & 1) || nv > 64) return false;
+    for (const void* p : ptrs)
+        if (reinterpret_cast<uintptr_t>(p) & 15u) return false;
+    return true;
+}
+#define THOR_DISPATCH_OP2(KERNEL, nv, N, stream, ...)                                              \
+    do {                                                                                           \
+        const int G_ = (nv) <= 8 ? 4 : ((nv) <= 16 ? 8 : ((nv) <= 32 ? 16 : 32));                  \
+        const int cpb_ = kWarpsPerBlock * (32 / G_);                                               \
+        const dim3 grid_(((N) + cpb_ - 1) / cpb_), block_(kWarpsPerBlock * 32);                    \
+        if (G_ == 4) KERNEL<4><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                         \
+        else if (G_ == 8) KERNEL<8><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                    \
+        else if (G_ == 16) KERNEL<16><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                  \
+        else KERNEL<32><<<grid_, block_, 0, stream>>>(__VA_ARGS__);                                \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                                        \
+    } while (0)
 
 // L2 schedule of the two acoustic kernels; THOR_B200_TUNE="rev,k1_ahead,k2_ahead,tail"
 // overrides the defaults for measurement.
@@ -601,7 +622,8 @@ int thor_apply_div_device(const thor_grid* grid, const double* vx, const double*
     if (rc) return rc;
     const Geom g = make_geom(grid);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    THOR_DISPATCH_OP(k_div, g.nv, g.N, st, g, vx, vy, vz, out);
+    if (op_fast_path(g.nv, {vx, vy, vz, out})) THOR_DISPATCH_OP2(k_div2, g.nv, g.N, st, g, vx, vy, vz, out);
+    else THOR_DISPATCH_OP(k_div, g.nv, g.N, st, g, vx, vy, vz, out);
     CU(cudaGetLastError());
     return THOR_OK;
 }
@@ -613,7 +635,8 @@ int thor_apply_grad_device(const thor_grid* grid, const double* sfield, double* 
     if (rc) return rc;
     const Geom g = make_geom(grid);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    THOR_DISPATCH_OP(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
+    if (op_fast_path(g.nv, {sfield, gx, gy, gz})) THOR_DISPATCH_OP2(k_grad2, g.nv, g.N, st, g, sfield, gx, gy, gz);
+    else THOR_DISPATCH_OP(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
     CU(cudaGetLastError());
     return THOR_OK;
 }

@@ -328,6 +328,71 @@ k_grad(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* __
     }
 }
 
+// The same two operators for even layer counts <= 64: two consecutive layers per lane (128-bit
+// accesses), G = 4..32 lanes per column, weights staged in shared memory -- the fast path of config 1.
+template <int G>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_div2(Geom g, const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+       double* __restrict__ out) {
+    const int lane = threadIdx.x & 31, warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int c0 = warp * (32 / G) + lane / G, gl = lane & (G - 1), k0 = 2 * gl, nv = g.nv;
+    const bool live = c0 < g.N;
+    const int col = live ? c0 : g.N - 1;
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][24];
+    double* w = wsm[threadIdx.x / G];
+    stage_weights<G>(g.wdiv + size_t(col) * 24, w, 12, gl);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    const int nb[7] = {col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    __syncwarp();
+    if (k0 >= nv) return;
+    double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+        const size_t o = size_t(nb[j]) * nv + k0;
+        const double2 x = __ldg(reinterpret_cast<const double2*>(vx + o)), y = __ldg(reinterpret_cast<const double2*>(vy + o)),
+                      z = __ldg(reinterpret_cast<const double2*>(vz + o));
+        const double wx = w[3 * j], wy = w[3 * j + 1], wz = w[3 * j + 2];
+        acc.x = fma(wx, x.x, fma(wy, y.x, fma(wz, z.x, acc.x)));
+        acc.y = fma(wx, x.y, fma(wy, y.y, fma(wz, z.y, acc.y)));
+    }
+    const double2 ri = __ldg(reinterpret_cast<const double2*>(g.rinv + k0));
+    if (live) *reinterpret_cast<double2*>(out + size_t(col) * nv + k0) = make_double2(acc.x * ri.x, acc.y * ri.y);
+}
+
+template <int G>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_grad2(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* __restrict__ gy, double* __restrict__ gz) {
+    const int lane = threadIdx.x & 31, warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int c0 = warp * (32 / G) + lane / G, gl = lane & (G - 1), k0 = 2 * gl, nv = g.nv;
+    const bool live = c0 < g.N;
+    const int col = live ? c0 : g.N - 1;
+    __shared__ double wsm[kWarpsPerBlock * 32 / G][18];
+    double* w = wsm[threadIdx.x / G];
+    stage_weights<G>(g.wgrad + size_t(col) * 18, w, 9, gl);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    __syncwarp();
+    if (k0 >= nv) return;
+    const double2 s0 = __ldg(reinterpret_cast<const double2*>(s + size_t(col) * nv + k0));
+    double2 ax = make_double2(0.0, 0.0), ay = ax, az = ax;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const double2 sj = __ldg(reinterpret_cast<const double2*>(s + size_t(nb[j]) * nv + k0));
+        const double d0 = sj.x - s0.x, d1 = sj.y - s0.y;
+        ax.x = fma(w[3 * j], d0, ax.x); ay.x = fma(w[3 * j + 1], d0, ay.x); az.x = fma(w[3 * j + 2], d0, az.x);
+        ax.y = fma(w[3 * j], d1, ax.y); ay.y = fma(w[3 * j + 1], d1, ay.y); az.y = fma(w[3 * j + 2], d1, az.y);
+    }
+    const double2 ri = __ldg(reinterpret_cast<const double2*>(g.rinv + k0));
+    if (live) {
+        const size_t o = size_t(col) * nv + k0;
+        *reinterpret_cast<double2*>(gx + o) = make_double2(ax.x * ri.x, ax.y * ri.y);
+        *reinterpret_cast<double2*>(gy + o) = make_double2(ay.x * ri.x, ay.y * ri.y);
+        *reinterpret_cast<double2*>(gz + o) = make_double2(az.x * ri.x, az.y * ri.y);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // S1: stage preparation (column-local).  Fig. 6 large-step 4 of the previous stage and
 // large-step 1 of this one:  Phi^[t] <- Phi^n (stage 1) or Phi^[t] + Phi* (stages 2, 3);
@@ -420,23 +485,57 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
         ta[e] = -ck * (dlob[e] * hhb[e] + 0.5 * gtb[e]) + cg * dlob[e];
         tb[e] = 1.0 + ck * hh[e] * (dlo[e] + dhib[e]) - cg * (dhib[e] - dlo[e]);
     }
-    // Thomas forward elimination of the matrix (L339): c'_k = c_k/(b_k - a_k c'_(k-1)), serial over the
-    // interfaces.  Lane by lane: in phase l every lane runs its own E steps from the carry it holds,
-    // only lane l's carry-in is the true c'_(k0-1); its carry-out is then handed to the whole group.
-    // fi = 1/b'_k, fa = a_k/b'_k, fc = c'_k; all three stay 0 on the ground, on pads and in pad columns.
+    // Thomas forward elimination of the matrix (L339): b'_k = b_k - a_k c_(k-1)/b'_(k-1).  The leading
+    // minors theta_k = b'_1 ... b'_k obey the LINEAR recurrence theta_k = b_k theta_(k-1) - a_k c_(k-1) theta_(k-2),
+    // so the pivots come out of a scan of 2x2 matrices instead of a serial chain of divisions.  Scaled
+    // by s_k = 1/b_k (t_k = theta_k s_1...s_k stays in (0, 1] for these diagonally dominant matrices, no
+    // overflow at 128 layers):  t_k = t_(k-1) - beta_k t_(k-2),  beta_k = a_k s_k c_(k-1) s_(k-1),
+    // 1/b'_k = s_k t_(k-1)/t_k.  fi = 1/b'_k, fa = a_k/b'_k, fc = c_k/b'_k; 0 on the ground, on pads and
+    // in pad columns (identity maps in the scan).
     double fa[E], fi[E], fc[E];
-    double carry = 0.0;
-    for (int l = 0; l < G; ++l) {
-        double cp = carry;
+    {
+        bool in[E];
+        double sk[E], cs[E], csb[E], beta[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int k = L.k0 + e;
-            const bool in = k >= 1 && k < nv && L.col < g.N;
-            const double inv = 1.0 / (tb[e] - ta[e] * cp);
-            cp = in ? tc[e] * inv : 0.0;
-            if (L.gl == l) { fi[e] = in ? inv : 0.0; fa[e] = in ? ta[e] * inv : 0.0; fc[e] = cp; }
+            in[e] = k >= 1 && k < nv && L.col < g.N;
+            sk[e] = in[e] ? 1.0 / tb[e] : 0.0;
+            cs[e] = in[e] ? tc[e] * sk[e] : 0.0;
         }
-        carry = __shfl_sync(kFull, cp, l, G);
+        below<G, E>(cs, csb, L.gl, 0.0);
+        double p00 = 1.0, p01 = 0.0, p10 = 0.0, p11 = 1.0;      // product of this lane's maps [[1, -beta], [1, 0]]
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            beta[e] = in[e] ? ta[e] * sk[e] * csb[e] : 0.0;
+            if (in[e]) {
+                const double n00 = fma(-beta[e], p10, p00), n01 = fma(-beta[e], p11, p01);
+                p10 = p00; p11 = p01; p00 = n00; p01 = n01;
+            }
+        }
+#pragma unroll
+        for (int sft = 1; sft < G; sft <<= 1) {                   // Kogge-Stone: P_lane <- P_lane x P_(lane - sft)
+            const double o00 = __shfl_up_sync(kFull, p00, sft, G), o01 = __shfl_up_sync(kFull, p01, sft, G);
+            const double o10 = __shfl_up_sync(kFull, p10, sft, G), o11 = __shfl_up_sync(kFull, p11, sft, G);
+            if (L.gl >= sft) {
+                const double r00 = fma(p00, o00, p01 * o10), r01 = fma(p00, o01, p01 * o11);
+                const double r10 = fma(p10, o00, p11 * o10), r11 = fma(p10, o01, p11 * o11);
+                p00 = r00; p01 = r01; p10 = r10; p11 = r11;
+            }
+        }
+        double t1 = __shfl_up_sync(kFull, p00, 1, G), t2 = __shfl_up_sync(kFull, p10, 1, G);   // t_(k0-1), t_(k0-2)
+        if (L.gl == 0) { t1 = 1.0; t2 = 0.0; }
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            fi[e] = 0.0;
+            if (in[e]) {
+                const double t0 = fma(-beta[e], t2, t1);
+                fi[e] = sk[e] * t1 / t0;
+                t2 = t1; t1 = t0;
+            }
+            fa[e] = ta[e] * fi[e];
+            fc[e] = tc[e] * fi[e];
+        }
     }
     st_row<E>(me + F_RHOT * NVP, rho); st_row<E>(me + F_VXT * NVP, Vx); st_row<E>(me + F_VYT * NVP, Vy);
     st_row<E>(me + F_VZT * NVP, Vz);   st_row<E>(me + F_WT * NVP, W);   st_row<E>(me + F_PT * NVP, p);

@@ -156,6 +156,55 @@ def test_kernel_variants_one_step(tune, nv, monkeypatch):
     _compare(st.get(), ref, 1e-12, "tune=%s nv=%d" % (tune, nv), floor)
 
 
+@pytest.mark.parametrize("level,nv,n_sub", [(0, 2, 2), (0, 8, 4), (1, 2, 2), (1, 3, 6), (2, 128, 2)])
+def test_degenerate_grids_and_layer_counts(level, nv, n_sub):
+    """The smallest grids (12 and 42 columns: every column touches a pentagon), the smallest layer
+    count (2: one interior interface, a 1x1 'tridiagonal' system), the largest (128) and n = 2."""
+    planet = dict(ti.EARTH)
+    planet["z_top"] = min(36.0e3, 4.0e3 * nv)          # keep g dz/(2 Rd T) < 1: the discrete hydrostatic column stays positive
+    g, G = _setup(level, nv, planet)
+    assert g.n_cols == ti.n_columns(level)
+    s = _random_state(G, planet, 1000 + 10 * level + nv, vel=1.0, wamp=0.1)
+    st = thor.State(g, *s)
+    m0, _ = st.diagnostics()
+    st.step(2, 300.0, n_sub)
+    ref, floor = _noise_floor(G, s, 2, 300.0, n_sub)
+    _compare(st.get(), ref, 1e-12, "level=%d nv=%d n=%d" % (level, nv, n_sub), floor, K=8.0)
+    m1, _ = st.diagnostics()
+    assert abs(m1 - m0) <= 1e-13 * m0
+    f = ti.harmonic_test_fields(G.xyz, planet, nv, seed=5, lmax=2)
+    assert _rel(g.apply_div(f["v"]), G.hdiv(f["v"])) <= 1e-12
+    assert _rel(g.apply_grad(f["s"]), G.hgrad(f["s"])) <= 1e-12
+
+
+def test_step_argument_errors_leave_the_state_untouched_and_set_restarts_it():
+    import torch
+    cfg = ti.CONFIGS[0]
+    g, G = _setup(3, cfg["nv"], cfg["planet"])
+    s = _random_state(G, cfg["planet"], 77)
+    stream = torch.cuda.Stream()
+    st = thor.State(g, *s, cuda_stream=stream.cuda_stream)
+    for bad in (dict(n_large=1, dt=-1.0, n=4), dict(n_large=1, dt=600.0, n=3), dict(n_large=1, dt=600.0, n=0),
+                dict(n_large=-1, dt=600.0, n=4)):
+        with pytest.raises(thor.ThorError) as e:
+            st.step(bad["n_large"], bad["dt"], bad["n"])
+        assert e.value.code == thor.THOR_EINVAL
+    st.step(0, 600.0, 4)                                       # zero steps: nothing happens
+    for a, b in zip(st.get(), s):
+        assert np.array_equal(a, b)
+    st.step(3, 600.0, 4)                                       # direct, then graph replays
+    first = [a.copy() for a in st.get()]
+    st.set(*s)                                                 # restart on the same handle (graph is reused)
+    st.step(3, 600.0, 4)
+    for a, b in zip(st.get(), first):
+        assert np.array_equal(a, b)
+    F = dict(T_eq=np.full(s[0].shape, 250.0), k_T=np.full(s[0].shape, 1e-4), k_v=np.full(s[0].shape, 1e-4))
+    m0, e0 = st.diagnostics()
+    st.step(2, 600.0, 4, F)                                    # forcing switches the graph key
+    m1, e1 = st.diagnostics()
+    assert abs(m1 - m0) <= 1e-13 * m0 and e1 != e0             # physics does not touch mass (L200)
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""
