@@ -230,6 +230,7 @@ def run_cuda(args):
             return a.elapsed_time(b) / reps
         div_ms = time_op(lambda: thor.thor_apply_div_device(grid.handle, ptr[0], ptr[1], ptr[2], ptr[3], stream.cuda_stream))
         grad_ms = time_op(lambda: thor.thor_apply_grad_device(grid.handle, ptr[0], ptr[4], ptr[5], ptr[6], stream.cuda_stream))
+        lap_ms = time_op(lambda: thor.thor_apply_lap_device(grid.handle, ptr[0], ptr[3], stream.cuda_stream))
         del bufs
         k2_ms = time_kernels(2)
         k1_ms = time_kernels(1)
@@ -298,7 +299,9 @@ def run_cuda(args):
             "gpu_launches": int(launches), "roofline": roofline,
             "operators": {"what": "config 1 stencils alone on this grid (level 6 x 32), device arrays, 32 B/cell + geometry",
                           "div_ms": div_ms, "div_GBs": (cells * 32 + N * 224) / (div_ms * 1e-3) / 1e9,
-                          "grad_ms": grad_ms, "grad_GBs": (cells * 32 + N * 176) / (grad_ms * 1e-3) / 1e9}}
+                          "grad_ms": grad_ms, "grad_GBs": (cells * 32 + N * 176) / (grad_ms * 1e-3) / 1e9,
+                          "lap_ms": lap_ms, "lap_GBs": (cells * 16 + N * 96) / (lap_ms * 1e-3) / 1e9,
+                          "lap_what": "horizontal Laplacian of L369-L371 (NEXT-1 building block), 16 B/cell + geometry"}}
     if world == 1 and not args.no_cpu_baseline:
         v, per, cores, sample = time_oracle(5, 4, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}

@@ -125,6 +125,14 @@ int thor_apply_div_device(const thor_grid *grid, const double *vx, const double 
 int thor_apply_grad_device(const thor_grid *grid, const double *s, double *gx, double *gy, double *gz,
                            void *cuda_stream);
 
+/* Horizontal Laplacian of L369-L371 (the building block of the paper's fourth-order hyper-diffusion,
+ * Eq. 43-48): the Eq. 7 gradient on the primary (triangle) grid, which places a vector at every
+ * control-volume corner, then Eq. 6 over the control volume; at radius r_k (unit-sphere operator
+ * / r_k^2).  s, out: [n_cols][n_layers]; host arrays in canonical order, or DEVICE arrays in device
+ * column order for the _device variant (asynchronous on cuda_stream). */
+int thor_apply_lap(const thor_grid *grid, const double *s, double *out);
+int thor_apply_lap_device(const thor_grid *grid, const double *s, double *out, void *cuda_stream);
+
 /* Number of kernels this library has launched in the calling process so far. */
 long long thor_launch_count(void);
 

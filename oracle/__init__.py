@@ -55,6 +55,12 @@ def _load():
         L.orc_geom_deg.argtypes = [ctypes.c_void_p]
         L.orc_hdiv.argtypes = [ctypes.c_void_p, _D, _D]
         L.orc_hgrad.argtypes = [ctypes.c_void_p, _D, _D]
+        L.orc_hlap.argtypes = [ctypes.c_void_p, _D, _D]
+        for name, nargs in (("orc_dbar", None), ("orc_kd", None), ("orc_tau_d", None)):
+            getattr(L, name).restype = ctypes.c_double
+        L.orc_dbar.argtypes = [ctypes.c_double, ctypes.c_int]
+        L.orc_kd.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.orc_tau_d.argtypes = [ctypes.c_double, ctypes.c_double]
         L.orc_thomas.argtypes = [ctypes.c_int, _D, _D, _D, _D, _D]
         L.orc_centroid_eq13.argtypes = [_D, ctypes.c_int, _D]
         L.orc_step.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D]
@@ -132,6 +138,14 @@ class Geometry:
         _load().orc_hgrad(self._h, _p(s), _p(out))
         return out
 
+    # L369-L371: horizontal Laplacian (gradient on the triangles, then Eq. 6) of s [N][nv] at radius r_k
+    def hlap(self, s):
+        s = _c(s)
+        assert s.shape == (self.N, self.nv)
+        out = np.empty((self.N, self.nv))
+        _load().orc_hlap(self._h, _p(s), _p(out))
+        return out
+
     def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None):
         """n_large large steps; returns new (rho, V, W, p); inputs are not modified."""
         rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
@@ -196,3 +210,16 @@ def centroid_eq13(r):
     out = np.zeros(3)
     _load().orc_centroid_eq13(_p(r), int(r.shape[0]), _p(out))
     return out
+
+
+# Eq. 2, 49, 50 (L55, L373-L381)
+def dbar(radius, level):
+    return float(_load().orc_dbar(float(radius), int(level)))
+
+
+def kd(D, dbar_, dt):
+    return float(_load().orc_kd(float(D), float(dbar_), float(dt)))
+
+
+def tau_d(dbar_, kd_):
+    return float(_load().orc_tau_d(float(dbar_), float(kd_)))

@@ -43,6 +43,11 @@ typedef struct {
     double *nrm;  /* [N][6][3] outward unit normal of that arc (L67) */
     double *bary; /* [N][6][3] Eq. 5 weights of (Phi_0, Phi_k, Phi_k+1) at corner k: A2,A3,A1 / sum */
     double *Ac;   /* [N] control-volume area (Eq. 6) */
+    /* Eq. 7 on the primary (triangle) grid, for the Laplacian of L369-L371: per corner k the triangle's
+     * vertices in canonical order and its three edge vectors l_e n_e/(2 A_T), the centre weights */
+    int *tv;      /* [N][6][3]    triangle vertices a, b, c (smallest index first, counter-clockwise) */
+    double *tE;   /* [N][6][3][3] E_ab, E_bc, E_ca */
+    double *tbw;  /* [N][6][2]    Eq. 5 weights of b and c at the centre C_k */
 } orc_geom;
 
 static void cross3(const double *a, const double *b, double *c) {
@@ -88,6 +93,7 @@ void orc_geom_free(orc_geom *G) {
     if (!G) return;
     free(G->r_c); free(G->r_h); free(G->z_c); free(G->xyz); free(G->nbr); free(G->deg);
     free(G->C); free(G->len); free(G->nrm); free(G->bary); free(G->Ac);
+    free(G->tv); free(G->tE); free(G->tbw);
     free(G);
 }
 
@@ -115,6 +121,9 @@ orc_geom *orc_geom_build(int N, int nv, const orc_planet *P, const double *xyz, 
     G->nrm = (double *)calloc((size_t)N * 18, sizeof(double));
     G->bary = (double *)calloc((size_t)N * 18, sizeof(double));
     G->Ac = (double *)calloc((size_t)N, sizeof(double));
+    G->tv = (int *)calloc((size_t)N * 18, sizeof(int));
+    G->tE = (double *)calloc((size_t)N * 54, sizeof(double));
+    G->tbw = (double *)calloc((size_t)N * 12, sizeof(double));
     for (int i = 0; i < N; i++) {
         int m = 6;
         if (nbr[6 * i + 5] < 0) m = 5;
@@ -151,6 +160,23 @@ orc_geom *orc_geom_build(int N, int nv, const orc_planet *P, const double *xyz, 
             B[0] = wa[(3 - rot) % 3] / ws;       /* A2/sum: weight of P_0   */
             B[1] = wa[(4 - rot) % 3] / ws;       /* A3/sum: weight of P_k   */
             B[2] = wa[(5 - rot) % 3] / ws;       /* A1/sum: weight of P_k+1 */
+            /* triangle-grid gradient (Eq. 7 applied to the triangle a, b, c; L369): edge e between two
+             * vertices: geodesic arc l_e, outward normal n_e; E_e = l_e n_e / (2 A_T) */
+            {
+                int *tv = G->tv + 18 * (size_t)i + 3 * k;
+                double *tE = G->tE + 54 * (size_t)i + 9 * k, *tbw = G->tbw + 12 * (size_t)i + 2 * k;
+                tv[0] = c0; tv[1] = c1; tv[2] = c2;
+                double AT = tri_area(tri + 0, tri + 3, tri + 6);
+                for (int e = 0; e < 3; e++) {
+                    const double *x = tri + 3 * e, *y = tri + 3 * ((e + 1) % 3);
+                    double n[3];
+                    cross3(x, y, n);
+                    double ln = norm3(n), l = arc3(x, y);
+                    for (int d = 0; d < 3; d++) tE[3 * e + d] = l * (-n[d] / ln) / (2.0 * AT);
+                }
+                tbw[0] = wa[1] / ws;
+                tbw[1] = wa[2] / ws;
+            }
         }
         double area = 0.0;
         for (int k = 0; k < m; k++) {
@@ -258,6 +284,52 @@ void orc_hgrad(const orc_geom *G, const double *s, double *out) {
         free(ds);
     }
 }
+
+/* Horizontal Laplacian of L369-L371 (NEXT-1 of SURVEY 8(f)): "we first compute the gradient using
+ * Eq. (7) in the primary grid (triangles), which place the calculated vectors at the corners of the
+ * control volume ... Then using these vectors we apply Eq. 6 to the control volume."
+ *   corner k:  G_k = sum_e E_e ((s_e1 - s_m) + (s_e2 - s_m)),  s_m = Eq. 5 value at the centre C_k
+ *              (difference form relative to vertex a, so that a constant gives exactly zero and
+ *               the three columns sharing the triangle obtain the bit-identical vector)
+ *   column:    lap_0 = (1/A_c) sum_k l_k (G_k + G_k+1)/2 . n_k,  times 1/r_k^2 at radius r_k.
+ * s, out: [N][nv]. */
+void orc_hlap(const orc_geom *G, const double *s, double *out) {
+    const int N = G->N, nv = G->nv;
+#pragma omp parallel
+    {
+        double *gk = (double *)malloc(sizeof(double) * 6 * 3);
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            int m = G->deg[i];
+            for (int lay = 0; lay < nv; lay++) {
+                for (int k = 0; k < m; k++) {
+                    const int *tv = G->tv + 18 * (size_t)i + 3 * k;
+                    const double *tE = G->tE + 54 * (size_t)i + 9 * k, *tbw = G->tbw + 12 * (size_t)i + 2 * k;
+                    double sa = s[(size_t)tv[0] * nv + lay];
+                    double db = s[(size_t)tv[1] * nv + lay] - sa, dc = s[(size_t)tv[2] * nv + lay] - sa;
+                    double ma = -(tbw[0] * db + tbw[1] * dc);       /* s_a - s_m */
+                    double mb = db + ma, mc = dc + ma;               /* s_b - s_m, s_c - s_m */
+                    for (int d = 0; d < 3; d++)
+                        gk[3 * k + d] = tE[0 + d] * (ma + mb) + tE[3 + d] * (mb + mc) + tE[6 + d] * (mc + ma);
+                }
+                double sum = 0.0;
+                for (int k = 0; k < m; k++) {
+                    const double *g0 = gk + 3 * k, *g1 = gk + 3 * ((k + 1) % m);
+                    const double *n = G->nrm + 18 * (size_t)i + 3 * k;
+                    double f = 0.5 * (g0[0] + g1[0]) * n[0] + 0.5 * (g0[1] + g1[1]) * n[1] + 0.5 * (g0[2] + g1[2]) * n[2];
+                    sum += G->len[6 * i + k] * f;
+                }
+                out[(size_t)i * nv + lay] = sum / G->Ac[i] / (G->r_c[lay] * G->r_c[lay]);
+            }
+        }
+        free(gk);
+    }
+}
+
+/* Eq. 49-50 (L373-L381): K_d = D dbar^4 / dt, tau_d = dbar^4 / (2^5 K_d); dbar from Eq. 2 (G13). */
+double orc_dbar(double radius, int level) { return sqrt(2.0 * 3.14159265358979323846 / 5.0) * radius / pow(2.0, level); }
+double orc_kd(double D, double dbar, double dt) { return D * dbar * dbar * dbar * dbar / dt; }
+double orc_tau_d(double dbar, double kd) { return dbar * dbar * dbar * dbar / (32.0 * kd); }
 
 /* ---------------------------------------------------------------------------------------------
  * Vertical operators (O3; Eq. 8-9 with k = 1, L88-L94; Eq. 27's radial part, L227).

@@ -60,6 +60,8 @@ _SIGNATURES = {
     "thor_apply_grad": (ctypes.c_int, [_V, _D, _D]),
     "thor_apply_div_device": (ctypes.c_int, [_V, _V, _V, _V, _V, _V]),
     "thor_apply_grad_device": (ctypes.c_int, [_V, _V, _V, _V, _V, _V]),
+    "thor_apply_lap": (ctypes.c_int, [_V, _D, _D]),
+    "thor_apply_lap_device": (ctypes.c_int, [_V, _V, _V, _V]),
     "thor_launch_count": (ctypes.c_longlong, []),
     "thor_last_error": (ctypes.c_char_p, []),
 }
@@ -176,6 +178,14 @@ def thor_apply_grad_device(grid, s, gx, gy, gz, cuda_stream=None):
     _check(load_library().thor_apply_grad_device(grid, _V(s), _V(gx), _V(gy), _V(gz), _V(cuda_stream or 0)))
 
 
+def thor_apply_lap(grid, s, out):
+    _check(load_library().thor_apply_lap(grid, _ptr(s), _ptr(out)))
+
+
+def thor_apply_lap_device(grid, s, out, cuda_stream=None):
+    _check(load_library().thor_apply_lap_device(grid, _V(s), _V(out), _V(cuda_stream or 0)))
+
+
 def thor_launch_count():
     return int(load_library().thor_launch_count())
 
@@ -208,6 +218,12 @@ class Grid:
         s = _f64(s, (self.n_cols, self.n_layers))
         out = np.empty((self.n_cols, self.n_layers, 3))
         thor_apply_grad(self._h, s, out)
+        return out
+
+    def apply_lap(self, s):
+        s = _f64(s, (self.n_cols, self.n_layers))
+        out = np.empty((self.n_cols, self.n_layers))
+        thor_apply_lap(self._h, s, out)
         return out
 
     def close(self):

@@ -273,6 +273,28 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
         bary[size_t(t) * 3 + 1] = wb / s;
         bary[size_t(t) * 3 + 2] = wc / s;
     }
+    // --- Eq. 7 on the primary grid (L369): gradient of a scalar on triangle t at its centre C_t as a
+    // combination of the three vertex values, G_t = sum_v gw[t][v] s_v with
+    //   G = sum_e E_e (s_e1 + s_e2 - 2 s_m),  E_e = l_e n_e / (2 A_T),  s_m = Eq. 5 value at C_t
+    std::vector<V3> gw(size_t(T) * 3);
+    for (int t = 0; t < T; ++t) {
+        const V3 v[3] = {pts[tris[t].a], pts[tris[t].b], pts[tris[t].c]};
+        const double AT = tri_area(v[0], v[1], v[2]);
+        V3 Ee[3], ES{0, 0, 0};
+        for (int e = 0; e < 3; ++e) {
+            const V3 x = v[e], y = v[(e + 1) % 3];
+            const V3 n = cross(x, y);
+            Ee[e] = (-arc(x, y) / (2.0 * AT * norm(n))) * n;          // outward for counter-clockwise order
+            ES = ES + Ee[e];
+        }
+        for (int q = 0; q < 3; ++q)                                     // vertex q sits on edges q-1 and q
+            gw[size_t(t) * 3 + q] = Ee[(q + 2) % 3] + Ee[q] - (2.0 * bary[size_t(t) * 3 + q]) * ES;
+    }
+    auto gw_of = [&](int t, int v) {
+        if (tris[t].a == v) return gw[size_t(t) * 3 + 0];
+        if (tris[t].b == v) return gw[size_t(t) * 3 + 1];
+        return gw[size_t(t) * 3 + 2];
+    };
     auto weight_of = [&](int t, int v) {
         if (tris[t].a == v) return bary[size_t(t) * 3 + 0];
         if (tris[t].b == v) return bary[size_t(t) * 3 + 1];
@@ -320,6 +342,7 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
     g.d_wdiv.assign(size_t(N) * 21, 0.0);
     g.d_wgrad.assign(size_t(N) * 18, 0.0);
     g.d_rhat.assign(size_t(N) * 3, 0.0);
+    g.d_wlap.assign(size_t(N) * 6, 0.0);
     g.d_area.assign(N, 0.0);
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < N; ++i) {
@@ -353,6 +376,19 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
             w[1 + (k + 1) % m] = w[1 + (k + 1) % m] + weight_of(t, nb) * E[k];
         }
         const int d = g.rank[i];
+        {   // Laplacian: Eq. 6 applied to the corner gradients, lap_i = sum_k (E_k / A_c) . G_k, kept in
+            // difference form (the coefficient of s_i is minus the sum of the others)
+            double wl[7] = {0, 0, 0, 0, 0, 0, 0};
+            for (int k = 0; k < m; ++k) {
+                const int t = corner_tri[size_t(i) * 6 + k];
+                const int na = nbr[size_t(i) * 6 + k], nb = nbr[size_t(i) * 6 + (k + 1) % m];
+                const V3 Ek = (1.0 / area) * E[k];
+                wl[0] += dot(Ek, gw_of(t, i));
+                wl[1 + k] += dot(Ek, gw_of(t, na));
+                wl[1 + (k + 1) % m] += dot(Ek, gw_of(t, nb));
+            }
+            for (int j = 0; j < 6; ++j) g.d_wlap[size_t(d) * 6 + j] = wl[1 + j];
+        }
         for (int j = 0; j < 7; ++j) {
             V3 wj = (1.0 / area) * w[j];
             g.d_wdiv[size_t(d) * 21 + 3 * j + 0] = wj.x;

@@ -26,6 +26,7 @@ struct HostGrid {
     std::vector<double> d_wdiv;    // [N][7][3] div_i = sum_j wdiv[j] . Phi_j   (j = 0 self, 1..6 neighbours)
     std::vector<double> d_wgrad;   // [N][6][3] grad_i = sum_j wgrad[j] (s_j - s_i), already tangent (Eq. 28)
     std::vector<double> d_rhat;    // [N][3]
+    std::vector<double> d_wlap;    // [N][6] lap_i = sum_j wlap[j] (s_j - s_i): gradient on the triangles, then Eq. 6 (L369-L371)
     // tangent-plane storage of the acoustic horizontal momentum: per-column orthonormal basis (e1, e2)
     // and the same two stencils contracted with it, so that V* = a e1 + b e2 moves as 2 rows, not 3
     std::vector<double> d_basis;   // [N][6]  e1(3), e2(3)

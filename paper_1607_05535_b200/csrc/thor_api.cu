@@ -46,7 +46,7 @@ struct DeviceGeom {
     int* nbr = nullptr;
     int* order = nullptr;
     double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
-    double *basis = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr;
+    double *basis = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr, *wlap = nullptr;
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr;
     // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
     int tcol = 0, hmax = 0;
@@ -114,13 +114,15 @@ int ensure_device_geom(const thor_grid* grid) {
     d.Npad = Npad;
     std::vector<int> nbr(size_t(Npad) * 8);
     std::vector<double> wdiv(size_t(Npad) * 24, 0.0), wgrad(size_t(Npad) * 18, 0.0), rhat(size_t(Npad) * 4, 0.0),
-        area(Npad, 0.0), basis(size_t(Npad) * 8, 0.0), wdiv2(size_t(Npad) * 16, 0.0), wgrad2(size_t(Npad) * 12, 0.0);
+        area(Npad, 0.0), basis(size_t(Npad) * 8, 0.0), wdiv2(size_t(Npad) * 16, 0.0), wgrad2(size_t(Npad) * 12, 0.0),
+        wlap(size_t(Npad) * 8, 0.0);
     for (int c = 0; c < Npad; ++c) {
         for (int k = 0; k < 8; ++k) nbr[size_t(c) * 8 + k] = (c < N && k < 6) ? h.d_nbr[size_t(c) * 6 + k] : c;
         if (c >= N) { rhat[size_t(c) * 4 + 2] = 1.0; basis[size_t(c) * 8] = 1.0; basis[size_t(c) * 8 + 4] = 1.0; continue; }
         std::copy_n(&h.d_basis[size_t(c) * 6], 6, &basis[size_t(c) * 8]);
         std::copy_n(&h.d_wdiv2[size_t(c) * 14], 14, &wdiv2[size_t(c) * 16]);
         std::copy_n(&h.d_wgrad2[size_t(c) * 12], 12, &wgrad2[size_t(c) * 12]);
+        std::copy_n(&h.d_wlap[size_t(c) * 6], 6, &wlap[size_t(c) * 8]);
         std::copy_n(&h.d_wdiv[size_t(c) * 21], 21, &wdiv[size_t(c) * 24]);
         std::copy_n(&h.d_wgrad[size_t(c) * 18], 18, &wgrad[size_t(c) * 18]);
         std::copy_n(&h.d_rhat[size_t(c) * 3], 3, &rhat[size_t(c) * 4]);
@@ -141,6 +143,7 @@ int ensure_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.basis, basis))) return rc;
     if ((rc = upload(&d.wdiv2, wdiv2))) return rc;
     if ((rc = upload(&d.wgrad2, wgrad2))) return rc;
+    if ((rc = upload(&d.wlap, wlap))) return rc;
     if ((rc = upload(&d.rinv, padded(h.rinv)))) return rc;
     if ((rc = upload(&d.dlo, padded(h.dlo)))) return rc;
     if ((rc = upload(&d.dhi, padded(h.dhi)))) return rc;
@@ -187,7 +190,7 @@ Geom make_geom(const thor_grid* grid) {
     Geom g;
     g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
     g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
-    g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2;
+    g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc;
     g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
@@ -398,7 +401,7 @@ void thor_grid_destroy(thor_grid* grid) {
     if (d.ready) {
         cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
         cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc);
-        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2);
+        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap);
     }
     delete grid;
 }
@@ -638,6 +641,45 @@ int thor_apply_grad_device(const thor_grid* grid, const double* sfield, double* 
     if (op_fast_path(g.nv, {sfield, gx, gy, gz})) THOR_DISPATCH_OP2(k_grad2, g.nv, g.N, st, g, sfield, gx, gy, gz);
     else THOR_DISPATCH_OP(k_grad, g.nv, g.N, st, g, sfield, gx, gy, gz);
     CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+int thor_apply_lap_device(const thor_grid* grid, const double* sfield, double* out, void* cuda_stream) {
+    if (!grid || !sfield || !out) return fail(THOR_EINVAL, "thor_apply_lap_device: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const Geom g = make_geom(grid);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (op_fast_path(g.nv, {sfield, out})) THOR_DISPATCH_OP2(k_lap2, g.nv, g.N, st, g, sfield, out);
+    else THOR_DISPATCH_OP(k_lap, g.nv, g.N, st, g, sfield, out);
+    CU(cudaGetLastError());
+    return THOR_OK;
+}
+
+int thor_apply_lap(const thor_grid* grid, const double* sfield, double* out) {
+    if (!grid || !sfield || !out) return fail(THOR_EINVAL, "thor_apply_lap: null argument");
+    int rc = ensure_device_geom(grid);
+    if (rc) return rc;
+    const HostGrid& h = grid->h;
+    const int N = h.N, nv = h.nv;
+    const size_t nc = size_t(N) * nv;
+    double* buf = nullptr;   // [staging][s][out]
+    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 3 * nc * sizeof(double)));
+    double *stg = buf, *sd = buf + nc, *od = sd + nc;
+    cudaError_t e = cudaMemcpy(stg, sfield, nc * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_gather_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, stg, nv, 1, 0, sd);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        rc = thor_apply_lap_device(grid, sd, od, nullptr);
+        if (rc == THOR_OK) {
+            k_scatter_rows<<<flat_blocks(nc), 256>>>(N, nv, grid->d.order, od, nv, 1, 0, stg);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            e = cudaMemcpy(out, stg, nc * sizeof(double), cudaMemcpyDeviceToHost);
+        }
+    }
+    cudaFree(buf);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_lap: ") + cudaGetErrorString(e));
     return THOR_OK;
 }
 

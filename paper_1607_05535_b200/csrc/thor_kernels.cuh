@@ -53,6 +53,7 @@ struct Geom {                 // device pointers, device column order, padded to
     const int* nbr;           // [Npad][8]   6 neighbours (pentagons, pad columns: self), 2 x self
     const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad
     const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)
+    const double* wlap;       // [Npad][8]   6 Laplacian weights (Eq. 7 on the triangles, then Eq. 6; L369-L371), 2 pad
     const double* rhat;       // [Npad][4]   unit vector of the column, 1 pad
     const double* basis;      // [Npad][8]   tangent basis e1(3), e2(3), 2 pad
     const double* wdiv2;      // [Npad][16]  7 x 2 divergence weights contracted with the basis of column j, 2 pad
@@ -328,6 +329,40 @@ k_grad(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* __
     }
 }
 
+// Horizontal Laplacian of L369-L371 at radius r_k (NEXT-1 building block): lap_i = sum_j wlap[j] (s_j - s_i) / r_k^2
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_lap(Geom g, const double* __restrict__ s, double* __restrict__ out) {
+    Lanes<G, E> L(g.N);
+    const int nv = g.nv;
+    const double* w = g.wlap + size_t(L.col) * 8;
+    double s0[E], acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = L.gl + e * G;
+        s0[e] = k < nv ? __ldg(s + size_t(L.col) * nv + k) : 0.0;
+        acc[e] = 0.0;
+    }
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const int c = __ldg(g.nbr + size_t(L.col) * 8 + j);
+        const double wj = __ldg(w + j);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int k = L.gl + e * G;
+            acc[e] = fma(wj, (k < nv ? __ldg(s + size_t(c) * nv + k) : 0.0) - s0[e], acc[e]);
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = L.gl + e * G;
+        if (L.live && k < nv) {
+            const double ri = __ldg(g.rinv + k);
+            out[size_t(L.col) * nv + k] = acc[e] * ri * ri;
+        }
+    }
+}
+
 // The same two operators for even layer counts <= 64: two consecutive layers per lane (128-bit
 // accesses), G = 4..32 lanes per column, weights staged in shared memory -- the fast path of config 1.
 template <int G>
@@ -391,6 +426,32 @@ k_grad2(Geom g, const double* __restrict__ s, double* __restrict__ gx, double* _
         *reinterpret_cast<double2*>(gy + o) = make_double2(ay.x * ri.x, ay.y * ri.y);
         *reinterpret_cast<double2*>(gz + o) = make_double2(az.x * ri.x, az.y * ri.y);
     }
+}
+
+template <int G>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_lap2(Geom g, const double* __restrict__ s, double* __restrict__ out) {
+    const int lane = threadIdx.x & 31, warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int c0 = warp * (32 / G) + lane / G, gl = lane & (G - 1), k0 = 2 * gl, nv = g.nv;
+    const bool live = c0 < g.N;
+    const int col = live ? c0 : g.N - 1;
+    if (k0 >= nv) return;
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    const double2* wp = reinterpret_cast<const double2*>(g.wlap + size_t(col) * 8);
+    const double2 w01 = __ldg(wp), w23 = __ldg(wp + 1), w45 = __ldg(wp + 2);
+    const double w[6] = {w01.x, w01.y, w23.x, w23.y, w45.x, w45.y};
+    const double2 s0 = __ldg(reinterpret_cast<const double2*>(s + size_t(col) * nv + k0));
+    double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const double2 sj = __ldg(reinterpret_cast<const double2*>(s + size_t(nb[j]) * nv + k0));
+        acc.x = fma(w[j], sj.x - s0.x, acc.x);
+        acc.y = fma(w[j], sj.y - s0.y, acc.y);
+    }
+    const double2 ri = __ldg(reinterpret_cast<const double2*>(g.rinv + k0));
+    if (live) *reinterpret_cast<double2*>(out + size_t(col) * nv + k0) = make_double2(acc.x * ri.x * ri.x, acc.y * ri.y * ri.y);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -126,6 +126,28 @@ def test_config1_operator_sweep_levels_5_6_7_second_order():
         assert o56 > 1.7 and o67 > 1.7
 
 
+@pytest.mark.parametrize("level,nv", [(0, 2), (2, 5), (3, 8), (4, 32), (5, 32), (3, 70)])
+def test_laplacian_matches_oracle(level, nv):
+    """thor_apply_lap (L369-L371: gradient on the triangles, then Eq. 6) against the oracle's two-stage
+    evaluation; even and odd layer counts take the vectorised and the scalar kernel."""
+    planet = dict(ti.EARTH)
+    g, G = _setup(level, nv, planet)
+    f = ti.harmonic_test_fields(G.xyz, planet, nv, seed=11 + nv, lmax=6 if level >= 2 else 2)
+    lap = g.apply_lap(f["s"])
+    assert _rel(lap, G.hlap(f["s"])) <= 1e-12
+    assert np.all(g.apply_lap(np.full((G.N, nv), -2.5)) == 0.0)
+    if level >= 4:                                                  # analytic: lap(f(z) sum a Y) = -f sum l(l+1) a Y / r^2
+        assert np.median(np.abs(lap - _lap_exact(G, planet, nv, 11 + nv))) < 0.01 * np.abs(lap).max()
+
+
+def _lap_exact(G, planet, nv, seed, lmax=6):
+    rng = np.random.default_rng(seed)
+    Y, _, ell = ti.real_sph_harm(G.xyz, lmax)
+    a = rng.standard_normal(Y.shape[1])                            # first draw of harmonic_test_fields = the scalar's coefficients
+    f = 1.0 + G.z_c / planet["z_top"]
+    return (-(Y * (ell * (ell + 1))[None, :]) @ a)[:, None] * (f / G.r_c ** 2)[None, :]
+
+
 @pytest.mark.parametrize("nv", [8, 16, 32, 64, 37, 5, 70, 128])
 def test_every_layer_shape_one_step(nv):
     """All lane-group shapes (G, E) incl. ragged layer counts, one large step with forcing."""

@@ -242,3 +242,70 @@ def test_p3_spring_dynamics_reduces_distortion(ogrid):
     raw, smooth = spread(3, False), spread(3, True)
     assert smooth[0] < 0.8 * raw[0]
     assert smooth[1] - 1 < 0.6 * (raw[1] - 1)
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-1 building block: the horizontal Laplacian of L369-L371 and the diffusion coefficient
+# --------------------------------------------------------------------------------------------
+def _lap_setup(ogrid, level, nv=2, lmax=4, seed=0):
+    import oracle
+    xyz, nbr, C = ogrid(level)
+    G = oracle.Geometry(xyz, nbr, nv, ti.EARTH, C)
+    Y, _, ell = ti.real_sph_harm(xyz, lmax)
+    a = np.random.default_rng(seed).standard_normal(Y.shape[1])
+    a[0] = 0.0
+    s1 = Y @ a
+    exact = -(Y * (ell * (ell + 1))[None, :]) @ a            # Laplace-Beltrami eigenfunctions on the unit sphere
+    return G, np.repeat(s1[:, None], nv, axis=1), exact
+
+
+def test_laplacian_of_a_constant_is_exactly_zero_and_it_is_in_flux_form(ogrid):
+    G, s, _ = _lap_setup(ogrid, 3)
+    assert np.all(G.hlap(np.full_like(s, 3.7)) == 0.0)
+    lap = G.hlap(s)
+    # Eq. 6 structure: every edge flux is shared by two control volumes with opposite normals and the
+    # bit-identical corner vectors, so the area integral telescopes to round-off
+    assert abs((G.Ac * lap[:, 0]).sum()) <= 1e-13 * (G.Ac * np.abs(lap[:, 0])).sum()
+    # deep atmosphere: the same unit-sphere operator over r_k^2 in every layer
+    assert np.allclose(lap[:, 0] * G.r_c[0] ** 2, lap[:, 1] * G.r_c[1] ** 2, rtol=1e-14, atol=0)
+
+
+def test_laplacian_converges_on_spherical_harmonics(ogrid):
+    """lap Y_lm = -l(l+1) Y_lm.  Second order in the bulk of the grid (median error falls ~4x per
+    level), l2 falls every level; the twelve pentagons keep an O(1) error, as for any such stencil on
+    a hexagonal-pentagonal grid, so l_inf is not asserted.  At these levels it beats div(grad)
+    composed from Eq. 6 and Eq. 7 in l2 -- the reason the paper gives for the construction (L369)."""
+    med, l2, l2_dg = {}, {}, {}
+    for level in (2, 3, 4):
+        G, s, exact = _lap_setup(ogrid, level)
+        r2 = G.r_c[0] ** 2
+        lap = G.hlap(s)[:, 0] * r2
+        dg = G.hdiv(G.hgrad(s))[:, 0] * r2
+        w = G.Ac / G.Ac.sum()
+        scale = np.abs(exact).max()
+        med[level] = np.median(np.abs(lap - exact)) / scale
+        l2[level] = np.sqrt((w * (lap - exact) ** 2).sum() / (w * exact ** 2).sum())
+        l2_dg[level] = np.sqrt((w * (dg - exact) ** 2).sum() / (w * exact ** 2).sum())
+        hexagons = G.deg == 6
+        assert np.abs(lap - exact)[hexagons].max() / scale < 0.12
+    assert med[2] / med[3] > 3.0 and med[3] / med[4] > 3.0
+    assert l2[2] > 2.0 * l2[3] and l2[3] > 2.0 * l2[4]
+    assert all(l2[k] < l2_dg[k] for k in (2, 3, 4))
+
+
+def test_diffusion_coefficient_formulas_and_table1_timescales():
+    """Eq. 49-50 (L373-L381): K_d = D dbar^4/dt and tau_d = dbar^4/(2^5 K_d), so tau_d = dt/(32 D)
+    whatever the resolution; with Table 1's timescales and the runs' time steps this gives the
+    non-dimensional D the paper used (0.004837 Earth, 0.01992 hot Jupiter)."""
+    import oracle
+    gold = _golden()
+    assert abs(oracle.dbar(7.0e7, 5) / 1e3 - gold["dbar_km_A70000km_g5"]) < 1.0          # Eq. 2
+    for key, dt, radius, D_expect in (("tau_d_earth_s", 1000.0, 6.371e6, 0.004837), ("tau_d_hotjupiter_s", 600.0, 1.0e8, 0.01992)):
+        tau = gold[key]
+        D = dt / (32.0 * tau)
+        assert abs(D - D_expect) < 5e-6
+        for level in (4, 5, 6):
+            db = oracle.dbar(radius, level)
+            K = oracle.kd(D, db, dt)
+            assert abs(oracle.tau_d(db, K) - tau) <= 1e-12 * tau
+            assert abs(K - D * db ** 4 / dt) <= 1e-15 * K
