@@ -58,10 +58,19 @@ def test_topology_and_device_order(level):
     assert sorted(v["device_order"]) == list(range(N))                      # a permutation
     assert np.allclose(np.linalg.norm(v["xyz"], axis=1), 1.0, atol=1e-15)
     if level >= 5:
-        # locality: neighbours sit close in device order (quadtree order of the leaf triangles)
+        # device order = rhombus by rhombus along the Morton curve of the lattice: every aligned run of
+        # 4 / 8 / 16 columns is a 2x2 / 2x4 / 4x4 patch, whose halo (distinct neighbours outside the run)
+        # is the minimum 10 / 14 / 18 columns; and neighbours sit close in memory
         rank = np.empty(N, dtype=np.int64)
         rank[v["device_order"]] = np.arange(N)
-        gaps = [abs(rank[i] - rank[j]) for i in range(N) for j in v["nbr"][i] if j >= 0]
+        dn = np.where(v["nbr"] >= 0, rank[np.where(v["nbr"] >= 0, v["nbr"], 0)], -1)[v["device_order"]]
+        for tc, hmax in ((4, 10), (8, 14), (16, 18)):
+            halos = []
+            for t in range(0, N - tc + 1, tc):
+                own = set(range(t, t + tc))
+                halos.append(len({int(x) for x in dn[t:t + tc].ravel() if x >= 0} - own))
+            assert max(halos) <= hmax and np.mean(halos) > hmax - 1
+        gaps = np.abs(dn - np.arange(N)[:, None])[dn >= 0]
         assert np.median(gaps) < 64
 
 
