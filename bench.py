@@ -133,8 +133,8 @@ def time_oracle(level, n_steps, warmup):
     dt = time.perf_counter() - t0
     cells = v["n_cols"] * cfg["nv"] * ti.substeps_per_large_step(cfg["n_sub"])
     return cells * n_steps / dt, dt / max(n_steps, 1), oracle.num_threads(), \
-        "config-3 constants and forcing at level %d x %d layers (%d columns), %d large steps" % (
-            level, cfg["nv"], v["n_cols"], n_steps)
+        "config-%d constants and forcing at level %d x %d layers (%d columns), %d large steps" % (
+            WORKLOAD, level, cfg["nv"], v["n_cols"], n_steps)
 
 
 def run_reference(args):
@@ -145,7 +145,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config 3 (hot Jupiter, n=8) sampled: " + sample},
+            "config": {"workload": "config %d (hot Jupiter, n=%d) sampled: " % (WORKLOAD, ti.CONFIGS[WORKLOAD]["n_sub"]) + sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -289,15 +289,17 @@ def run_cuda(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config 3: level 6 (40962 columns) x 32 layers, hot-Jupiter constants, dt=300 s, "
-                                   "n=8 (13 substeps per large step), Newtonian relaxation forcing",
+            "config": {"workload": "config %d: level %d (%d columns) x %d layers, hot-Jupiter constants, dt=%g s, "
+                                   "n=%d (%d substeps per large step), Newtonian relaxation forcing" % (
+                                       WORKLOAD, cfg["level"], N, nv, dt, n, substeps),
                        "cells": cells, "substeps_per_step": substeps, "parallelism": "replicas x%d" % world,
-                       "l2": "one large step streams the 33-row column-record slab (346 MB) > 126 MB L2; no flush"},
+                       "l2": "one large step streams the 33-row column-record slab (%d MB) > 126 MB L2; no flush" % (
+                           33 * 8 * cells * (64 if nv > 32 else 32) // nv // 1000000)},
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
             "gpu_launches": int(launches), "roofline": roofline,
-            "operators": {"what": "config 1 stencils alone on this grid (level 6 x 32), device arrays, 32 B/cell + geometry",
+            "operators": {"what": "config 1 stencils alone on this grid (level %d x %d), device arrays, 32 B/cell + geometry" % (cfg["level"], nv),
                           "div_ms": div_ms, "div_GBs": (cells * 32 + N * 224) / (div_ms * 1e-3) / 1e9,
                           "grad_ms": grad_ms, "grad_GBs": (cells * 32 + N * 176) / (grad_ms * 1e-3) / 1e9,
                           "lap_ms": lap_ms, "lap_GBs": (cells * 16 + N * 96) / (lap_ms * 1e-3) / 1e9,
@@ -317,7 +319,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", type=int, default=3, choices=[3, 4],
+                    help="BASELINE.json config: 3 = level 6 x 32 (default, the configuration the target is stated on), "
+                         "4 = level 7 x 64 (throughput at scale)")
     args = ap.parse_args()
+    global WORKLOAD
+    WORKLOAD = args.workload
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -64,6 +64,8 @@ def _load():
         L.orc_thomas.argtypes = [ctypes.c_int, _D, _D, _D, _D, _D]
         L.orc_centroid_eq13.argtypes = [_D, ctypes.c_int, _D]
         L.orc_step.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D]
+        L.orc_step_diffusion.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D,
+                                         ctypes.c_double, ctypes.c_double]
         L.orc_diagnostics.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, _D, _D]
         L.orc_tridiag_coefficients.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D, _D]
         L.orc_slow_terms.argtypes = [ctypes.c_void_p] + [_D] * 12
@@ -146,8 +148,10 @@ class Geometry:
         _load().orc_hlap(self._h, _p(s), _p(out))
         return out
 
-    def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None):
-        """n_large large steps; returns new (rho, V, W, p); inputs are not modified."""
+    def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None, D_hyp=0.0, D_div=0.0):
+        """n_large large steps; returns new (rho, V, W, p); inputs are not modified.  D_hyp, D_div:
+        non-dimensional diffusion parameter of Eq. 49 for the hyper-diffusion / divergence damping
+        (NEXT-1; 0 = off = the base path)."""
         rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
         assert rho.shape == (self.N, self.nv) and V.shape == (self.N, self.nv, 3)
         assert W.shape == (self.N, self.nv + 1) and p.shape == (self.N, self.nv)
@@ -157,8 +161,12 @@ class Geometry:
             T_eq = None if forcing.get("T_eq") is None else _c(forcing["T_eq"])
             k_T = None if forcing.get("k_T") is None else _c(forcing["k_T"])
             k_v = None if forcing.get("k_v") is None else _c(forcing["k_v"])
-        _load().orc_step(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
-                         _p(T_eq), _p(k_T), _p(k_v))
+        if D_hyp == 0.0 and D_div == 0.0:
+            _load().orc_step(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
+                             _p(T_eq), _p(k_T), _p(k_v))
+        else:
+            _load().orc_step_diffusion(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
+                                       _p(T_eq), _p(k_T), _p(k_v), float(D_hyp), float(D_div))
         return rho, V, W, p
 
     def diagnostics(self, rho, V, W, p):

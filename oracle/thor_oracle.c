@@ -293,8 +293,8 @@ void orc_hgrad(const orc_geom *G, const double *s, double *out) {
  *               the three columns sharing the triangle obtain the bit-identical vector)
  *   column:    lap_0 = (1/A_c) sum_k l_k (G_k + G_k+1)/2 . n_k,  times 1/r_k^2 at radius r_k.
  * s, out: [N][nv]. */
-void orc_hlap(const orc_geom *G, const double *s, double *out) {
-    const int N = G->N, nv = G->nv;
+static void hlap_unit(const orc_geom *G, const double *s, int nv, double *out) {
+    const int N = G->N;
 #pragma omp parallel
     {
         double *gk = (double *)malloc(sizeof(double) * 6 * 3);
@@ -319,11 +319,26 @@ void orc_hlap(const orc_geom *G, const double *s, double *out) {
                     double f = 0.5 * (g0[0] + g1[0]) * n[0] + 0.5 * (g0[1] + g1[1]) * n[1] + 0.5 * (g0[2] + g1[2]) * n[2];
                     sum += G->len[6 * i + k] * f;
                 }
-                out[(size_t)i * nv + lay] = sum / G->Ac[i] / (G->r_c[lay] * G->r_c[lay]);
+                out[(size_t)i * nv + lay] = sum / G->Ac[i];
             }
         }
         free(gk);
     }
+}
+void orc_hlap(const orc_geom *G, const double *s, double *out) {
+    const int N = G->N, nv = G->nv;
+    hlap_unit(G, s, nv, out);
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++)
+        for (int k = 0; k < nv; k++) out[(size_t)i * nv + k] = out[(size_t)i * nv + k] / (G->r_c[k] * G->r_c[k]);
+}
+/* the same operator on interface rows [N][nv+1] at the interface radii r_h,k */
+static void hlap_interfaces(const orc_geom *G, const double *s, double *out) {
+    const int N = G->N, nv = G->nv;
+    hlap_unit(G, s, nv + 1, out);
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++)
+        for (int k = 0; k <= nv; k++) out[(size_t)i * (nv + 1) + k] = out[(size_t)i * (nv + 1) + k] / (G->r_h[k] * G->r_h[k]);
 }
 
 /* Eq. 49-50 (L373-L381): K_d = D dbar^4 / dt, tau_d = dbar^4 / (2^5 K_d); dbar from Eq. 2 (G13). */
@@ -387,6 +402,9 @@ typedef struct {
     double *rho_s, *V_s, *W_s, *p_s, *rt;
     /* scratch */
     double *vec, *sc1, *sc2, *sc3, *gradp, *u, *Avec, *Wc;
+    /* NEXT-1 (Eq. 43-50): diffusion coefficients K_d (0 = term off), scratch, divergence-damping flux */
+    double Kd_hyp, Kd_div;
+    double *di1, *di2, *di3, *Fdd;     /* di*: [N][nv+1]; Fdd: [N][nv][3] */
 } orc_work;
 
 static double *dalloc(size_t n) { return (double *)calloc(n, sizeof(double)); }
@@ -402,13 +420,14 @@ static orc_work *work_new(const orc_geom *G) {
     w->rho_s = dalloc(nc); w->V_s = dalloc(3 * nc); w->W_s = dalloc(ni); w->p_s = dalloc(nc); w->rt = dalloc(nc);
     w->vec = dalloc(3 * nc); w->sc1 = dalloc(nc); w->sc2 = dalloc(nc); w->sc3 = dalloc(nc);
     w->gradp = dalloc(3 * nc); w->u = dalloc(3 * nc); w->Avec = dalloc(3 * nc); w->Wc = dalloc(nc);
+    w->di1 = dalloc(ni); w->di2 = dalloc(ni); w->di3 = dalloc(ni); w->Fdd = dalloc(3 * nc);
     return w;
 }
 static void work_free(orc_work *w) {
     double **p[] = {&w->rho_n, &w->V_n, &w->W_n, &w->p_n, &w->rt_n, &w->rho_t, &w->V_t, &w->W_t, &w->p_t,
                     &w->h, &w->th, &w->gt, &w->slowV, &w->slowrho, &w->Svr, &w->slowp, &w->slowrt,
                     &w->rho_s, &w->V_s, &w->W_s, &w->p_s, &w->rt, &w->vec, &w->sc1, &w->sc2, &w->sc3,
-                    &w->gradp, &w->u, &w->Avec, &w->Wc};
+                    &w->gradp, &w->u, &w->Avec, &w->Wc, &w->di1, &w->di2, &w->di3, &w->Fdd};
     for (size_t i = 0; i < sizeof(p) / sizeof(p[0]); i++) free(*p[i]);
     free(w);
 }
@@ -543,6 +562,131 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
     }
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-1: explicit fourth-order hyper-diffusion and 3-D divergence damping (section 4;
+ * Eq. 43-48, of which 43-44 are lost and 45-46 damaged in PAPER.md -- readings RD1-RD5 of DESIGN.md).
+ * Every nabla_h^2 is orc_hlap's operator (L369-L371).  K_d = D dbar^4 / dt (Eq. 49).
+ * ------------------------------------------------------------------------------------------- */
+
+/* RD2 (Fig. 6 large-step 2, L307: "Compute diffuse fluxes" inside the three-stage loop): fluxes of the
+ * stage reference state, added to the slow terms of the stage:
+ *   F_rho = -K_d lap(lap(rho))                                   (Eq. 43 by the pattern of Eq. 47)
+ *   F_vhj = -K_d lap(rho lap(v_j)), v = V/rho, j = x, y, z, then Eq. 28   (Eq. 44-46, first term)
+ *   F_vr  = -K_d lap(rho_h lap(w)) on interfaces, w = W/I_h[rho]          (Eq. 47)
+ *   F_p   = -Rd K_d lap(rho lap(T)), T = p/(Rd rho)                        (Eq. 48)
+ * RD3: F_p enters the slow pressure term and, because the substeps carry rho*theta (Eq. 35) and
+ * diagnose p from it (Eq. 36), the slow rho*theta term through Eq. 24: d(rho theta) = (rho theta)/(gamma p) dp. */
+static void hyper_diffusion(const orc_geom *G, orc_work *w) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const size_t nc = w->nc, ni = w->ni;
+    const double Kd = w->Kd_hyp, gam = P->Cp / (P->Cp - P->Rd);
+    double *a = w->di1, *b = w->di2, *c = w->di3;
+    /* density */
+    orc_hlap(G, w->rho_t, a);
+    orc_hlap(G, a, b);
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < nc; q++) w->slowrho[q] = w->slowrho[q] + (-Kd * b[q]);
+    /* horizontal momentum, one Cartesian component at a time */
+    for (int j = 0; j < 3; j++) {
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < nc; q++) a[q] = w->V_t[3 * q + j] / w->rho_t[q];
+        orc_hlap(G, a, b);
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < nc; q++) b[q] = w->rho_t[q] * b[q];
+        orc_hlap(G, b, c);
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < nc; q++) w->Avec[3 * q + j] = -Kd * c[q];
+    }
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rh = G->xyz + 3 * i;
+        for (int k = 0; k < nv; k++) {
+            size_t q = (size_t)i * nv + k;
+            double Fr = dot3(w->Avec + 3 * q, rh);
+            for (int d = 0; d < 3; d++) w->slowV[3 * q + d] = w->slowV[3 * q + d] + (w->Avec[3 * q + d] - Fr * rh[d]);
+        }
+    }
+    /* vertical momentum on interior interfaces */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rho = w->rho_t + (size_t)i * nv, *W = w->W_t + (size_t)i * (nv + 1);
+        double *wv = a + (size_t)i * (nv + 1);
+        wv[0] = 0.0; wv[nv] = 0.0;
+        for (int k = 1; k < nv; k++) wv[k] = W[k] / I_h(rho, k);
+    }
+    hlap_interfaces(G, a, b);
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rho = w->rho_t + (size_t)i * nv;
+        double *x = b + (size_t)i * (nv + 1);
+        x[0] = 0.0; x[nv] = 0.0;
+        for (int k = 1; k < nv; k++) x[k] = I_h(rho, k) * x[k];
+    }
+    hlap_interfaces(G, b, c);
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++)
+        for (int k = 1; k < nv; k++) {
+            size_t q = (size_t)i * (nv + 1) + k;
+            w->Svr[q] = w->Svr[q] + (-Kd * c[q]);
+        }
+    (void)ni;
+    /* pressure through temperature */
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < nc; q++) a[q] = w->p_t[q] / (P->Rd * w->rho_t[q]);
+    orc_hlap(G, a, b);
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < nc; q++) b[q] = w->rho_t[q] * b[q];
+    orc_hlap(G, b, c);
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < nc; q++) {
+        double Fp = -P->Rd * Kd * c[q];
+        w->slowp[q] = w->slowp[q] + Fp;
+        w->slowrt[q] = w->slowrt[q] + Fp * eos_rt(P, w->p_t[q]) / (gam * w->p_t[q]);
+    }
+}
+
+/* RD4 (Eq. 44-46 second term; Fig. 6 small-step 1, L318; "updated every short time step", L367):
+ *   D3 = div_h(V) + D_c[W] of the CURRENT momentum V = V^[t] + V*, W = W^[t] + W*;
+ *   F_dd = -K_d lap(grad_h D3), the Laplacian applied to each Cartesian component, then Eq. 28;
+ * it enters the explicit horizontal momentum step (Eq. 33) only (Eq. 47 carries no such term). */
+static void divergence_damping(const orc_geom *G, orc_work *w) {
+    const int N = G->N, nv = G->nv;
+    const size_t nc = w->nc;
+    double *a = w->di1, *b = w->di2;
+#pragma omp parallel for schedule(static)
+    for (size_t q = 0; q < 3 * nc; q++) w->vec[q] = w->V_t[q] + w->V_s[q];
+    orc_hdiv(G, w->vec, w->sc1);
+#pragma omp parallel
+    {
+        double *X = (double *)calloc(nv + 1, sizeof(double));
+#pragma omp for schedule(static)
+        for (int i = 0; i < N; i++) {
+            const double *Wt = w->W_t + (size_t)i * (nv + 1), *Ws = w->W_s + (size_t)i * (nv + 1);
+            for (int k = 0; k <= nv; k++) X[k] = Wt[k] + Ws[k];
+            for (int k = 0; k < nv; k++) w->sc1[(size_t)i * nv + k] = w->sc1[(size_t)i * nv + k] + D_c(G, X, k);
+        }
+        free(X);
+    }
+    orc_hgrad(G, w->sc1, w->gradp);                 /* gradp is free here: Eq. 33 recomputes it afterwards */
+    for (int j = 0; j < 3; j++) {
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < nc; q++) a[q] = w->gradp[3 * q + j];
+        orc_hlap(G, a, b);
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < nc; q++) w->Fdd[3 * q + j] = -w->Kd_div * b[q];
+    }
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double *rh = G->xyz + 3 * i;
+        for (int k = 0; k < nv; k++) {
+            size_t q = (size_t)i * nv + k;
+            double Fr = dot3(w->Fdd + 3 * q, rh);
+            for (int d = 0; d < 3; d++) w->Fdd[3 * q + d] = w->Fdd[3 * q + d] - Fr * rh[d];
+        }
+    }
+}
+
 /* Tridiagonal coefficients of O6 item 3 for one column at interior interfaces k = 1..nv-1
  * (exact elimination of Eq. 32, the linearised pressure equation and Eq. 34; reading R8). */
 static void tridiag_coefficients(const orc_geom *G, double delta, const double *h, const double *gt,
@@ -573,10 +717,17 @@ static void substep(const orc_geom *G, orc_work *w, double delta) {
     const double kv = P->Rd / (P->Cp - P->Rd), dz = G->dz, g = P->gravity;
     const size_t nc = w->nc;
 
+    /* Fig. 6 small-step 1 (NEXT-1, only when K_d > 0) */
+    if (w->Kd_div > 0.0) divergence_damping(G, w);
     /* a4: Eq. 33 */
     orc_hgrad(G, w->p_s, w->gradp);
+    if (w->Kd_div > 0.0) {
 #pragma omp parallel for schedule(static)
-    for (size_t q = 0; q < 3 * nc; q++) w->V_s[q] = w->V_s[q] + delta * (-w->gradp[q] + w->slowV[q]);
+        for (size_t q = 0; q < 3 * nc; q++) w->V_s[q] = w->V_s[q] + delta * (-w->gradp[q] + w->slowV[q] + w->Fdd[q]);
+    } else {
+#pragma omp parallel for schedule(static)
+        for (size_t q = 0; q < 3 * nc; q++) w->V_s[q] = w->V_s[q] + delta * (-w->gradp[q] + w->slowV[q]);
+    }
 
     /* a5: divergences of the new momentum */
     orc_hdiv(G, w->V_s, w->sc1);
@@ -648,11 +799,24 @@ static void forcing(const orc_geom *G, double dt, double *rho, double *V, double
 
 /* One call = n_large large steps (Fig. 6; stage convention R1 of SURVEY O5).
  * State arrays are updated in place: rho,p [N][nv]; V [N][nv][3]; W [N][nv+1] (ends forced to 0). */
-void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
-              int n_sub, const double *T_eq, const double *k_T, const double *k_v) {
+double orc_dbar(double radius, int level);
+double orc_kd(double D, double dbar, double dt);
+
+/* D_hyp, D_div: the non-dimensional diffusion parameter of Eq. 49 for the hyper-diffusion and for the
+ * divergence damping (the paper uses the same value for both, L367); 0 switches a term off, and
+ * (0, 0) is the base path of SURVEY 8(a), arithmetic untouched. */
+void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
+                        int n_sub, const double *T_eq, const double *k_T, const double *k_v, double D_hyp, double D_div) {
     const int N = G->N, nv = G->nv;
     orc_work *w = work_new(G);
     const size_t nc = w->nc, ni = w->ni;
+    {
+        int level = 0;
+        while (10 * (1 << (2 * level)) + 2 < N) level++;          /* Eq. 1 inverted */
+        const double dbar = orc_dbar(G->P.radius, level);         /* Eq. 2 */
+        w->Kd_hyp = D_hyp > 0.0 ? orc_kd(D_hyp, dbar, dt) : 0.0;  /* Eq. 49 */
+        w->Kd_div = D_div > 0.0 ? orc_kd(D_div, dbar, dt) : 0.0;
+    }
     for (int i = 0; i < N; i++) { W[(size_t)i * (nv + 1)] = 0.0; W[(size_t)i * (nv + 1) + nv] = 0.0; }
     for (int step = 0; step < n_large; step++) {
         memcpy(w->rho_n, rho, 8 * nc); memcpy(w->V_n, V, 24 * nc); memcpy(w->W_n, W, 8 * ni); memcpy(w->p_n, p, 8 * nc);
@@ -662,6 +826,7 @@ void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, i
         for (int stage = 1; stage <= 3; stage++) {                 /* Eq. 30 (L245-L250) */
             stage_coefficients(G, w);                              /* Fig. 6 large-step 1 */
             slow_terms(G, w);                                      /* Fig. 6 large-step 3 */
+            if (w->Kd_hyp > 0.0) hyper_diffusion(G, w);            /* Fig. 6 large-step 2 (NEXT-1) */
             int ns; double delta;                                  /* L252, L312-L316 */
             if (stage == 1) { ns = 1; delta = dt / 3.0; }
             else if (stage == 2) { ns = n_sub / 2; delta = dt / n_sub; }
@@ -691,6 +856,10 @@ void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, i
         forcing(G, dt, rho, V, p, T_eq, k_T, k_v);
     }
     work_free(w);
+}
+void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
+              int n_sub, const double *T_eq, const double *k_T, const double *k_v) {
+    orc_step_diffusion(G, rho, V, W, p, n_large, dt, n_sub, T_eq, k_T, k_v, 0.0, 0.0);
 }
 
 /* a12 (O8, R10): total mass and total energy with the weight A_c r_k^2 dz under which D_c telescopes.
