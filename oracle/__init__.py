@@ -70,6 +70,8 @@ def _load():
         L.orc_tridiag_coefficients.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D, _D]
         L.orc_slow_terms.argtypes = [ctypes.c_void_p] + [_D] * 12
         L.orc_substep.argtypes = [ctypes.c_void_p, ctypes.c_double] + [_D] * 14
+        L.orc_diffusion_fluxes.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_double, _D, _D, _D, _D, _D]
+        L.orc_divergence_damping.argtypes = [ctypes.c_void_p, _D, _D, ctypes.c_double, _D]
         L.orc_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -168,6 +170,20 @@ class Geometry:
             _load().orc_step_diffusion(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
                                        _p(T_eq), _p(k_T), _p(k_v), float(D_hyp), float(D_div))
         return rho, V, W, p
+
+    # NEXT-1 (Eq. 43-48): hyper-diffusion fluxes of a state, and the divergence-damping flux of a momentum field
+    def diffusion_fluxes(self, rho, V, W, p, Kd):
+        rho, V, W, p = (_c(x) for x in (rho, V, W, p))
+        N, nv = self.N, self.nv
+        Frho, FV, FW, Fp, Frt = np.empty((N, nv)), np.empty((N, nv, 3)), np.empty((N, nv + 1)), np.empty((N, nv)), np.empty((N, nv))
+        _load().orc_diffusion_fluxes(self._h, _p(rho), _p(V), _p(W), _p(p), float(Kd), _p(Frho), _p(FV), _p(FW), _p(Fp), _p(Frt))
+        return Frho, FV, FW, Fp, Frt
+
+    def divergence_damping(self, V, W, Kd):
+        V, W = _c(V), _c(W)
+        out = np.empty((self.N, self.nv, 3))
+        _load().orc_divergence_damping(self._h, _p(V), _p(W), float(Kd), _p(out))
+        return out
 
     def diagnostics(self, rho, V, W, p):
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))

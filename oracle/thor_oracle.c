@@ -931,6 +931,27 @@ void orc_substep(const orc_geom *G, double delta, const double *h, const double 
     work_free(w);
 }
 
+/* NEXT-1 pins: the diffusive fluxes of a given state alone (slow terms start at zero), and the
+ * divergence-damping flux of a given momentum field */
+void orc_diffusion_fluxes(const orc_geom *G, const double *rho, const double *V, const double *W, const double *p,
+                          double Kd, double *Frho, double *FV, double *FW, double *Fp, double *Frt) {
+    orc_work *w = work_new(G);
+    memcpy(w->rho_t, rho, 8 * w->nc); memcpy(w->V_t, V, 24 * w->nc); memcpy(w->W_t, W, 8 * w->ni); memcpy(w->p_t, p, 8 * w->nc);
+    w->Kd_hyp = Kd;
+    hyper_diffusion(G, w);
+    memcpy(Frho, w->slowrho, 8 * w->nc); memcpy(FV, w->slowV, 24 * w->nc); memcpy(FW, w->Svr, 8 * w->ni);
+    memcpy(Fp, w->slowp, 8 * w->nc); memcpy(Frt, w->slowrt, 8 * w->nc);
+    work_free(w);
+}
+void orc_divergence_damping(const orc_geom *G, const double *V, const double *W, double Kd, double *Fdd) {
+    orc_work *w = work_new(G);
+    memcpy(w->V_t, V, 24 * w->nc); memcpy(w->W_t, W, 8 * w->ni);
+    w->Kd_div = Kd;
+    divergence_damping(G, w);
+    memcpy(Fdd, w->Fdd, 24 * w->nc);
+    work_free(w);
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     extern int omp_get_max_threads(void);

@@ -318,3 +318,108 @@ def test_forcing_limits(ogrid):
     b = G.step(*state, 1, 600.0, 2, dict(T_eq=None, k_T=None, k_v=np.full(shape, 1e-3)))
     assert np.abs(b[1] * 1.6 - a[1]).max() < 1e-12 * np.abs(a[1]).max()
     assert np.array_equal(a[2], b[2]) and np.array_equal(a[0], b[0]) and np.array_equal(a[3], b[3])
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-1: hyper-diffusion and divergence damping (Eq. 43-50; readings RD1-RD5 of DESIGN.md)
+# --------------------------------------------------------------------------------------------
+def test_diffusion_off_is_the_base_path_bit_for_bit(ogrid):
+    cfg = ti.CONFIGS[0]
+    G = _geom(ogrid, 2, cfg["nv"], cfg["planet"])
+    state = ti.initial_state(0, G.xyz)
+    a = G.step(*state, 2, cfg["dt"], cfg["n_sub"])
+    b = G.step(*state, 2, cfg["dt"], cfg["n_sub"], None, 0.0, 0.0)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+
+
+def test_diffusion_conserves_mass_and_keeps_the_rest_state(ogrid):
+    cfg = ti.CONFIGS[0]
+    planet, nv = cfg["planet"], cfg["nv"]
+    G = _geom(ogrid, 3, nv, planet)
+    D = 0.004837                                     # the paper's Earth value (Table 1 with dt = 1000 s)
+    state = ti.initial_state(0, G.xyz)
+    m0, _ = G.diagnostics(*state)
+    out = G.step(*state, 5, cfg["dt"], cfg["n_sub"], None, D, D)
+    m1, _ = G.diagnostics(*out)
+    assert abs(m1 - m0) <= 1e-14 * m0                # the Laplacian is in flux form: F_rho integrates to zero
+    assert not np.array_equal(out[0], G.step(*state, 5, cfg["dt"], cfg["n_sub"])[0])
+    rest = ti.rest_state(planet, nv, G.N, cfg["p_s"], cfg["T0"])
+    a = G.step(*rest, 3, cfg["dt"], cfg["n_sub"], None, D, D)
+    b = G.step(*rest, 3, cfg["dt"], cfg["n_sub"])
+    assert np.abs(a[1]).max() < 1e-9 and np.abs(a[2]).max() < 1e-9      # still at rest (P12)
+    assert np.abs(a[0] - b[0]).max() <= 1e-13 * np.abs(b[0]).max()     # horizontally uniform fields: lap = 0
+
+
+def test_hyper_diffusion_fluxes_closed_forms(ogrid):
+    """On a horizontally uniform density: solid-body rotation v = w x r has Cartesian components that
+    are degree-1 harmonics, lap v_j = -2 v_j / r^2, so F_vh = -K_d lap(rho lap v) = -4 K_d rho v / r^4
+    (tangent already); T = T0 + a Y_l gives F_p = -Rd K_d rho [l(l+1)]^2 a Y_l / r^4, and the same
+    pattern on rho gives F_rho.  F_rt follows F_p through Eq. 24."""
+    import oracle
+    planet, nv = dict(ti.EARTH), 3
+    planet["z_top"] = 9000.0
+    xyz, nbr, C = ogrid(4, True)
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1.0e5, 280.0)
+    Kd = 1.0e16
+    om = np.array([0.3, -0.2, 1.0]) * 1e-5
+    vel = np.cross(om[None, None, :], xyz[:, None, :] * G.r_c[None, :, None])
+    V = rho[..., None] * vel
+    Y, _, ell = ti.real_sph_harm(xyz, 3)
+    k = int(np.where(ell == 3)[0][2])
+    T = 280.0 + 2.0 * Y[:, k][:, None] * np.ones(nv)[None, :]
+    p = rho * planet["Rd"] * T
+    Frho, FV, FW, Fp, Frt = G.diffusion_fluxes(rho, V, W, p, Kd)
+    exact_V = -4.0 * Kd * V / G.r_c[None, :, None] ** 4
+    # A biharmonic operator built from two 7-point Laplacians is not pointwise consistent on an irregular
+    # grid (the second Laplacian differentiates the first one's O(h^2) error twice): the pins are the median
+    # and the 90th percentile away from the twelve pentagons, not the maximum
+    far = np.ones(G.N, dtype=bool)
+    ring = np.where(G.deg == 5)[0]
+    for _ in range(3):
+        far[ring] = False
+        ring = np.unique(G.nbr[ring][G.nbr[ring] >= 0])
+    assert np.median(np.abs(FV - exact_V)) < 0.01 * np.abs(exact_V).max()
+    assert np.percentile(np.abs(FV - exact_V)[far], 90) < 0.05 * np.abs(exact_V).max()
+    exact_p = -planet["Rd"] * Kd * rho * 144.0 * (T - 280.0) / G.r_c[None, :] ** 4
+    assert np.median(np.abs(Fp - exact_p)) < 0.02 * np.abs(exact_p).max()
+    assert np.percentile(np.abs(Fp - exact_p)[far], 90) < 0.1 * np.abs(exact_p).max()
+    assert np.all(Frho == 0.0) and np.all(FW == 0.0)                   # uniform rho, W = 0
+    gam = planet["Cp"] / (planet["Cp"] - planet["Rd"])
+    rt = planet["p_ref"] / planet["Rd"] * (p / planet["p_ref"]) ** (1.0 / gam)
+    assert np.allclose(Frt, Fp * rt / (gam * p), rtol=1e-12, atol=0)
+    # density pattern and vertical velocity pattern: same operator, same eigenvalue
+    rho2 = rho * (1.0 + 1e-3 * Y[:, k][:, None])
+    W2 = np.zeros_like(W)
+    W2[:, 1:nv] = 0.5 * (rho[:, 1:] + rho[:, :-1]) * 0.01 * Y[:, k][:, None]
+    Frho2, _, FW2, _, _ = G.diffusion_fluxes(rho2, np.zeros_like(V), W2, rho2 * planet["Rd"] * 280.0, Kd)
+    ex_rho = -Kd * 144.0 * (rho2 - rho) / G.r_c[None, :] ** 4
+    assert np.median(np.abs(Frho2 - ex_rho)) < 0.02 * np.abs(ex_rho).max()
+    ex_W = -Kd * 144.0 * W2[:, 1:nv] / G.r_h[None, 1:nv] ** 4
+    assert np.median(np.abs(FW2[:, 1:nv] - ex_W)) < 0.03 * np.abs(ex_W).max()
+    assert np.all(FW2[:, 0] == 0.0) and np.all(FW2[:, nv] == 0.0)
+
+
+def test_divergence_damping_acts_on_divergence_only(ogrid):
+    """F_dd = -K_d lap(grad D3): tangent; (nearly) zero for a non-divergent flow; for a divergent flow
+    it opposes the divergence pattern (div F_dd anti-correlated with D3)."""
+    import oracle
+    planet, nv = dict(ti.EARTH), 2
+    planet["z_top"] = 6000.0
+    xyz, nbr, C = ogrid(4, True)
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1.0e5, 280.0)
+    Y, gY, ell = ti.real_sph_harm(xyz, 4)
+    a = np.random.default_rng(3).standard_normal(Y.shape[1])
+    a[0] = 0.0
+    gchi = np.einsum("nkd,k->nd", gY, a)
+    Vdiv = rho[..., None] * gchi[:, None, :]
+    Vrot = rho[..., None] * np.cross(xyz, gchi)[:, None, :]
+    Kd = 1.0e16
+    Fd, Fr = G.divergence_damping(Vdiv, W, Kd), G.divergence_damping(Vrot, W, Kd)
+    assert np.abs(np.sum(Fd * xyz[:, None, :], axis=-1)).max() <= 1e-12 * np.abs(Fd).max()
+    assert np.median(np.linalg.norm(Fr, axis=-1)) < 0.02 * np.median(np.linalg.norm(Fd, axis=-1))   # (spikes at the pentagons only)
+    D3 = G.hdiv(Vdiv)
+    w = G.Ac[:, None]
+    corr = (w * G.hdiv(Fd) * D3).sum() / np.sqrt((w * G.hdiv(Fd) ** 2).sum() * (w * D3 ** 2).sum())
+    assert corr < -0.7
