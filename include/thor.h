@@ -103,6 +103,14 @@ void thor_state_destroy(thor_state *state);
  * then the forcing (NULL = none) with the large step dt (L385).  n_acoustic_substeps = n, even, >= 2. */
 int thor_step(thor_state *state, int n_large, double dt, int n_acoustic_substeps, const thor_forcing *forcing);
 
+/* NEXT-1 (section 4 of the paper, Eq. 43-50): switch on the explicit fourth-order hyper-diffusion of
+ * rho, v_h, v_r and T (per Runge-Kutta stage, Fig. 6 large-step 2) and the 3-D divergence damping
+ * (per acoustic substep, Fig. 6 small-step 1) for the following thor_step calls.  D_hyper, D_div are
+ * the non-dimensional parameter of Eq. 49, K_d = D dbar^4 / dt with dbar of Eq. 2; the paper uses the
+ * same value for both (L367; 0.004837 for its Earth run, 0.01992 for its hot Jupiter, from Table 1).
+ * 0 switches a term off; (0, 0), the default, is the base path.  Allocates the work rows on first use. */
+int thor_state_set_diffusion(thor_state *state, double D_hyper, double D_div);
+
 /* Only the hot loop: n_substeps acoustic substeps (steps a4-a9 of DESIGN.md) of length delta on the
  * stage data left by the last thor_step.  which: 1 = explicit horizontal momentum kernel only,
  * 2 = divergence + column-solve kernel only, 3 = both.  For measurement; the state it leaves is

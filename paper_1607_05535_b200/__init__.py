@@ -54,6 +54,7 @@ _SIGNATURES = {
     "thor_state_get": (ctypes.c_int, [_V, _D, _D, _D, _D]),
     "thor_state_destroy": (None, [_V]),
     "thor_step": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(thor_forcing)]),
+    "thor_state_set_diffusion": (ctypes.c_int, [_V, ctypes.c_double, ctypes.c_double]),
     "thor_acoustic_substeps": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int]),
     "thor_diagnostics": (ctypes.c_int, [_V, ctypes.POINTER(thor_diag)]),
     "thor_apply_div": (ctypes.c_int, [_V, _D, _D]),
@@ -149,6 +150,10 @@ def thor_state_destroy(state):
 def thor_step(state, n_large, dt, n_acoustic_substeps, forcing=None):
     _check(load_library().thor_step(state, int(n_large), float(dt), int(n_acoustic_substeps),
                                     None if forcing is None else ctypes.byref(forcing)))
+
+
+def thor_state_set_diffusion(state, D_hyper, D_div):
+    _check(load_library().thor_state_set_diffusion(state, float(D_hyper), float(D_div)))
 
 
 def thor_acoustic_substeps(state, n_substeps, delta, which=3):
@@ -274,6 +279,10 @@ class State:
                 f = thor_forcing(_ptr(arrs["T_eq"]), _ptr(arrs["k_T"]), _ptr(arrs["k_v"]), 0)
                 self._forcing, self._forcing_keep, self._forcing_arrays = f, forcing, arrs
         thor_step(self._h, n_large, dt, n_acoustic_substeps, f)
+
+    def set_diffusion(self, D_hyper, D_div=None):
+        """NEXT-1: hyper-diffusion and divergence damping parameter D of Eq. 49 (D_div defaults to D_hyper, L367)."""
+        thor_state_set_diffusion(self._h, D_hyper, D_hyper if D_div is None else D_div)
 
     def acoustic_substeps(self, n_substeps, delta, which=3):
         thor_acoustic_substeps(self._h, n_substeps, delta, which)

@@ -47,7 +47,7 @@ struct DeviceGeom {
     int* order = nullptr;
     double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
     double *basis = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr, *wlap = nullptr;
-    double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr;
+    double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr, *rhinv = nullptr;
     // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
     int tcol = 0, hmax = 0;
     int* tile_halo = nullptr;
@@ -76,6 +76,8 @@ struct thor_state {
     cudaStream_t stream = nullptr;
     int NVP = 0;
     double* S = nullptr;             // the slab of column records [Npad][NF][NVP]
+    double* X = nullptr;             // NEXT-1 work rows [Npad][XF][NVP], allocated by thor_state_set_diffusion
+    double D_hyp = 0.0, D_div = 0.0; // non-dimensional diffusion parameters of Eq. 49 (0 = term off)
     double* stage_buf = nullptr;     // canonical-order staging, max(N*nv*3, N*(nv+1)) doubles
     double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;   // [Npad][NVP]
     bool has_Teq = false, has_kT = false, has_kv = false;
@@ -83,7 +85,7 @@ struct thor_state {
     bool stepped = false;
     int walk = 0;                    // direction of the last launch (0 ascending, 1 descending)
     // one large step captured as a CUDA graph, per starting walk direction (replayed while the key holds)
-    struct GraphKey { double dt = 0; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
+    struct GraphKey { double dt = 0, D_hyp = 0, D_div = 0; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
     GraphKey gkey;
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     int gwalk_end[2] = {0, 0};
@@ -149,6 +151,11 @@ int ensure_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.dhi, padded(h.dhi)))) return rc;
     if ((rc = upload(&d.vol, padded(h.vol)))) return rc;
     if ((rc = upload(&d.zc, padded(h.zc)))) return rc;
+    {
+        std::vector<double> rh(h.nv);
+        for (int k = 0; k < h.nv; ++k) rh[k] = 1.0 / (h.P.radius + k * h.dz);
+        if ((rc = upload(&d.rhinv, padded(rh)))) return rc;
+    }
     {   // tile tables: halo columns of every tile and, per column, the slot of each neighbour
         const Shape sh = shape_for(h.nv);
         const int TC = kTmaWarps * (32 / sh.G), ntiles = Npad / TC;
@@ -191,7 +198,7 @@ Geom make_geom(const thor_grid* grid) {
     g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
     g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
     g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
-    g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc;
+    g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
     g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
@@ -400,7 +407,7 @@ void thor_grid_destroy(thor_grid* grid) {
     DeviceGeom& d = grid->d;
     if (d.ready) {
         cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
-        cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc);
+        cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc); cudaFree(d.rhinv);
         cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap);
     }
     delete grid;
@@ -410,7 +417,7 @@ static void drop_graphs(thor_state* s);
 
 void thor_state_destroy(thor_state* s) {
     if (!s) return;
-    cudaFree(s->S); cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
+    cudaFree(s->S); cudaFree(s->X); cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
     cudaFree(s->col_mass); cudaFree(s->col_energy);
     drop_graphs(s);
     delete s;
@@ -488,6 +495,11 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
     const int nv = g.nv, Npad = g.Npad;
     cudaStream_t st = s->stream;
     double* S = s->S;
+    // K_d = D dbar^4 / dt (Eq. 49), dbar = sqrt(2 pi / 5) A / 2^level (Eq. 2)
+    const HostGrid& hg = s->grid->h;
+    const double dbar = std::sqrt(2.0 * 3.14159265358979323846 / 5.0) * hg.P.radius / std::pow(2.0, hg.level);
+    const double Kd_hyp = (s->X && s->D_hyp > 0.0) ? s->D_hyp * dbar * dbar * dbar * dbar / dt : 0.0;
+    const double Kd_div = (s->X && s->D_div > 0.0) ? s->D_div * dbar * dbar * dbar * dbar / dt : 0.0;
     // every launch walks the columns opposite to the one before it (L2 hand-over)
     auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
     for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
@@ -495,8 +507,18 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         const double delta = stage == 1 ? dt / 3.0 : dt / n;
         THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks));
         THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks));
+        if (Kd_hyp > 0.0) {                                            // Fig. 6 large-step 2 (NEXT-1)
+            THOR_DISPATCH(k_diff0, nv, Npad, st, g, S, s->X);
+            THOR_DISPATCH(k_diff1, nv, Npad, st, g, S, s->X);
+            THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp);
+        }
         for (int sub = 0; sub < ns; ++sub) {
-            THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
+            if (Kd_div > 0.0) {                                        // Fig. 6 small-step 1 (NEXT-1)
+                THOR_DISPATCH(k_dd1, nv, Npad, st, g, S, s->X);
+                THOR_DISPATCH(k_dd2, nv, Npad, st, g, s->X);
+                THOR_DISPATCH(k_dd3, nv, Npad, st, g, s->X, Kd_div);
+            }
+            THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1), Kd_div > 0.0 ? s->X : nullptr);
             TunePair t2 = tn;
             t2.k2 = dir(tn.k2);
             if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st)) return rc;
@@ -535,7 +557,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (use_graph) {
         thor_state::GraphKey key;
         std::memset(&key, 0, sizeof(key));
-        key.dt = dt; key.n = n; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
+        key.dt = dt; key.n = n; key.D_hyp = s->D_hyp; key.D_div = s->D_div; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
         if (const char* e = std::getenv("THOR_B200_TUNE")) std::strncpy(key.tune, e, sizeof(key.tune) - 1);
         if (std::memcmp(&key, &s->gkey, sizeof(key)) != 0) {
             drop_graphs(s);
@@ -573,6 +595,22 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     return THOR_OK;
 }
 
+int thor_state_set_diffusion(thor_state* s, double D_hyper, double D_div) {
+    if (!s) return fail(THOR_EINVAL, "thor_state_set_diffusion: null state");
+    if (!(D_hyper >= 0.0) || !(D_div >= 0.0)) return fail(THOR_EINVAL, "thor_state_set_diffusion: need D >= 0");
+    if ((D_hyper > 0.0 || D_div > 0.0) && !s->X) {
+        const size_t n = size_t(s->grid->d.Npad) * XF * s->NVP;
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&s->X), n * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemsetAsync(s->X, 0, n * sizeof(double), s->stream);
+        if (e != cudaSuccess)
+            return fail(e == cudaErrorMemoryAllocation ? THOR_ENOMEM : THOR_ECUDA,
+                        std::string("thor_state_set_diffusion: ") + cudaGetErrorString(e));
+    }
+    s->D_hyp = D_hyper;
+    s->D_div = D_div;
+    return THOR_OK;
+}
+
 int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int which) {
     if (!s) return fail(THOR_EINVAL, "thor_acoustic_substeps: null state");
     if (n_substeps < 0 || !(delta > 0) || which < 1 || which > 3) return fail(THOR_EINVAL, "thor_acoustic_substeps: bad argument");
@@ -583,7 +621,7 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     const TunePair tn = tune();
     auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
     for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1));
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1), (const double*)nullptr);
         TunePair t2 = tn;
         if (which & 2) t2.k2 = dir(tn.k2);
         if (which & 2)

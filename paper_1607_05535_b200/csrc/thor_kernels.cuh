@@ -48,6 +48,14 @@ enum Field : int {
     NF
 };
 
+// rows of the NEXT-1 work slab X (hyper-diffusion and divergence damping, see k_diff0 .. k_dd3)
+enum XField : int {
+    X_VX = 0, X_VY, X_VZ, X_W, X_T,              // k_diff0: v = V/rho, w = W/I_h[rho], T = p/(Rd rho) of Phi^[t]
+    X_Q0, X_Q1, X_Q2, X_Q3, X_Q4, X_Q5,          // k_diff1: lap(rho), rho lap(v_x..z), rho_h lap(w), rho lap(T)
+    XF,
+    X_D3 = 0, X_GX = 1, X_GY = 2, X_GZ = 3, X_FA = 4, X_FB = 5    // divergence damping reuses rows 0-5 during the substeps
+};
+
 struct Geom {                 // device pointers, device column order, padded to Npad columns
     int N, Npad, nv;
     const int* nbr;           // [Npad][8]   6 neighbours (pentagons, pad columns: self), 2 x self
@@ -64,6 +72,7 @@ struct Geom {                 // device pointers, device column order, padded to
     const double* dhi;        // [128] r_h,k+1^2/(r_k^2 dz)
     const double* vol;        // [128] r_k^2 dz
     const double* zc;         // [128]
+    const double* rhinv;      // [128] 1/r_h,k: radius of the LOWER interface of layer k (pad layers: 0)
     double dz, omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
@@ -790,7 +799,7 @@ k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
+k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -826,6 +835,13 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
             const double d = pj[j][e] - p0[e];
             ga[e] = fma(wgv[2 * j], d, ga[e]); gb[e] = fma(wgv[2 * j + 1], d, gb[e]);
         }
+    }
+    if (Xdd) {                                   // NEXT-1: divergence-damping flux of this substep (k_dd3), Eq. 33's extra term
+        double fa[E], fb[E];
+        const double* xe = Xdd + size_t(L.col) * (size_t(XF) * NVP) + L.k0;
+        ld_nc<E>(xe + X_FA * NVP, fa); ld_nc<E>(xe + X_FB * NVP, fb);
+#pragma unroll
+        for (int e = 0; e < E; ++e) { sa[e] += fa[e]; sb[e] += fb[e]; }
     }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -1128,6 +1144,267 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, double dt, Tune tn) {
     }
     st_row<E>(me + F_RHON * NVP, rho); st_row<E>(me + F_PN * NVP, p);
     st_row<E>(me + F_VXN * NVP, vx);   st_row<E>(me + F_VYN * NVP, vy); st_row<E>(me + F_VZN * NVP, vz);
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-1 (section 4 of the paper, Eq. 43-50; readings RD1-RD5 of DESIGN.md): explicit fourth-order
+// hyper-diffusion of rho, v_h (Cartesian components), v_r and T per Runge-Kutta stage, and the 3-D
+// divergence damping per acoustic substep.  Every nabla_h^2 is the 7-point stencil of L369-L371
+// (Geom::wlap).  Work rows live in a second slab X[column][XF][layer], allocated only when a
+// diffusion coefficient is set; the base path and its slab are untouched.
+// ---------------------------------------------------------------------------------------------
+
+template <int G, int E>
+__device__ __forceinline__ void lap_gather(const double* base, size_t stride, const int (&nb)[6], const double (&w)[6],
+                                           int self, int k0, double (&out)[E]) {   // sum_j w_j (s_j - s_self), unit sphere
+    double s0[E];
+    ld_nc<E>(base + size_t(self) * stride + k0, s0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) out[e] = 0.0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        double sj[E];
+        ld_nc<E>(base + size_t(nb[j]) * stride + k0, sj);
+#pragma unroll
+        for (int e = 0; e < E; ++e) out[e] = fma(w[j], sj[e] - s0[e], out[e]);
+    }
+}
+__device__ __forceinline__ void ld_lap_weights(const Geom& g, int col, int (&nb)[6], double (&w)[6]) {
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    nb[0] = n03.x; nb[1] = n03.y; nb[2] = n03.z; nb[3] = n03.w; nb[4] = n47.x; nb[5] = n47.y;
+    const double2* wp = reinterpret_cast<const double2*>(g.wlap + size_t(col) * 8);
+    const double2 a = __ldg(wp), b = __ldg(wp + 1), c = __ldg(wp + 2);
+    w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x; w[5] = c.y;
+}
+
+// column-local: the diffused quantities of the stage reference state
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_diff0(Geom g, const double* __restrict__ S, double* __restrict__ X) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    const double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
+    double* xe = X + size_t(L.col) * (size_t(XF) * NVP) + L.k0;
+    double rho[E], rb[E], v[E], W[E], p[E];
+    ld_nc<E>(me + F_RHOT * NVP, rho); ld_nc<E>(me + F_WT * NVP, W); ld_nc<E>(me + F_PT * NVP, p);
+    below<G, E>(rho, rb, L.gl, 1.0);
+    const int fv[3] = {F_VXT, F_VYT, F_VZT};
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        ld_nc<E>(me + fv[j] * NVP, v);
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = v[e] / rho[e];
+        st_row<E>(xe + (X_VX + j) * NVP, v);
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = L.k0 + e;
+        v[e] = (k >= 1 && k < g.nv) ? W[e] / (0.5 * (rb[e] + rho[e])) : 0.0;       // w on interior interfaces
+    }
+    st_row<E>(xe + X_W * NVP, v);
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = p[e] / (g.Rd * rho[e]);
+    st_row<E>(xe + X_T * NVP, v);
+}
+
+// first Laplacian, weighted for the second: q = lap(rho) | rho lap(v_j) | rho_h lap(w) | rho lap(T)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_diff1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
+    int nb[6]; double w[6];
+    ld_lap_weights(g, L.col, nb, w);
+    double* xe = X + size_t(L.col) * XREC + L.k0;
+    double rho[E], rb[E], ri[E], rhi[E], q[E];
+    ld_nc<E>(S + size_t(L.col) * REC + L.k0 + F_RHOT * NVP, rho);
+    below<G, E>(rho, rb, L.gl, 1.0);
+    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.rhinv + L.k0, rhi);
+    lap_gather<G, E>(S + F_RHOT * NVP, REC, nb, w, L.col, L.k0, q);
+#pragma unroll
+    for (int e = 0; e < E; ++e) q[e] = q[e] * ri[e] * ri[e];
+    st_row<E>(xe + X_Q0 * NVP, q);
+    const int src[4] = {X_VX, X_VY, X_VZ, X_T}, dst[4] = {X_Q1, X_Q2, X_Q3, X_Q5};
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+        lap_gather<G, E>(X + src[f] * NVP, XREC, nb, w, L.col, L.k0, q);
+#pragma unroll
+        for (int e = 0; e < E; ++e) q[e] = rho[e] * (q[e] * ri[e] * ri[e]);
+        st_row<E>(xe + dst[f] * NVP, q);
+    }
+    lap_gather<G, E>(X + X_W * NVP, XREC, nb, w, L.col, L.k0, q);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = L.k0 + e;
+        q[e] = (k >= 1 && k < g.nv) ? (0.5 * (rb[e] + rho[e])) * (q[e] * rhi[e] * rhi[e]) : 0.0;
+    }
+    st_row<E>(xe + X_Q4 * NVP, q);
+}
+
+// second Laplacian; the fluxes are added to the slow terms of the stage (RD2, RD3)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
+    int nb[6]; double w[6];
+    ld_lap_weights(g, L.col, nb, w);
+    double* me = S + size_t(L.col) * REC + L.k0;
+    const double gam = g.Cp / (g.Cp - g.Rd);
+    double ri[E], rhi[E], q[E], t[E];
+    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.rhinv + L.k0, rhi);
+    auto real = [&](int e) { return (L.k0 + e < g.nv) && (L.col < g.N); };
+    // density
+    lap_gather<G, E>(X + X_Q0 * NVP, XREC, nb, w, L.col, L.k0, q);
+    ld_rw<E>(me + F_SRHO * NVP, t);
+#pragma unroll
+    for (int e = 0; e < E; ++e) t[e] = real(e) ? t[e] + (-Kd * (q[e] * ri[e] * ri[e])) : 0.0;
+    st_row<E>(me + F_SRHO * NVP, t);
+    // horizontal momentum: Cartesian flux, Eq. 28, tangent components
+    double Fx[E], Fy[E], Fz[E];
+    lap_gather<G, E>(X + X_Q1 * NVP, XREC, nb, w, L.col, L.k0, Fx);
+    lap_gather<G, E>(X + X_Q2 * NVP, XREC, nb, w, L.col, L.k0, Fy);
+    lap_gather<G, E>(X + X_Q3 * NVP, XREC, nb, w, L.col, L.k0, Fz);
+    const double3 rh = ld_rhat(g.rhat, L.col);
+    const Basis B = ld_basis(g.basis, L.col);
+    double sa[E], sb[E];
+    ld_rw<E>(me + F_SVA * NVP, sa); ld_rw<E>(me + F_SVB * NVP, sb);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const double s2 = ri[e] * ri[e];
+        double fx = -Kd * (Fx[e] * s2), fy = -Kd * (Fy[e] * s2), fz = -Kd * (Fz[e] * s2);
+        const double fr = fx * rh.x + fy * rh.y + fz * rh.z;
+        fx -= fr * rh.x; fy -= fr * rh.y; fz -= fr * rh.z;
+        sa[e] = real(e) ? sa[e] + (fx * B.e1.x + fy * B.e1.y + fz * B.e1.z) : 0.0;
+        sb[e] = real(e) ? sb[e] + (fx * B.e2.x + fy * B.e2.y + fz * B.e2.z) : 0.0;
+    }
+    st_row<E>(me + F_SVA * NVP, sa); st_row<E>(me + F_SVB * NVP, sb);
+    // vertical momentum on interior interfaces
+    lap_gather<G, E>(X + X_Q4 * NVP, XREC, nb, w, L.col, L.k0, q);
+    ld_rw<E>(me + F_SW * NVP, t);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int k = L.k0 + e;
+        t[e] = (k >= 1 && k < g.nv && L.col < g.N) ? t[e] + (-Kd * (q[e] * rhi[e] * rhi[e])) : 0.0;
+    }
+    st_row<E>(me + F_SW * NVP, t);
+    // pressure and, through Eq. 24, rho*theta
+    lap_gather<G, E>(X + X_Q5 * NVP, XREC, nb, w, L.col, L.k0, q);
+    double p[E], u[E];
+    ld_nc<E>(me + F_PT * NVP, p);
+    ld_rw<E>(me + F_SP * NVP, t); ld_rw<E>(me + F_SRT * NVP, u);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const double Fp = -g.Rd * Kd * (q[e] * ri[e] * ri[e]);
+        t[e] = real(e) ? t[e] + Fp : 0.0;
+        u[e] = real(e) ? u[e] + Fp * eos_rt(p[e], g.Rd, g.p_ref, 1.0 / gam) / (gam * p[e]) : 0.0;
+    }
+    st_row<E>(me + F_SP * NVP, t); st_row<E>(me + F_SRT * NVP, u);
+}
+
+// divergence damping, step 1: D3 = div_h(V^[t] + V*) + D_c[W^[t] + W*]  (RD4)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
+    const double* me = S + size_t(L.col) * REC + L.k0;
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    const double* wc = g.wdiv + size_t(L.col) * 24;
+    const double* wt = g.wdiv2 + size_t(L.col) * 16;
+    double d[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) d[e] = 0.0;
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+        const double* q = S + size_t(nb[j]) * REC + L.k0;
+        double x[E], y[E], z[E], a[E], b[E];
+        ld_nc<E>(q + F_VXT * NVP, x); ld_nc<E>(q + F_VYT * NVP, y); ld_nc<E>(q + F_VZT * NVP, z);
+        ld_nc<E>(q + F_VAS * NVP, a); ld_nc<E>(q + F_VBS * NVP, b);
+        const double wx = __ldg(wc + 3 * j), wy = __ldg(wc + 3 * j + 1), wz = __ldg(wc + 3 * j + 2);
+        const double wa = __ldg(wt + 2 * j), wb = __ldg(wt + 2 * j + 1);
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+            d[e] += fma(wx, x[e], fma(wy, y[e], wz * z[e])) + fma(wa, a[e], wb * b[e]);
+    }
+    double ri[E], dlo[E], dhi[E], W[E], Ws[E], Wup[E];
+    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
+    ld_nc<E>(me + F_WT * NVP, W); ld_nc<E>(me + F_WS * NVP, Ws);
+#pragma unroll
+    for (int e = 0; e < E; ++e) W[e] += Ws[e];
+    above<G, E>(W, Wup, L.gl, 0.0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) d[e] = d[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * W[e]);
+    st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d);
+}
+
+// step 2: G = grad_h D3 (Eq. 7, projected), Cartesian
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_dd2(Geom g, double* __restrict__ X) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t XREC = size_t(XF) * NVP;
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    const double* wg = g.wgrad + size_t(L.col) * 18;
+    double* xe = X + size_t(L.col) * XREC + L.k0;
+    double s0[E], gx[E], gy[E], gz[E], ri[E];
+    ld_nc<E>(xe + X_D3 * NVP, s0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) gx[e] = gy[e] = gz[e] = 0.0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        double sj[E];
+        ld_nc<E>(X + size_t(nb[j]) * XREC + L.k0 + X_D3 * NVP, sj);
+        const double wx = __ldg(wg + 3 * j), wy = __ldg(wg + 3 * j + 1), wz = __ldg(wg + 3 * j + 2);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double dd = sj[e] - s0[e];
+            gx[e] = fma(wx, dd, gx[e]); gy[e] = fma(wy, dd, gy[e]); gz[e] = fma(wz, dd, gz[e]);
+        }
+    }
+    ld_nc<E>(g.rinv + L.k0, ri);
+#pragma unroll
+    for (int e = 0; e < E; ++e) { gx[e] *= ri[e]; gy[e] *= ri[e]; gz[e] *= ri[e]; }
+    st_row<E>(xe + X_GX * NVP, gx); st_row<E>(xe + X_GY * NVP, gy); st_row<E>(xe + X_GZ * NVP, gz);
+}
+
+// step 3: F_dd = -K_d lap(G_j) per Cartesian component, Eq. 28, tangent components
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_dd3(Geom g, double* __restrict__ X, double Kd) {
+    Map<G, E> L;
+    constexpr int NVP = Map<G, E>::NVP;
+    constexpr size_t XREC = size_t(XF) * NVP;
+    int nb[6]; double w[6];
+    ld_lap_weights(g, L.col, nb, w);
+    double Fx[E], Fy[E], Fz[E], ri[E], fa[E], fb[E];
+    lap_gather<G, E>(X + X_GX * NVP, XREC, nb, w, L.col, L.k0, Fx);
+    lap_gather<G, E>(X + X_GY * NVP, XREC, nb, w, L.col, L.k0, Fy);
+    lap_gather<G, E>(X + X_GZ * NVP, XREC, nb, w, L.col, L.k0, Fz);
+    ld_nc<E>(g.rinv + L.k0, ri);
+    const double3 rh = ld_rhat(g.rhat, L.col);
+    const Basis B = ld_basis(g.basis, L.col);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const double s2 = ri[e] * ri[e];
+        double fx = -Kd * (Fx[e] * s2), fy = -Kd * (Fy[e] * s2), fz = -Kd * (Fz[e] * s2);
+        const double fr = fx * rh.x + fy * rh.y + fz * rh.z;
+        fx -= fr * rh.x; fy -= fr * rh.y; fz -= fr * rh.z;
+        const bool real = (L.k0 + e < g.nv) && (L.col < g.N);
+        fa[e] = real ? fx * B.e1.x + fy * B.e1.y + fz * B.e1.z : 0.0;
+        fb[e] = real ? fx * B.e2.x + fy * B.e2.y + fz * B.e2.z : 0.0;
+    }
+    double* xe = X + size_t(L.col) * XREC + L.k0;
+    st_row<E>(xe + X_FA * NVP, fa); st_row<E>(xe + X_FB * NVP, fb);
 }
 
 // ---------------------------------------------------------------------------------------------
