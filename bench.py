@@ -238,6 +238,21 @@ def run_cuda(args):
         sampler.stop_flag.set()
         sampler.join()
 
+        # NEXT-1 switched on (hyper-diffusion + divergence damping, the paper's hot-Jupiter D): same step, extra kernels
+        state.set(*host)
+        state.set_diffusion(0.01992)
+        for _ in range(3):
+            state.step(1, dt, n, forcing)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(stream)
+        for _ in range(5):
+            state.step(1, dt, n, forcing)
+        b.record(stream)
+        torch.cuda.synchronize()
+        next1_ms = a.elapsed_time(b) / 5
+        state.set_diffusion(0.0, 0.0)
+
         # end to end through the public API with host buffers: upload, step, download every step
         state.set(*host)
         pinned = [torch.from_numpy(a).pin_memory() for a in host]
@@ -299,6 +314,8 @@ def run_cuda(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
             "gpu_launches": int(launches), "roofline": roofline,
+            "next1": {"what": "the same large step with NEXT-1 on (hyper-diffusion + 3-D divergence damping, D = 0.01992)",
+                      "ms_per_step": next1_ms, "cell_updates_per_s": cells_per_step / (next1_ms * 1e-3)},
             "operators": {"what": "config 1 stencils alone on this grid (level %d x %d), device arrays, 32 B/cell + geometry" % (cfg["level"], nv),
                           "div_ms": div_ms, "div_GBs": (cells * 32 + N * 224) / (div_ms * 1e-3) / 1e9,
                           "grad_ms": grad_ms, "grad_GBs": (cells * 32 + N * 176) / (grad_ms * 1e-3) / 1e9,

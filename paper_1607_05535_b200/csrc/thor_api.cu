@@ -348,12 +348,12 @@ int launch_vertical_staged(const Geom& g, const DeviceGeom& d, double* S, double
     return THOR_OK;
 }
 int launch_vertical(const thor_grid* grid, const Geom& g, double* S, double delta, int first, const TunePair& tn,
-                    cudaStream_t st) {
+                    cudaStream_t st, double* Xdd = nullptr) {
     const Shape sh = shape_for(g.nv);
     const DeviceGeom& d = grid->d;
     bool done = false;
     int rc = THOR_OK;
-    if (tn.tma_stages >= 1 && sh.E == 2) {
+    if (tn.tma_stages >= 1 && sh.E == 2 && !Xdd) {
         const bool two = tn.tma_stages >= 2;
         if (sh.G == 4) rc = two ? launch_vertical_staged<4, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<4, 1>(g, d, S, delta, first, tn, st, &done);
         else if (sh.G == 8) rc = two ? launch_vertical_staged<8, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<8, 1>(g, d, S, delta, first, tn, st, &done);
@@ -361,7 +361,8 @@ int launch_vertical(const thor_grid* grid, const Geom& g, double* S, double delt
         else rc = two ? launch_vertical_staged<32, 2>(g, d, S, delta, first, tn, st, &done) : launch_vertical_staged<32, 1>(g, d, S, delta, first, tn, st, &done);
         if (rc || done) return rc;
     }
-    THOR_DISPATCH(k_vertical, g.nv, g.Npad, st, g, S, delta, first, tn.k2);
+    if (Xdd) THOR_DISPATCH(k_vertical_dd, g.nv, g.Npad, st, g, S, delta, first, tn.k2, Xdd);
+    else THOR_DISPATCH(k_vertical, g.nv, g.Npad, st, g, S, delta, first, tn.k2);
     return THOR_OK;
 }
 
@@ -512,16 +513,16 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
             THOR_DISPATCH(k_diff1, nv, Npad, st, g, S, s->X);
             THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp);
         }
+        if (Kd_div > 0.0) THOR_DISPATCH(k_dd1, nv, Npad, st, g, S, s->X);   // D3^[t] and the first substep's D3
         for (int sub = 0; sub < ns; ++sub) {
             if (Kd_div > 0.0) {                                        // Fig. 6 small-step 1 (NEXT-1)
-                THOR_DISPATCH(k_dd1, nv, Npad, st, g, S, s->X);
                 THOR_DISPATCH(k_dd2, nv, Npad, st, g, s->X);
                 THOR_DISPATCH(k_dd3, nv, Npad, st, g, s->X, Kd_div);
             }
             THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1), Kd_div > 0.0 ? s->X : nullptr);
             TunePair t2 = tn;
             t2.k2 = dir(tn.k2);
-            if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st)) return rc;
+            if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
         }
     }
     THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, dt, dir(tn.ks));

@@ -53,7 +53,7 @@ enum XField : int {
     X_VX = 0, X_VY, X_VZ, X_W, X_T,              // k_diff0: v = V/rho, w = W/I_h[rho], T = p/(Rd rho) of Phi^[t]
     X_Q0, X_Q1, X_Q2, X_Q3, X_Q4, X_Q5,          // k_diff1: lap(rho), rho lap(v_x..z), rho_h lap(w), rho lap(T)
     XF,
-    X_D3 = 0, X_GX = 1, X_GY = 2, X_GZ = 3, X_FA = 4, X_FB = 5    // divergence damping reuses rows 0-5 during the substeps
+    X_D3 = 0, X_GX = 1, X_GY = 2, X_GZ = 3, X_FA = 4, X_FB = 5, X_D3T = 6   // divergence damping reuses rows 0-6 during the substeps
 };
 
 struct Geom {                 // device pointers, device column order, padded to Npad columns
@@ -864,10 +864,13 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn, const double* 
 // stage a TMA bulk copy has filled (k_vertical_tma); neighbours are always gathered from global
 // memory (L1/L2 hits).  wdv: the column's 21 divergence weights in shared memory.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E>
+// DD (NEXT-1 with divergence damping on): also emit the 3-D divergence of the momentum this substep
+// leaves, D3 = D3^[t] + div_h(V*')/r + D_c[W'], which the next substep's damping needs -- the two
+// terms are already in registers here; xd points at row 0 (layer k0) of the column's X record.
+template <int G, int E, bool DD = false>
 __device__ __forceinline__ void vertical_column(const Geom& g, double* __restrict__ me, const double* own,
                                                 const double* const (&nbp)[6], const double* wdv,
-                                                int gl, int k0, double delta, int first) {
+                                                int gl, int k0, double delta, int first, double* xd = nullptr) {
     constexpr int NVP = G * E;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
 
@@ -954,11 +957,18 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
     }
     st_row<E>(me + F_WS * NVP, Wn);   st_row<E>(me + F_RHOS * NVP, rho_s);
     st_row<E>(me + F_RTS * NVP, rts); st_row<E>(me + F_PS * NVP, p_s);
+    if constexpr (DD) {
+        double d3[E];
+        ld_nc<E>(xd + X_D3T * NVP, d3);
+#pragma unroll
+        for (int e = 0; e < E; ++e) d3[e] += divV[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * Wn[e]);
+        st_row<E>(xd + X_D3 * NVP, d3);
+    }
 }
 
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
+template <int G, int E, bool DD>
+__device__ __forceinline__ void vertical_block(const Geom& g, double* __restrict__ S, double delta, int first, const Tune& tn,
+                                               double* __restrict__ Xdd) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, F_PT + 1);
@@ -973,7 +983,21 @@ k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
                                   S + size_t(n03.w) * REC + L.k0, S + size_t(n47.x) * REC + L.k0, S + size_t(n47.y) * REC + L.k0};
     __syncwarp();
     double* me = S + size_t(L.col) * REC + L.k0;
-    vertical_column<G, E>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first);
+    if constexpr (DD)
+        vertical_column<G, E, true>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first, Xdd + size_t(L.col) * (size_t(XF) * Map<G, E>::NVP) + L.k0);
+    else
+        vertical_column<G, E>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
+    vertical_block<G, E, false>(g, S, delta, first, tn, nullptr);
+}
+// the same kernel with NEXT-1's divergence damping on: also writes D3 for the next substep (vertical_column<.., DD>)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_vertical_dd(Geom g, double* __restrict__ S, double delta, int first, Tune tn, double* __restrict__ Xdd) {
+    vertical_block<G, E, true>(g, S, delta, first, tn, Xdd);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1305,7 +1329,8 @@ k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd)
     st_row<E>(me + F_SP * NVP, t); st_row<E>(me + F_SRT * NVP, u);
 }
 
-// divergence damping, step 1: D3 = div_h(V^[t] + V*) + D_c[W^[t] + W*]  (RD4)
+// divergence damping, once per stage: D3^[t] = div_h(V^[t]) + D_c[W^[t]] (constant over the stage) and the
+// first substep's D3 = D3^[t] + div_h(V*(0)) + D_c[W*(0)]  (RD4); later substeps get D3 from the column-solve kernel
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
@@ -1318,9 +1343,9 @@ k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
     const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
     const double* wc = g.wdiv + size_t(L.col) * 24;
     const double* wt = g.wdiv2 + size_t(L.col) * 16;
-    double d[E];
+    double d[E], ds[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = 0.0;
+    for (int e = 0; e < E; ++e) d[e] = ds[e] = 0.0;
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
         const double* q = S + size_t(nb[j]) * REC + L.k0;
@@ -1330,17 +1355,21 @@ k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
         const double wx = __ldg(wc + 3 * j), wy = __ldg(wc + 3 * j + 1), wz = __ldg(wc + 3 * j + 2);
         const double wa = __ldg(wt + 2 * j), wb = __ldg(wt + 2 * j + 1);
 #pragma unroll
-        for (int e = 0; e < E; ++e)
-            d[e] += fma(wx, x[e], fma(wy, y[e], wz * z[e])) + fma(wa, a[e], wb * b[e]);
+        for (int e = 0; e < E; ++e) {
+            d[e] += fma(wx, x[e], fma(wy, y[e], wz * z[e]));
+            ds[e] += fma(wa, a[e], wb * b[e]);
+        }
     }
     double ri[E], dlo[E], dhi[E], W[E], Ws[E], Wup[E];
     ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
     ld_nc<E>(me + F_WT * NVP, W); ld_nc<E>(me + F_WS * NVP, Ws);
-#pragma unroll
-    for (int e = 0; e < E; ++e) W[e] += Ws[e];
     above<G, E>(W, Wup, L.gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) d[e] = d[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * W[e]);
+    st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3T * NVP, d);
+    above<G, E>(Ws, Wup, L.gl, 0.0);
+#pragma unroll
+    for (int e = 0; e < E; ++e) d[e] += ds[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * Ws[e]);
     st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d);
 }
 
