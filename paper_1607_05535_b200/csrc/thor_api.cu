@@ -50,6 +50,9 @@ struct DeviceGeom {
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr, *rhinv = nullptr;
     // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
     int tcol = 0, hmax = 0;
+    // NEXT-1 divergence damping as ONE stencil: -lap(grad D3) composed on the host over the two rings of a column
+    int* dd_idx = nullptr;            // [Npad][20] the 18 columns of the two rings (pads: the column itself)
+    double* dd_coef = nullptr;        // [Npad][20][2] tangent-basis coefficients of (D3_m - D3_i), unit sphere (x -K_d / r^3)
     int* tile_halo = nullptr;
     unsigned char* tile_slots = nullptr;
 };
@@ -156,6 +159,54 @@ int ensure_device_geom(const thor_grid* grid) {
         for (int k = 0; k < h.nv; ++k) rh[k] = 1.0 / (h.P.radius + k * h.dz);
         if ((rc = upload(&d.rhinv, padded(rh)))) return rc;
     }
+    {   // composed operator of the divergence damping (RD4): F_i = -K_d P_i lap(grad D3)_i
+        //   grad D3 at column c:  G_c = sum_j wgrad_cj (D3_nbr(c,j) - D3_c)
+        //   lap of each Cartesian component: sum_c wlap_ic (G_c - G_i), then Eq. 28 at i and its tangent basis
+        std::vector<int> idx(size_t(Npad) * 20);
+        std::vector<double> coef(size_t(Npad) * 40, 0.0);
+        for (int i = 0; i < Npad; ++i) {
+            int* id = &idx[size_t(i) * 20];
+            std::fill(id, id + 20, i);
+            if (i >= N) continue;
+            int cnt = 0;
+            double acc[20][3] = {};
+            double self[3] = {0, 0, 0};                               // coefficient of D3_i itself (minus the sum of the others)
+            auto add = [&](int m, double sx, double sy, double sz) {
+                if (m == i) { self[0] += sx; self[1] += sy; self[2] += sz; return; }
+                int q = 0;
+                while (q < cnt && id[q] != m) ++q;
+                if (q == cnt) id[cnt++] = m;
+                acc[q][0] += sx; acc[q][1] += sy; acc[q][2] += sz;
+            };
+            auto add_grad = [&](int c, double scale) {               // scale * G_c expanded on the D3 values
+                for (int j = 0; j < 6; ++j) {
+                    const double* wg = &wgrad[size_t(c) * 18 + 3 * j];
+                    const int m = nbr[size_t(c) * 8 + j];
+                    add(m, scale * wg[0], scale * wg[1], scale * wg[2]);
+                    add(c, -scale * wg[0], -scale * wg[1], -scale * wg[2]);
+                }
+            };
+            double lsum = 0.0;
+            for (int k = 0; k < 6; ++k) {
+                const double L = wlap[size_t(i) * 8 + k];
+                add_grad(nbr[size_t(i) * 8 + k], L);
+                lsum += L;
+            }
+            add_grad(i, -lsum);
+            const double* r = &rhat[size_t(i) * 4];
+            const double* b = &basis[size_t(i) * 8];
+            for (int q = 0; q < cnt; ++q) {
+                double v[3] = {acc[q][0], acc[q][1], acc[q][2]};
+                const double vr = v[0] * r[0] + v[1] * r[1] + v[2] * r[2];
+                for (int d2 = 0; d2 < 3; ++d2) v[d2] -= vr * r[d2];
+                coef[size_t(i) * 40 + 2 * q] = v[0] * b[0] + v[1] * b[1] + v[2] * b[2];
+                coef[size_t(i) * 40 + 2 * q + 1] = v[0] * b[3] + v[1] * b[4] + v[2] * b[5];
+            }
+            (void)self;                                               // difference form: applied to D3_m - D3_i
+        }
+        if ((rc = upload(&d.dd_idx, idx))) return rc;
+        if ((rc = upload(&d.dd_coef, coef))) return rc;
+    }
     {   // tile tables: halo columns of every tile and, per column, the slot of each neighbour
         const Shape sh = shape_for(h.nv);
         const int TC = kTmaWarps * (32 / sh.G), ntiles = Npad / TC;
@@ -198,6 +249,7 @@ Geom make_geom(const thor_grid* grid) {
     g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
     g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
     g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
+    g.dd_idx = d.dd_idx; g.dd_coef = d.dd_coef;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
     g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
@@ -409,7 +461,7 @@ void thor_grid_destroy(thor_grid* grid) {
     if (d.ready) {
         cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
         cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc); cudaFree(d.rhinv);
-        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap);
+        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.dd_idx); cudaFree(d.dd_coef); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap);
     }
     delete grid;
 }
@@ -515,11 +567,8 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         }
         if (Kd_div > 0.0) THOR_DISPATCH(k_dd1, nv, Npad, st, g, S, s->X);   // D3^[t] and the first substep's D3
         for (int sub = 0; sub < ns; ++sub) {
-            if (Kd_div > 0.0) {                                        // Fig. 6 small-step 1 (NEXT-1)
-                THOR_DISPATCH(k_dd2, nv, Npad, st, g, s->X);
-                THOR_DISPATCH(k_dd3, nv, Npad, st, g, s->X, Kd_div);
-            }
-            THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1), Kd_div > 0.0 ? s->X : nullptr);
+            if (Kd_div > 0.0) THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div);   // + Fig. 6 small-step 1
+            else THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
             TunePair t2 = tn;
             t2.k2 = dir(tn.k2);
             if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
@@ -622,7 +671,7 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     const TunePair tn = tune();
     auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
     for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1), (const double*)nullptr);
+        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1));
         TunePair t2 = tn;
         if (which & 2) t2.k2 = dir(tn.k2);
         if (which & 2)

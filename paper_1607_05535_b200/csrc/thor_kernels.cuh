@@ -53,7 +53,7 @@ enum XField : int {
     X_VX = 0, X_VY, X_VZ, X_W, X_T,              // k_diff0: v = V/rho, w = W/I_h[rho], T = p/(Rd rho) of Phi^[t]
     X_Q0, X_Q1, X_Q2, X_Q3, X_Q4, X_Q5,          // k_diff1: lap(rho), rho lap(v_x..z), rho_h lap(w), rho lap(T)
     XF,
-    X_D3 = 0, X_GX = 1, X_GY = 2, X_GZ = 3, X_FA = 4, X_FB = 5, X_D3T = 6   // divergence damping reuses rows 0-6 during the substeps
+    X_D3 = 0, X_D3T = 1          // divergence damping reuses rows 0-1 during the substeps
 };
 
 struct Geom {                 // device pointers, device column order, padded to Npad columns
@@ -62,6 +62,8 @@ struct Geom {                 // device pointers, device column order, padded to
     const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad
     const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)
     const double* wlap;       // [Npad][8]   6 Laplacian weights (Eq. 7 on the triangles, then Eq. 6; L369-L371), 2 pad
+    const int* dd_idx;        // [Npad][20]  NEXT-1 divergence damping composed over two rings: columns m ...
+    const double* dd_coef;    // [Npad][20][2] ... and tangent coefficients of (D3_m - D3_i); F_dd = -K_d/r^3 sum_m coef_m (D3_m - D3_i)
     const double* rhat;       // [Npad][4]   unit vector of the column, 1 pad
     const double* basis;      // [Npad][8]   tangent basis e1(3), e2(3), 2 pad
     const double* wdiv2;      // [Npad][16]  7 x 2 divergence weights contracted with the basis of column j, 2 pad
@@ -797,9 +799,9 @@ k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
 // K1 (a4): explicit horizontal momentum, Eq. 33 (Fig. 6 small-step 2):
 //   V*' = V* + delta (-grad_h p* / r + slowV).  Gathers p* from the 6 neighbours.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd) {
+template <int G, int E, bool DD>
+__device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict__ S, double delta, const Tune& tn,
+                                               const double* __restrict__ Xdd, double Kd_div) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -836,12 +838,33 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn, const double* 
             ga[e] = fma(wgv[2 * j], d, ga[e]); gb[e] = fma(wgv[2 * j + 1], d, gb[e]);
         }
     }
-    if (Xdd) {                                   // NEXT-1: divergence-damping flux of this substep (k_dd3), Eq. 33's extra term
-        double fa[E], fb[E];
-        const double* xe = Xdd + size_t(L.col) * (size_t(XF) * NVP) + L.k0;
-        ld_nc<E>(xe + X_FA * NVP, fa); ld_nc<E>(xe + X_FB * NVP, fb);
+    if constexpr (DD) {
+        // NEXT-1, Fig. 6 small-step 1: divergence damping F_dd = -K_d lap(grad_h D3) (RD4) as ONE two-ring
+        // stencil on the D3 row (composed on the host: thor_api.cu), already projected and in the tangent basis
+        constexpr size_t XREC = size_t(XF) * NVP;
+        const int* di = g.dd_idx + size_t(L.col) * 20;
+        const double2* dc = reinterpret_cast<const double2*>(g.dd_coef + size_t(L.col) * 40);
+        double d0[E], fa[E], fb[E];
+        ld_nc<E>(Xdd + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d0);
 #pragma unroll
-        for (int e = 0; e < E; ++e) { sa[e] += fa[e]; sb[e] += fb[e]; }
+        for (int e = 0; e < E; ++e) fa[e] = fb[e] = 0.0;
+#pragma unroll 6
+        for (int q = 0; q < 18; ++q) {
+            const int m = __ldg(di + q);
+            const double2 c = __ldg(dc + q);
+            double dm[E];
+            ld_nc<E>(Xdd + size_t(m) * XREC + L.k0 + X_D3 * NVP, dm);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const double dd = dm[e] - d0[e];
+                fa[e] = fma(c.x, dd, fa[e]); fb[e] = fma(c.y, dd, fb[e]);
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double sc = -Kd_div * (ri[e] * ri[e] * ri[e]);
+            sa[e] += sc * fa[e]; sb[e] += sc * fb[e];
+        }
     }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -849,6 +872,17 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn, const double* 
         vb[e] = fma(delta, sb[e] - gb[e] * ri[e], vb[e]);
     }
     st_row<E>(me + F_VAS * NVP, va); st_row<E>(me + F_VBS * NVP, vb);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
+    momentum_block<G, E, false>(g, S, delta, tn, nullptr, 0.0);
+}
+// the same kernel with NEXT-1's divergence damping added to Eq. 33
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_momentum_dd(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div) {
+    momentum_block<G, E, true>(g, S, delta, tn, Xdd, Kd_div);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1371,69 +1405,6 @@ k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
 #pragma unroll
     for (int e = 0; e < E; ++e) d[e] += ds[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * Ws[e]);
     st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d);
-}
-
-// step 2: G = grad_h D3 (Eq. 7, projected), Cartesian
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_dd2(Geom g, double* __restrict__ X) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t XREC = size_t(XF) * NVP;
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    const double* wg = g.wgrad + size_t(L.col) * 18;
-    double* xe = X + size_t(L.col) * XREC + L.k0;
-    double s0[E], gx[E], gy[E], gz[E], ri[E];
-    ld_nc<E>(xe + X_D3 * NVP, s0);
-#pragma unroll
-    for (int e = 0; e < E; ++e) gx[e] = gy[e] = gz[e] = 0.0;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-        double sj[E];
-        ld_nc<E>(X + size_t(nb[j]) * XREC + L.k0 + X_D3 * NVP, sj);
-        const double wx = __ldg(wg + 3 * j), wy = __ldg(wg + 3 * j + 1), wz = __ldg(wg + 3 * j + 2);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const double dd = sj[e] - s0[e];
-            gx[e] = fma(wx, dd, gx[e]); gy[e] = fma(wy, dd, gy[e]); gz[e] = fma(wz, dd, gz[e]);
-        }
-    }
-    ld_nc<E>(g.rinv + L.k0, ri);
-#pragma unroll
-    for (int e = 0; e < E; ++e) { gx[e] *= ri[e]; gy[e] *= ri[e]; gz[e] *= ri[e]; }
-    st_row<E>(xe + X_GX * NVP, gx); st_row<E>(xe + X_GY * NVP, gy); st_row<E>(xe + X_GZ * NVP, gz);
-}
-
-// step 3: F_dd = -K_d lap(G_j) per Cartesian component, Eq. 28, tangent components
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_dd3(Geom g, double* __restrict__ X, double Kd) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t XREC = size_t(XF) * NVP;
-    int nb[6]; double w[6];
-    ld_lap_weights(g, L.col, nb, w);
-    double Fx[E], Fy[E], Fz[E], ri[E], fa[E], fb[E];
-    lap_gather<G, E>(X + X_GX * NVP, XREC, nb, w, L.col, L.k0, Fx);
-    lap_gather<G, E>(X + X_GY * NVP, XREC, nb, w, L.col, L.k0, Fy);
-    lap_gather<G, E>(X + X_GZ * NVP, XREC, nb, w, L.col, L.k0, Fz);
-    ld_nc<E>(g.rinv + L.k0, ri);
-    const double3 rh = ld_rhat(g.rhat, L.col);
-    const Basis B = ld_basis(g.basis, L.col);
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const double s2 = ri[e] * ri[e];
-        double fx = -Kd * (Fx[e] * s2), fy = -Kd * (Fy[e] * s2), fz = -Kd * (Fz[e] * s2);
-        const double fr = fx * rh.x + fy * rh.y + fz * rh.z;
-        fx -= fr * rh.x; fy -= fr * rh.y; fz -= fr * rh.z;
-        const bool real = (L.k0 + e < g.nv) && (L.col < g.N);
-        fa[e] = real ? fx * B.e1.x + fy * B.e1.y + fz * B.e1.z : 0.0;
-        fb[e] = real ? fx * B.e2.x + fy * B.e2.y + fz * B.e2.z : 0.0;
-    }
-    double* xe = X + size_t(L.col) * XREC + L.k0;
-    st_row<E>(xe + X_FA * NVP, fa); st_row<E>(xe + X_FB * NVP, fb);
 }
 
 // ---------------------------------------------------------------------------------------------
