@@ -17,8 +17,14 @@
  *   geometry/div/grad ........ P2 P4 P5 P6 P7 P8 P9 (closed forms, convergence order, identities)
  *   tridiagonal (orc_substep)  P10 (dense solve of the three discrete fast equations)
  *   step ..................... P11 (mass), P12 (rest state), P13 (Coriolis), P14 (RK order), P15
+ *   NEXT-1 (orc_hlap, hyper_diffusion, divergence_damping): Laplacian of a constant, flux form,
+ *                              spherical-harmonic eigenvalues, Table 1 timescales (K_d, tau_d), closed forms of
+ *                              the fluxes on simple states, mass conservation, rest state, damping acts on
+ *                              divergence only; config 2 stays smooth for its 500 steps with the paper's D
  *   PARITY UNPINNED: the discrete advection form R7, the stage convention R1, the forcing
- *   convention R9 -- the paper fixes no value for them; only the invariants above constrain them.
+ *   convention R9, and the NEXT-1 readings RD2-RD4 (which state the fluxes use, where F_p enters, the
+ *   form of the divergence-damping term; Eq. 43-46 are lost or damaged in PAPER.md) -- the paper fixes
+ *   no value for them; only the invariants above constrain them.
  */
 #include <math.h>
 #include <stdlib.h>
