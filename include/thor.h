@@ -111,6 +111,21 @@ int thor_step(thor_state *state, int n_large, double dt, int n_acoustic_substeps
  * 0 switches a term off; (0, 0), the default, is the base path.  Allocates the work rows on first use. */
 int thor_state_set_diffusion(thor_state *state, double D_hyper, double D_div);
 
+/* NEXT-2 (section 7.1, Eq. 51-55): the Held-Suarez forcing with K_v, K_T and T_eq evaluated from the
+ * EVOLVING state instead of fixed tables: sigma = p/p_s, p_s extrapolated hydrostatically and
+ * isothermally from the lowest layer centre (L390);
+ *   K_v = k_f max(0, (sigma - sigma_b)/(1 - sigma_b))                                          (Eq. 53)
+ *   T_eq = max{T_min, [T_surf - dT_y sin^2(lat) - dth_z ln(p/p_star) cos^2(lat)] (p/p_star)^(Rd/Cp)}   (Eq. 54)
+ *   K_T = k_a + (k_s - k_a) max(0, (sigma - sigma_b)/(1 - sigma_b)) cos^4(lat)                  (Eq. 55)
+ * applied with Eq. 51-52 at the end of every large step.  hs = NULL switches it off.  While it is on,
+ * thor_step must be called with forcing = NULL (THOR_EINVAL otherwise). */
+typedef struct {
+    double T_surf, dT_y, dth_z, T_min;   /* K: 315, 60 (L448), (Delta theta)_z (not printed in the paper), 200 */
+    double k_a, k_s, k_f;                /* 1/s: 1/(40 d), 1/(4 d), 1/(1 d)  (L438, L448) */
+    double sigma_b, p_star;              /* 0.7; reference pressure of Eq. 54, Pa */
+} thor_held_suarez;
+int thor_state_set_held_suarez(thor_state *state, const thor_held_suarez *hs);
+
 /* Only the hot loop: n_substeps acoustic substeps (steps a4-a9 of DESIGN.md) of length delta on the
  * stage data left by the last thor_step.  which: 1 = explicit horizontal momentum kernel only,
  * 2 = divergence + column-solve kernel only, 3 = both.  For measurement; the state it leaves is

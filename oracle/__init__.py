@@ -72,6 +72,9 @@ def _load():
         L.orc_substep.argtypes = [ctypes.c_void_p, ctypes.c_double] + [_D] * 14
         L.orc_diffusion_fluxes.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_double, _D, _D, _D, _D, _D]
         L.orc_divergence_damping.argtypes = [ctypes.c_void_p, _D, _D, ctypes.c_double, _D]
+        L.orc_step_held_suarez.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
+                                           ctypes.c_double, ctypes.c_double]
+        L.orc_forcing_held_suarez.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D]
         L.orc_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -185,6 +188,20 @@ class Geometry:
         _load().orc_divergence_damping(self._h, _p(V), _p(W), float(Kd), _p(out))
         return out
 
+    # NEXT-2: Held-Suarez forcing from the evolving sigma (Eq. 51-55); hs = HELD_SUAREZ-like dict
+    def step_held_suarez(self, rho, V, W, p, n_large, dt, n_sub, hs, D_hyp=0.0, D_div=0.0):
+        rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
+        h = _c(hs_array(hs))
+        _load().orc_step_held_suarez(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
+                                     float(D_hyp), float(D_div))
+        return rho, V, W, p
+
+    def forcing_held_suarez(self, rho, V, p, dt, hs):
+        rho, V, p = (_c(x).copy() for x in (rho, V, p))
+        h = _c(hs_array(hs))
+        _load().orc_forcing_held_suarez(self._h, float(dt), _p(rho), _p(V), _p(p), _p(h))
+        return V, p
+
     def diagnostics(self, rho, V, W, p):
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))
         m = ctypes.c_double()
@@ -247,3 +264,10 @@ def kd(D, dbar_, dt):
 
 def tau_d(dbar_, kd_):
     return float(_load().orc_tau_d(float(dbar_), float(kd_)))
+
+
+HS_KEYS = ("T_surf", "dT_y", "dth_z", "T_min", "k_a", "k_s", "k_f", "sigma_b", "p_star")
+
+
+def hs_array(hs):
+    return np.array([float(hs[k]) for k in HS_KEYS])

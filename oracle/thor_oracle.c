@@ -803,6 +803,48 @@ static void forcing(const orc_geom *G, double dt, double *rho, double *V, double
     }
 }
 
+/* NEXT-2: the Held-Suarez forcing of section 7.1 with K_v, K_T, T_eq from the EVOLVING
+ * state (Eq. 51-55): sigma = p / p_s, the surface pressure "estimated extrapolating the
+ * pressures to the surface using the hydrostatic equation and keeping the temperature constant in that
+ * region" (L390): p_s = p_0 exp(g z_0 / (Rd T_0)) from the lowest layer centre.
+ *   K_v  = k_f max(0, (sigma - sigma_b)/(1 - sigma_b))                                    (Eq. 53)
+ *   T_eq = max{T_min, [T_surf - dT_y sin^2(phi) - dth_z ln(p/p*) cos^2(phi)] (p/p*)^(Rd/Cp)}  (Eq. 54, G14)
+ *   K_T  = k_a + (k_s - k_a) max(0, (sigma - sigma_b)/(1 - sigma_b)) cos^4(phi)              (Eq. 55, G14)
+ * then Eq. 51-52 as in forcing() (R9: rho unchanged, p = rho Rd T).  phi: latitude, sin(phi) = z of the
+ * column's unit vector (rotation axis through the polar vertices, L45). */
+typedef struct { double T_surf, dT_y, dth_z, T_min, k_a, k_s, k_f, sigma_b, p_star; } orc_held_suarez;
+
+static void forcing_held_suarez(const orc_geom *G, double dt, double *rho, double *V, double *p, const orc_held_suarez *H) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double kappa = P->Rd / P->Cp;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double sphi = G->xyz[3 * i + 2], cphi2 = 1.0 - sphi * sphi;
+        size_t c0 = (size_t)i * nv;
+        const double T0 = p[c0] / (rho[c0] * P->Rd);
+        const double ps = p[c0] * exp(P->gravity * G->z_c[0] / (P->Rd * T0));                   /* L390 */
+        for (int k = 0; k < nv; k++) {
+            size_t c = c0 + k;
+            const double sigma = p[c] / ps;
+            double ramp = (sigma - H->sigma_b) / (1.0 - H->sigma_b);
+            if (ramp < 0.0) ramp = 0.0;
+            const double Kv = H->k_f * ramp;                                                     /* Eq. 53 */
+            const double pr = p[c] / H->p_star;
+            double Teq = (H->T_surf - H->dT_y * sphi * sphi - H->dth_z * log(pr) * cphi2) * pow(pr, kappa);
+            if (Teq < H->T_min) Teq = H->T_min;                                                  /* Eq. 54 */
+            const double KT = H->k_a + (H->k_s - H->k_a) * ramp * cphi2 * cphi2;                 /* Eq. 55 */
+            for (int d = 0; d < 3; d++) V[3 * c + d] = V[3 * c + d] / (1.0 + Kv * dt);           /* Eq. 51 */
+            double T = p[c] / (rho[c] * P->Rd);
+            T = (T + KT * dt * Teq) / (1.0 + KT * dt);                                           /* Eq. 52 */
+            p[c] = rho[c] * P->Rd * T;
+        }
+    }
+}
+void orc_forcing_held_suarez(const orc_geom *G, double dt, double *rho, double *V, double *p, const double *hs) {
+    forcing_held_suarez(G, dt, rho, V, p, (const orc_held_suarez *)hs);
+}
+
 /* One call = n_large large steps (Fig. 6; stage convention R1 of SURVEY O5).
  * State arrays are updated in place: rho,p [N][nv]; V [N][nv][3]; W [N][nv+1] (ends forced to 0). */
 double orc_dbar(double radius, int level);
@@ -811,6 +853,8 @@ double orc_kd(double D, double dbar, double dt);
 /* D_hyp, D_div: the non-dimensional diffusion parameter of Eq. 49 for the hyper-diffusion and for the
  * divergence damping (the paper uses the same value for both, L367); 0 switches a term off, and
  * (0, 0) is the base path of SURVEY 8(a), arithmetic untouched. */
+static const orc_held_suarez *g_hs = NULL;   /* set by orc_step_held_suarez for the duration of its call */
+
 void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
                         int n_sub, const double *T_eq, const double *k_T, const double *k_v, double D_hyp, double D_div) {
     const int N = G->N, nv = G->nv;
@@ -859,9 +903,17 @@ void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, do
             for (size_t c = 0; c < ni; c++) w->W_t[c] = w->W_t[c] + w->W_s[c];
         }
         memcpy(rho, w->rho_t, 8 * nc); memcpy(V, w->V_t, 24 * nc); memcpy(W, w->W_t, 8 * ni); memcpy(p, w->p_t, 8 * nc);
-        forcing(G, dt, rho, V, p, T_eq, k_T, k_v);
+        if (g_hs) forcing_held_suarez(G, dt, rho, V, p, g_hs);
+        else forcing(G, dt, rho, V, p, T_eq, k_T, k_v);
     }
     work_free(w);
+}
+/* hs: the nine numbers of orc_held_suarez */
+void orc_step_held_suarez(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
+                          int n_sub, const double *hs, double D_hyp, double D_div) {
+    g_hs = (const orc_held_suarez *)hs;
+    orc_step_diffusion(G, rho, V, W, p, n_large, dt, n_sub, NULL, NULL, NULL, D_hyp, D_div);
+    g_hs = NULL;
 }
 void orc_step(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
               int n_sub, const double *T_eq, const double *k_T, const double *k_v) {

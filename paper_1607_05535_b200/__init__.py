@@ -40,6 +40,10 @@ class thor_forcing(ctypes.Structure):
     _fields_ = [("T_eq", _D), ("k_T", _D), ("k_v", _D), ("resident", ctypes.c_int)]
 
 
+class thor_held_suarez(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in ("T_surf", "dT_y", "dth_z", "T_min", "k_a", "k_s", "k_f", "sigma_b", "p_star")]
+
+
 class thor_diag(ctypes.Structure):
     _fields_ = [("total_mass", ctypes.c_double), ("total_energy", ctypes.c_double)]
 
@@ -55,6 +59,7 @@ _SIGNATURES = {
     "thor_state_destroy": (None, [_V]),
     "thor_step": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(thor_forcing)]),
     "thor_state_set_diffusion": (ctypes.c_int, [_V, ctypes.c_double, ctypes.c_double]),
+    "thor_state_set_held_suarez": (ctypes.c_int, [_V, ctypes.POINTER(thor_held_suarez)]),
     "thor_acoustic_substeps": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int]),
     "thor_diagnostics": (ctypes.c_int, [_V, ctypes.POINTER(thor_diag)]),
     "thor_apply_div": (ctypes.c_int, [_V, _D, _D]),
@@ -154,6 +159,15 @@ def thor_step(state, n_large, dt, n_acoustic_substeps, forcing=None):
 
 def thor_state_set_diffusion(state, D_hyper, D_div):
     _check(load_library().thor_state_set_diffusion(state, float(D_hyper), float(D_div)))
+
+
+def thor_state_set_held_suarez(state, hs):
+    """hs: dict with the fields of thor_held_suarez, or None to switch the evolving-sigma forcing off."""
+    if hs is None:
+        _check(load_library().thor_state_set_held_suarez(state, None))
+        return
+    H = thor_held_suarez(**{k: float(hs[k]) for k, _ in thor_held_suarez._fields_})
+    _check(load_library().thor_state_set_held_suarez(state, ctypes.byref(H)))
 
 
 def thor_acoustic_substeps(state, n_substeps, delta, which=3):
@@ -283,6 +297,9 @@ class State:
     def set_diffusion(self, D_hyper, D_div=None):
         """NEXT-1: hyper-diffusion and divergence damping parameter D of Eq. 49 (D_div defaults to D_hyper, L367)."""
         thor_state_set_diffusion(self._h, D_hyper, D_hyper if D_div is None else D_div)
+
+    def set_held_suarez(self, hs):
+        thor_state_set_held_suarez(self._h, hs)
 
     def acoustic_substeps(self, n_substeps, delta, which=3):
         thor_acoustic_substeps(self._h, n_substeps, delta, which)

@@ -82,6 +82,11 @@ struct Geom {                 // device pointers, device column order, padded to
 struct Forcing {              // [Npad][NVP] each, may be null (Eq. 51-52)
     const double *T_eq, *k_T, *k_v;
 };
+// NEXT-2: Held-Suarez forcing from the evolving sigma = p/p_s (Eq. 53-55); on != 0 replaces the tables
+struct HeldSuarez {
+    int on;
+    double T_surf, dT_y, dth_z, T_min, k_a, k_s, k_f, sigma_b, p_star;
+};
 
 // L2 schedule of one launch (defaults in thor_api.cu).  Successive kernels of a
 // large step walk the columns in ALTERNATING directions, so each starts on the rows the previous one has
@@ -1150,7 +1155,7 @@ k_vertical_staged(Geom g, TileTab tt, double* __restrict__ S, double delta, int 
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_finish(Geom g, double* __restrict__ S, Forcing F, double dt, Tune tn) {
+k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, double dt, Tune tn) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -1182,7 +1187,28 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, double dt, Tune tn) {
     }
     sum(F_WT, F_WS, a);
     st_row<E>(me + F_WN * NVP, a);
-    if (F.k_v) {
+    if (H.on) {
+        // sigma = p/p_s with the surface pressure extrapolated hydrostatically and isothermally from the lowest
+        // layer centre (L390); K_v (Eq. 53), T_eq (Eq. 54, G14), K_T (Eq. 55, G14); then Eq. 51-52
+        const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
+        const double T0 = p0 / (rho0 * g.Rd);
+        const double ps = p0 * exp(g.gravity * __ldg(g.zc) / (g.Rd * T0));
+        const double sphi = ld_rhat(g.rhat, L.col).z, cphi2 = 1.0 - sphi * sphi, kappa = g.Rd / g.Cp;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double sigma = p[e] / ps;
+            const double ramp = fmax(0.0, (sigma - H.sigma_b) / (1.0 - H.sigma_b));
+            const double Kv = H.k_f * ramp;
+            const double pr = p[e] / H.p_star;
+            const double Teq = fmax(H.T_min, (H.T_surf - H.dT_y * sphi * sphi - H.dth_z * log(pr) * cphi2) * pow(pr, kappa));
+            const double KT = H.k_a + (H.k_s - H.k_a) * ramp * cphi2 * cphi2;
+            const double sv = 1.0 + Kv * dt;
+            vx[e] /= sv; vy[e] /= sv; vz[e] /= sv;                            // Eq. 51
+            double T = p[e] / (rho[e] * g.Rd);
+            T = (T + KT * dt * Teq) / (1.0 + KT * dt);                        // Eq. 52
+            p[e] = (L.k0 + e < g.nv && L.col < g.N) ? rho[e] * g.Rd * T : p[e];
+        }
+    } else if (F.k_v) {
         ld_nc<E>(F.k_v + to, a);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -1190,7 +1216,7 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, double dt, Tune tn) {
             vx[e] /= s; vy[e] /= s; vz[e] /= s;                               // Eq. 51
         }
     }
-    if (F.k_T && F.T_eq) {
+    if (!H.on && F.k_T && F.T_eq) {
         double te[E];
         ld_nc<E>(F.k_T + to, a); ld_nc<E>(F.T_eq + to, te);
 #pragma unroll

@@ -282,6 +282,77 @@ def test_next1_config2_runs_its_500_steps_with_diffusion():
     assert 250.0 < T.min() and T.max() < 320.0
 
 
+@pytest.mark.parametrize("nv", [8, 32])
+def test_next2_held_suarez_forcing_parity(nv):
+    """NEXT-2 (Eq. 51-55 with K_v, K_T, T_eq from the evolving sigma) together with NEXT-1, 5 large steps."""
+    planet = dict(ti.EARTH)
+    g, G = _setup(3, nv, planet)
+    s = _random_state(G, planet, 500 + nv)
+    D = 0.004837
+    st = thor.State(g, *s)
+    st.set_diffusion(D)
+    st.set_held_suarez(ti.HELD_SUAREZ)
+    with pytest.raises(thor.ThorError):
+        st.step(1, 600.0, 4, dict(T_eq=s[0], k_T=s[0], k_v=None))          # tables and evolving-sigma forcing are exclusive
+    st.step(5, 600.0, 4)
+    ref = G.step_held_suarez(*s, 5, 600.0, 4, ti.HELD_SUAREZ, D, D)
+    eps, rng = np.finfo(np.float64).eps, np.random.default_rng(12345)
+    pert = [a * (1.0 + eps * rng.choice([-1.0, 1.0], size=a.shape)) for a in s]
+    floor = [np.abs(x - y).max() for x, y in zip(ref, G.step_held_suarez(*pert, 5, 600.0, 4, ti.HELD_SUAREZ, D, D))]
+    _compare(st.get(), ref, 1e-11, "held-suarez nv=%d" % nv, floor, K=40.0)
+    base = G.step(*s, 5, 600.0, 4, None, D, D)
+    assert np.abs(ref[3] - base[3]).max() > 1e4 * np.abs(st.get()[3] - ref[3]).max()     # the forcing is not a no-op
+    st.set_held_suarez(None)
+    st.set(*s)
+    st.step(5, 600.0, 4)
+    _compare(st.get(), base, 1e-11, "held-suarez off nv=%d" % nv, floor, K=40.0)
+
+
+def test_held_suarez_benchmark_spins_up_midlatitude_jets():
+    """End to end (base path + NEXT-1 + NEXT-2): the paper's Earth benchmark set-up (section 7.1: level 5,
+    dt = 1000 s, n = 6, D from Table 1, rest state at 300 K, top at 32 km) integrated 250 days on the GPU.
+    The paper reports westerly jets near 250 mbar and 45 degrees latitude (L460); every reading of the
+    step (R1, R7, R8, RD1-RD5) has to be right for this to come out.  About 10 s on a B200."""
+    import torch
+    level, nv = 5, 32
+    planet = dict(ti.EARTH)
+    planet["z_top"] = 32.0e3
+    g = thor.Grid(level, nv, planet)
+    xyz, N = g.view["xyz"], g.n_cols
+    rho, V, W, p = ti.rest_state(planet, nv, N, 1.0e5, 300.0)
+    T = 300.0 + np.random.default_rng(1).uniform(-0.1, 0.1, size=rho.shape)
+    rho = p / (planet["Rd"] * T)
+    stream = torch.cuda.Stream()
+    st = thor.State(g, rho, V, W, p, cuda_stream=stream.cuda_stream)
+    st.set_diffusion(0.004837)
+    st.set_held_suarez(ti.HELD_SUAREZ)
+    m0, _ = st.diagnostics()
+    st.step(int(250 * 86400 / 1000.0), 1000.0, 6)
+    rho, V, W, p = st.get()
+    m1, _ = st.diagnostics()
+    assert all(np.all(np.isfinite(a)) for a in (rho, V, W, p))
+    assert abs(m1 - m0) <= 1e-12 * m0
+    lat = np.degrees(np.arcsin(xyz[:, 2]))
+    lon = np.arctan2(xyz[:, 1], xyz[:, 0])
+    east = np.stack([-np.sin(lon), np.cos(lon), np.zeros(N)], axis=-1)
+    u = np.sum(V * east[:, None, :], axis=-1) / rho
+    bins = np.linspace(-90, 90, 37)
+    ib = np.clip(np.digitize(lat, bins) - 1, 0, 35)
+    ubar = np.array([[u[ib == b, k].mean() for k in range(nv)] for b in range(36)])      # zonal mean [latitude band][layer]
+    pbar = p.mean(axis=0)
+    centre = 0.5 * (bins[:-1] + bins[1:])
+    for hemi in (centre < 0, centre > 0):
+        j, k = np.unravel_index(np.argmax(ubar[hemi]), ubar[hemi].shape)
+        print("jet: %.1f m/s at latitude %.0f, %.0f hPa" % (ubar[hemi][j, k], centre[hemi][j], pbar[k] / 100))
+        assert 20.0 < ubar[hemi][j, k] < 55.0                       # tens of m/s, westerly
+        assert 30.0 <= abs(centre[hemi][j]) <= 55.0                 # mid-latitudes
+        assert 120e2 < pbar[k] < 400e2                              # upper troposphere
+    assert -10.0 < ubar[17:19, 0].mean() < 0.0                      # weak surface easterlies at the equator
+    Tk = p / (planet["Rd"] * rho)
+    assert 170.0 < Tk.min() and Tk.max() < 320.0
+    g.close()
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""

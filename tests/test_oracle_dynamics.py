@@ -423,3 +423,48 @@ def test_divergence_damping_acts_on_divergence_only(ogrid):
     w = G.Ac[:, None]
     corr = (w * G.hdiv(Fd) * D3).sum() / np.sqrt((w * G.hdiv(Fd) ** 2).sum() * (w * D3 ** 2).sum())
     assert corr < -0.7
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-2: Held-Suarez forcing from the evolving sigma (Eq. 51-55)
+# --------------------------------------------------------------------------------------------
+def test_held_suarez_forcing_closed_forms(ogrid):
+    """Eq. 53-55 evaluated by hand on an isothermal hydrostatic column: the extrapolated surface pressure
+    is the column's p_s exactly (L390), so sigma = p/p_s; drag only below sigma_b = 0.7 (Eq. 53); T_eq =
+    315 K at the equator's surface pressure, 255 K at the poles', 200 K aloft (Eq. 54); with a huge
+    step the backward-Euler update lands on T_eq and on zero wind (Eq. 51-52)."""
+    import oracle
+    planet, nv = dict(ti.EARTH), 16
+    xyz, nbr, C = ogrid(2, True)
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    ps, T0 = 1.0e5, 280.0
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, ps, T0)
+    V = rho[..., None] * np.cross(np.array([0.0, 0.0, 1.0e-6])[None, None, :], xyz[:, None, :] * G.r_c[None, :, None])
+    hs = dict(ti.HELD_SUAREZ)
+    sigma = p / ps
+    lat_s = xyz[:, 2][:, None]
+    c2 = 1.0 - lat_s ** 2
+    kappa = planet["Rd"] / planet["Cp"]
+    Teq = np.maximum(200.0, (315.0 - 60.0 * lat_s ** 2 - hs["dth_z"] * np.log(p / 1e5) * c2) * (p / 1e5) ** kappa)
+    ramp = np.maximum(0.0, (sigma - 0.7) / 0.3)
+    KT = hs["k_a"] + (hs["k_s"] - hs["k_a"]) * ramp * c2 ** 2
+    Kv = hs["k_f"] * ramp
+    dt = 1200.0
+    Vn, pn = G.forcing_held_suarez(rho, V, p, dt, hs)
+    T = p / (rho * planet["Rd"])
+    Tn = (T + KT * dt * Teq) / (1.0 + KT * dt)
+    assert np.allclose(pn, rho * planet["Rd"] * Tn, rtol=1e-13, atol=0)
+    assert np.allclose(Vn, V / (1.0 + Kv * dt)[..., None], rtol=1e-13, atol=1e-300)
+    assert np.all(Vn[sigma < 0.7] == V[sigma < 0.7])                       # no drag above the boundary layer
+    # the printed landmarks of Eq. 54, on a column whose lowest layer centre sits at p = p*: with a huge step the
+    # update lands on T_eq: 315 K at the equator, 315 - 60 = 255 K at the poles, 200 K aloft; and on zero wind
+    ps2 = 1.0e5 * np.exp(planet["gravity"] * G.z_c[0] / (planet["Rd"] * T0))
+    rho2, _, _, p2 = ti.rest_state(planet, nv, G.N, ps2, T0)
+    assert abs(p2[0, 0] - 1.0e5) < 1e-6
+    eq, pole = int(np.argmin(np.abs(xyz[:, 2]))), int(np.argmax(xyz[:, 2]))
+    Vbig, pbig = G.forcing_held_suarez(rho2, V, p2, 1.0e13, hs)
+    Tbig = pbig / (rho2 * planet["Rd"])
+    assert abs(Tbig[pole, 0] - 255.0) < 1e-3
+    assert abs(Tbig[eq, 0] - (315.0 - 60.0 * xyz[eq, 2] ** 2)) < 1e-3
+    assert np.all(np.abs(Tbig[:, -1] - 200.0) < 1e-3)                                # clipped aloft (top at 36 km)
+    assert np.abs(Vbig[p2 / ps2 > 0.75]).max() < 1e-6 * np.abs(V).max()

@@ -22,6 +22,12 @@ _HJ_H = 3779.0 * 1500.0 / 9.42                       # scale height Rd T0 / g
 HOT_JUPITER = dict(radius=9.44e7, omega=2.06e-5, gravity=9.42, Rd=3779.0, Cp=13226.0, p_ref=1.0e5,
                    z_top=_HJ_H * math.log(1.0e7 / 1.0e5))
 
+# Held-Suarez forcing parameters (Eq. 53-55): k_f = 1/day, sigma_b = 0.7, k_a = 1/40 d,
+# k_s = 1/4 d, (Delta T)_y = 60 K, 315 K, 200 K are printed; (Delta theta)_z and p* are not (G14): the
+# benchmark's published 10 K and the reference pressure 1e5 Pa are used.
+HELD_SUAREZ = dict(T_surf=315.0, dT_y=60.0, dth_z=10.0, T_min=200.0, k_a=1.0 / (40 * 86400.0), k_s=1.0 / (4 * 86400.0),
+                   k_f=1.0 / 86400.0, sigma_b=0.7, p_star=1.0e5)
+
 # BASELINE.json configs (index = config number).  n_large is the run length used for parity.
 CONFIGS = {
     0: dict(name="cfg0_level4x8_earth", level=4, nv=8, planet=EARTH, p_s=1.0e5, T0=300.0,
