@@ -126,6 +126,16 @@ typedef struct {
 } thor_held_suarez;
 int thor_state_set_held_suarez(thor_state *state, const thor_held_suarez *hs);
 
+/* NEXT-2, hot Jupiter (section 7.2, Eq. 59-61): T_eq = T_vert(z) + beta_trop(sigma, z) dT_EP cos(lon) cos(lat),
+ * beta_trop = sin(pi (sigma - sigma_stra)/(2 (1 - sigma_stra))) below z_stra (clamped at 0), 0 above;
+ * T_vert by Eq. 61; K_T = 1/tau_rad; no drag (L512).  The substellar point is on the +x axis.
+ * hj = NULL switches it off; exclusive with the tables and with the Held-Suarez forcing. */
+typedef struct {
+    double T_surf, Gamma, dT_stra, z_stra;   /* 1600 K, 2e-4 K/m, 10 K, 2e6 m  (L527) */
+    double sigma_stra, dT_EP, tau_rad;       /* 0.12, 300 K, 1.5e5 s           (L516-L529) */
+} thor_hot_jupiter;
+int thor_state_set_hot_jupiter(thor_state *state, const thor_hot_jupiter *hj);
+
 /* Only the hot loop: n_substeps acoustic substeps (steps a4-a9 of DESIGN.md) of length delta on the
  * stage data left by the last thor_step.  which: 1 = explicit horizontal momentum kernel only,
  * 2 = divergence + column-solve kernel only, 3 = both.  For measurement; the state it leaves is

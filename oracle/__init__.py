@@ -75,6 +75,9 @@ def _load():
         L.orc_step_held_suarez.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
                                            ctypes.c_double, ctypes.c_double]
         L.orc_forcing_held_suarez.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D]
+        L.orc_step_hot_jupiter.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
+                                           ctypes.c_double, ctypes.c_double]
+        L.orc_forcing_hot_jupiter.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D]
         L.orc_num_threads.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -202,6 +205,20 @@ class Geometry:
         _load().orc_forcing_held_suarez(self._h, float(dt), _p(rho), _p(V), _p(p), _p(h))
         return V, p
 
+    # NEXT-2, hot Jupiter (Eq. 59-61); hj: dict with HJ_KEYS
+    def step_hot_jupiter(self, rho, V, W, p, n_large, dt, n_sub, hj, D_hyp=0.0, D_div=0.0):
+        rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
+        h = _c(np.array([float(hj[k]) for k in HJ_KEYS]))
+        _load().orc_step_hot_jupiter(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
+                                     float(D_hyp), float(D_div))
+        return rho, V, W, p
+
+    def forcing_hot_jupiter(self, rho, p, dt, hj):
+        rho, p = _c(rho).copy(), _c(p).copy()
+        h = _c(np.array([float(hj[k]) for k in HJ_KEYS]))
+        _load().orc_forcing_hot_jupiter(self._h, float(dt), _p(rho), _p(p), _p(h))
+        return p
+
     def diagnostics(self, rho, V, W, p):
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))
         m = ctypes.c_double()
@@ -266,6 +283,7 @@ def tau_d(dbar_, kd_):
     return float(_load().orc_tau_d(float(dbar_), float(kd_)))
 
 
+HJ_KEYS = ("T_surf", "Gamma", "dT_stra", "z_stra", "sigma_stra", "dT_EP", "tau_rad")
 HS_KEYS = ("T_surf", "dT_y", "dth_z", "T_min", "k_a", "k_s", "k_f", "sigma_b", "p_star")
 
 

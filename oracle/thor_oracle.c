@@ -841,6 +841,49 @@ static void forcing_held_suarez(const orc_geom *G, double dt, double *rho, doubl
         }
     }
 }
+/* NEXT-2, second half: the tidally locked hot-Jupiter forcing of section 7.2 (Eq. 59-61):
+ *   K_v = 0 (L512); K_T = 1/tau_rad, constant (L529: 1.5e5 s);
+ *   T_eq = T_vert(z) + beta_trop(sigma, z) dT_EP cos(lon) cos(lat)                           (Eq. 59)
+ *   beta_trop = sin(pi (sigma - sigma_stra) / (2 (1 - sigma_stra))) for z <= z_stra, else 0    (Eq. 60)
+ *   T_vert = T_surf - Gamma (z_stra + (z - z_stra)/2) + sqrt((Gamma (z - z_stra)/2)^2 + dT_stra^2)  for z <= z_stra,
+ *            T_surf - Gamma z_stra + dT_stra                                                   for z >  z_stra  (Eq. 61, G15)
+ * cos(lon) cos(lat) is the x component of the column's unit vector: the substellar point is on the x axis.
+ * sigma as in the Held-Suarez forcing (L390).  beta_trop is clamped at 0 where sigma < sigma_stra below
+ * z_stra (the sine would turn negative; reading RJ1). */
+typedef struct { double T_surf, Gamma, dT_stra, z_stra, sigma_stra, dT_EP, tau_rad; } orc_hot_jupiter;
+
+static void forcing_hot_jupiter(const orc_geom *G, double dt, double *rho, double *p, const orc_hot_jupiter *J) {
+    const int N = G->N, nv = G->nv;
+    const orc_planet *P = &G->P;
+    const double KT = 1.0 / J->tau_rad, pi = 3.14159265358979323846;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; i++) {
+        const double mu = G->xyz[3 * i];
+        size_t c0 = (size_t)i * nv;
+        const double T0 = p[c0] / (rho[c0] * P->Rd);
+        const double ps = p[c0] * exp(P->gravity * G->z_c[0] / (P->Rd * T0));
+        for (int k = 0; k < nv; k++) {
+            size_t c = c0 + k;
+            const double z = G->z_c[k], sigma = p[c] / ps;
+            double Tvert, beta = 0.0;
+            if (z <= J->z_stra) {
+                const double hz = 0.5 * J->Gamma * (z - J->z_stra);
+                Tvert = J->T_surf - J->Gamma * (J->z_stra + 0.5 * (z - J->z_stra)) + sqrt(hz * hz + J->dT_stra * J->dT_stra);
+                if (sigma > J->sigma_stra) beta = sin(pi * (sigma - J->sigma_stra) / (2.0 * (1.0 - J->sigma_stra)));
+            } else {
+                Tvert = J->T_surf - J->Gamma * J->z_stra + J->dT_stra;
+            }
+            const double Teq = Tvert + beta * J->dT_EP * mu;                                     /* Eq. 59 */
+            double T = p[c] / (rho[c] * P->Rd);
+            T = (T + KT * dt * Teq) / (1.0 + KT * dt);                                           /* Eq. 52 */
+            p[c] = rho[c] * P->Rd * T;
+        }
+    }
+}
+void orc_forcing_hot_jupiter(const orc_geom *G, double dt, double *rho, double *p, const double *hj) {
+    forcing_hot_jupiter(G, dt, rho, p, (const orc_hot_jupiter *)hj);
+}
+
 void orc_forcing_held_suarez(const orc_geom *G, double dt, double *rho, double *V, double *p, const double *hs) {
     forcing_held_suarez(G, dt, rho, V, p, (const orc_held_suarez *)hs);
 }
@@ -854,6 +897,7 @@ double orc_kd(double D, double dbar, double dt);
  * divergence damping (the paper uses the same value for both, L367); 0 switches a term off, and
  * (0, 0) is the base path of SURVEY 8(a), arithmetic untouched. */
 static const orc_held_suarez *g_hs = NULL;   /* set by orc_step_held_suarez for the duration of its call */
+static const orc_hot_jupiter *g_hj = NULL;   /* likewise, orc_step_hot_jupiter */
 
 void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
                         int n_sub, const double *T_eq, const double *k_T, const double *k_v, double D_hyp, double D_div) {
@@ -903,10 +947,17 @@ void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, do
             for (size_t c = 0; c < ni; c++) w->W_t[c] = w->W_t[c] + w->W_s[c];
         }
         memcpy(rho, w->rho_t, 8 * nc); memcpy(V, w->V_t, 24 * nc); memcpy(W, w->W_t, 8 * ni); memcpy(p, w->p_t, 8 * nc);
-        if (g_hs) forcing_held_suarez(G, dt, rho, V, p, g_hs);
+        if (g_hj) forcing_hot_jupiter(G, dt, rho, p, g_hj);
+        else if (g_hs) forcing_held_suarez(G, dt, rho, V, p, g_hs);
         else forcing(G, dt, rho, V, p, T_eq, k_T, k_v);
     }
     work_free(w);
+}
+void orc_step_hot_jupiter(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,
+                          int n_sub, const double *hj, double D_hyp, double D_div) {
+    g_hj = (const orc_hot_jupiter *)hj;
+    orc_step_diffusion(G, rho, V, W, p, n_large, dt, n_sub, NULL, NULL, NULL, D_hyp, D_div);
+    g_hj = NULL;
 }
 /* hs: the nine numbers of orc_held_suarez */
 void orc_step_held_suarez(const orc_geom *G, double *rho, double *V, double *W, double *p, int n_large, double dt,

@@ -44,6 +44,10 @@ class thor_held_suarez(ctypes.Structure):
     _fields_ = [(n, ctypes.c_double) for n in ("T_surf", "dT_y", "dth_z", "T_min", "k_a", "k_s", "k_f", "sigma_b", "p_star")]
 
 
+class thor_hot_jupiter(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in ("T_surf", "Gamma", "dT_stra", "z_stra", "sigma_stra", "dT_EP", "tau_rad")]
+
+
 class thor_diag(ctypes.Structure):
     _fields_ = [("total_mass", ctypes.c_double), ("total_energy", ctypes.c_double)]
 
@@ -60,6 +64,7 @@ _SIGNATURES = {
     "thor_step": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(thor_forcing)]),
     "thor_state_set_diffusion": (ctypes.c_int, [_V, ctypes.c_double, ctypes.c_double]),
     "thor_state_set_held_suarez": (ctypes.c_int, [_V, ctypes.POINTER(thor_held_suarez)]),
+    "thor_state_set_hot_jupiter": (ctypes.c_int, [_V, ctypes.POINTER(thor_hot_jupiter)]),
     "thor_acoustic_substeps": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int]),
     "thor_diagnostics": (ctypes.c_int, [_V, ctypes.POINTER(thor_diag)]),
     "thor_apply_div": (ctypes.c_int, [_V, _D, _D]),
@@ -168,6 +173,14 @@ def thor_state_set_held_suarez(state, hs):
         return
     H = thor_held_suarez(**{k: float(hs[k]) for k, _ in thor_held_suarez._fields_})
     _check(load_library().thor_state_set_held_suarez(state, ctypes.byref(H)))
+
+
+def thor_state_set_hot_jupiter(state, hj):
+    if hj is None:
+        _check(load_library().thor_state_set_hot_jupiter(state, None))
+        return
+    J = thor_hot_jupiter(**{k: float(hj[k]) for k, _ in thor_hot_jupiter._fields_})
+    _check(load_library().thor_state_set_hot_jupiter(state, ctypes.byref(J)))
 
 
 def thor_acoustic_substeps(state, n_substeps, delta, which=3):
@@ -300,6 +313,9 @@ class State:
 
     def set_held_suarez(self, hs):
         thor_state_set_held_suarez(self._h, hs)
+
+    def set_hot_jupiter(self, hj):
+        thor_state_set_hot_jupiter(self._h, hj)
 
     def acoustic_substeps(self, n_substeps, delta, which=3):
         thor_acoustic_substeps(self._h, n_substeps, delta, which)

@@ -82,6 +82,7 @@ struct thor_state {
     double* X = nullptr;             // NEXT-1 work rows [Npad][XF][NVP], allocated by thor_state_set_diffusion
     double D_hyp = 0.0, D_div = 0.0; // non-dimensional diffusion parameters of Eq. 49 (0 = term off)
     HeldSuarez hs{};                 // NEXT-2: forcing from the evolving sigma (on = 0: tables or none)
+    HotJupiter hj{};
     double* stage_buf = nullptr;     // canonical-order staging, max(N*nv*3, N*(nv+1)) doubles
     double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;   // [Npad][NVP]
     bool has_Teq = false, has_kT = false, has_kv = false;
@@ -89,7 +90,7 @@ struct thor_state {
     bool stepped = false;
     int walk = 0;                    // direction of the last launch (0 ascending, 1 descending)
     // one large step captured as a CUDA graph, per starting walk direction (replayed while the key holds)
-    struct GraphKey { double dt = 0, D_hyp = 0, D_div = 0; HeldSuarez hs{}; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
+    struct GraphKey { double dt = 0, D_hyp = 0, D_div = 0; HeldSuarez hs{}; HotJupiter hj{}; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
     GraphKey gkey;
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     int gwalk_end[2] = {0, 0};
@@ -575,7 +576,7 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
             if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
         }
     }
-    THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, s->hs, dt, dir(tn.ks));
+    THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, s->hs, s->hj, dt, dir(tn.ks));
     return THOR_OK;
 }
 
@@ -588,7 +589,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (!s) return fail(THOR_EINVAL, "thor_step: null state");
     if (n_large < 0 || !(dt > 0) || n < 2 || (n & 1)) return fail(THOR_EINVAL, "thor_step: need n_large >= 0, dt > 0, even n >= 2");
     cudaStream_t st = s->stream;
-    if (forcing && s->hs.on) return fail(THOR_EINVAL, "thor_step: table forcing and Held-Suarez forcing are exclusive");
+    if (forcing && (s->hs.on || s->hj.on)) return fail(THOR_EINVAL, "thor_step: table forcing and evolving-sigma forcing are exclusive");
     if (forcing && !forcing->resident) {
         int rc;
         s->has_Teq = forcing->T_eq != nullptr; s->has_kT = forcing->k_T != nullptr; s->has_kv = forcing->k_v != nullptr;
@@ -609,7 +610,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (use_graph) {
         thor_state::GraphKey key;
         std::memset(&key, 0, sizeof(key));
-        key.dt = dt; key.n = n; key.D_hyp = s->D_hyp; key.D_div = s->D_div; key.hs = s->hs; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
+        key.dt = dt; key.n = n; key.D_hyp = s->D_hyp; key.D_div = s->D_div; key.hs = s->hs; key.hj = s->hj; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
         if (const char* e = std::getenv("THOR_B200_TUNE")) std::strncpy(key.tune, e, sizeof(key.tune) - 1);
         if (std::memcmp(&key, &s->gkey, sizeof(key)) != 0) {
             drop_graphs(s);
@@ -671,10 +672,24 @@ int thor_state_set_held_suarez(thor_state* s, const thor_held_suarez* hs) {
     }
     if (!(hs->sigma_b >= 0.0 && hs->sigma_b < 1.0) || !(hs->p_star > 0.0) || !(hs->k_a >= 0.0) || !(hs->k_s >= 0.0) || !(hs->k_f >= 0.0))
         return fail(THOR_EINVAL, "thor_state_set_held_suarez: need 0 <= sigma_b < 1, p_star > 0, rates >= 0");
+    if (s->hj.on) return fail(THOR_EINVAL, "thor_state_set_held_suarez: hot-Jupiter forcing is on");
     std::memset(&s->hs, 0, sizeof(s->hs));
     s->hs.on = 1;
     s->hs.T_surf = hs->T_surf; s->hs.dT_y = hs->dT_y; s->hs.dth_z = hs->dth_z; s->hs.T_min = hs->T_min;
     s->hs.k_a = hs->k_a; s->hs.k_s = hs->k_s; s->hs.k_f = hs->k_f; s->hs.sigma_b = hs->sigma_b; s->hs.p_star = hs->p_star;
+    return THOR_OK;
+}
+
+int thor_state_set_hot_jupiter(thor_state* s, const thor_hot_jupiter* hj) {
+    if (!s) return fail(THOR_EINVAL, "thor_state_set_hot_jupiter: null state");
+    std::memset(&s->hj, 0, sizeof(s->hj));
+    if (!hj) return THOR_OK;
+    if (!(hj->tau_rad > 0.0) || !(hj->sigma_stra >= 0.0 && hj->sigma_stra < 1.0))
+        return fail(THOR_EINVAL, "thor_state_set_hot_jupiter: need tau_rad > 0, 0 <= sigma_stra < 1");
+    if (s->hs.on) return fail(THOR_EINVAL, "thor_state_set_hot_jupiter: Held-Suarez forcing is on");
+    s->hj.on = 1;
+    s->hj.T_surf = hj->T_surf; s->hj.Gamma = hj->Gamma; s->hj.dT_stra = hj->dT_stra; s->hj.z_stra = hj->z_stra;
+    s->hj.sigma_stra = hj->sigma_stra; s->hj.dT_EP = hj->dT_EP; s->hj.tau_rad = hj->tau_rad;
     return THOR_OK;
 }
 

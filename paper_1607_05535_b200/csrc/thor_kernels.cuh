@@ -87,6 +87,11 @@ struct HeldSuarez {
     int on;
     double T_surf, dT_y, dth_z, T_min, k_a, k_s, k_f, sigma_b, p_star;
 };
+// NEXT-2: tidally locked hot-Jupiter forcing of section 7.2 (Eq. 59-61); K_v = 0, K_T = 1/tau_rad
+struct HotJupiter {
+    int on;
+    double T_surf, Gamma, dT_stra, z_stra, sigma_stra, dT_EP, tau_rad;
+};
 
 // L2 schedule of one launch (defaults in thor_api.cu).  Successive kernels of a
 // large step walk the columns in ALTERNATING directions, so each starts on the rows the previous one has
@@ -1155,7 +1160,7 @@ k_vertical_staged(Geom g, TileTab tt, double* __restrict__ S, double delta, int 
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, double dt, Tune tn) {
+k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, double dt, Tune tn) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -1187,7 +1192,30 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, double dt, Tun
     }
     sum(F_WT, F_WS, a);
     st_row<E>(me + F_WN * NVP, a);
-    if (H.on) {
+    if (J.on) {
+        // Eq. 59-61 (G15, RJ1): T_eq = T_vert(z) + beta_trop(sigma, z) dT_EP cos(lon) cos(lat); cos(lon) cos(lat) = x of the unit vector
+        const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
+        const double ps = p0 * exp(g.gravity * __ldg(g.zc) / (g.Rd * (p0 / (rho0 * g.Rd))));
+        const double mu = ld_rhat(g.rhat, L.col).x, KT = 1.0 / J.tau_rad;
+        double z[E];
+        ld_nc<E>(g.zc + L.k0, z);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double sigma = p[e] / ps;
+            double Tvert, beta = 0.0;
+            if (z[e] <= J.z_stra) {
+                const double hz = 0.5 * J.Gamma * (z[e] - J.z_stra);
+                Tvert = J.T_surf - J.Gamma * (J.z_stra + 0.5 * (z[e] - J.z_stra)) + sqrt(hz * hz + J.dT_stra * J.dT_stra);
+                if (sigma > J.sigma_stra) beta = sin(3.14159265358979323846 * (sigma - J.sigma_stra) / (2.0 * (1.0 - J.sigma_stra)));
+            } else {
+                Tvert = J.T_surf - J.Gamma * J.z_stra + J.dT_stra;
+            }
+            const double Teq = Tvert + beta * J.dT_EP * mu;
+            double T = p[e] / (rho[e] * g.Rd);
+            T = (T + KT * dt * Teq) / (1.0 + KT * dt);                        // Eq. 52
+            p[e] = (L.k0 + e < g.nv && L.col < g.N) ? rho[e] * g.Rd * T : p[e];
+        }
+    } else if (H.on) {
         // sigma = p/p_s with the surface pressure extrapolated hydrostatically and isothermally from the lowest
         // layer centre (L390); K_v (Eq. 53), T_eq (Eq. 54, G14), K_T (Eq. 55, G14); then Eq. 51-52
         const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
@@ -1216,7 +1244,7 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, double dt, Tun
             vx[e] /= s; vy[e] /= s; vz[e] /= s;                               // Eq. 51
         }
     }
-    if (!H.on && F.k_T && F.T_eq) {
+    if (!H.on && !J.on && F.k_T && F.T_eq) {
         double te[E];
         ld_nc<E>(F.k_T + to, a); ld_nc<E>(F.T_eq + to, te);
 #pragma unroll

@@ -308,6 +308,30 @@ def test_next2_held_suarez_forcing_parity(nv):
     _compare(st.get(), base, 1e-11, "held-suarez off nv=%d" % nv, floor, K=40.0)
 
 
+def test_next2_hot_jupiter_forcing_parity():
+    """Eq. 59-61 on the paper's hot-Jupiter planet (Table 1), with NEXT-1 at its D, 5 large steps."""
+    planet, nv, D = dict(ti.PAPER_HOT_JUPITER), 37, 0.01992
+    g, G = _setup(3, nv, planet)
+    rng = np.random.default_rng(9)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1.0e5, 1600.0)
+    T = 1600.0 * (1 + rng.uniform(-1e-3, 1e-3, size=rho.shape))
+    rho = p / (planet["Rd"] * T)
+    s = (rho, V, W, p)
+    st = thor.State(g, *s)
+    st.set_diffusion(D)
+    st.set_hot_jupiter(ti.HOT_JUPITER_FORCING)
+    with pytest.raises(thor.ThorError):
+        st.set_held_suarez(ti.HELD_SUAREZ)                                   # one evolving-sigma forcing at a time
+    st.step(5, 600.0, 6)
+    ref = G.step_hot_jupiter(*s, 5, 600.0, 6, ti.HOT_JUPITER_FORCING, D, D)
+    eps = np.finfo(np.float64).eps
+    pert = [a * (1.0 + eps * rng.choice([-1.0, 1.0], size=a.shape)) for a in s]
+    floor = [np.abs(x - y).max() for x, y in zip(ref, G.step_hot_jupiter(*pert, 5, 600.0, 6, ti.HOT_JUPITER_FORCING, D, D))]
+    _compare(st.get(), ref, 1e-11, "hot jupiter", floor, K=40.0)
+    base = G.step(*s, 5, 600.0, 6, None, D, D)
+    assert np.abs(ref[3] - base[3]).max() > 1e4 * np.abs(st.get()[3] - ref[3]).max()
+
+
 def test_held_suarez_benchmark_spins_up_midlatitude_jets():
     """End to end (base path + NEXT-1 + NEXT-2): the paper's Earth benchmark set-up (section 7.1: level 5,
     dt = 1000 s, n = 6, D from Table 1, rest state at 300 K, top at 32 km) integrated 250 days on the GPU.

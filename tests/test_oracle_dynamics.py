@@ -468,3 +468,35 @@ def test_held_suarez_forcing_closed_forms(ogrid):
     assert abs(Tbig[eq, 0] - (315.0 - 60.0 * xyz[eq, 2] ** 2)) < 1e-3
     assert np.all(np.abs(Tbig[:, -1] - 200.0) < 1e-3)                                # clipped aloft (top at 36 km)
     assert np.abs(Vbig[p2 / ps2 > 0.75]).max() < 1e-6 * np.abs(V).max()
+
+
+def test_hot_jupiter_forcing_closed_forms(ogrid):
+    """Eq. 59-61 by hand (G15: the second branch of T_vert is z > z_stra): with a huge step T lands on T_eq;
+    at the substellar point's lowest layer T_eq = T_vert + beta dT_EP with beta -> sin(pi/2 (sigma - 0.12)/0.88),
+    on the terminator (x = 0) T_eq = T_vert exactly, on the night side the contrast changes sign, above
+    z_stra = 2000 km T_eq = 1600 - 2e-4 * 2e6 + 10 = 1210 K everywhere; T_vert is continuous at z_stra."""
+    import oracle
+    planet, nv = dict(ti.PAPER_HOT_JUPITER), 37
+    xyz, nbr, C = ogrid(2, True)
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    hj = dict(ti.HOT_JUPITER_FORCING)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1.0e5, 1600.0)
+    pn = G.forcing_hot_jupiter(rho, p, 1.0e14, hj)
+    T = pn / (rho * planet["Rd"])
+    z, sigma = G.z_c, p[0] / 1.0e5                                   # isothermal hydrostatic column: p_s extrapolates to 1e5 exactly
+    hz = 0.5 * hj["Gamma"] * (z - hj["z_stra"])
+    Tvert = np.where(z <= hj["z_stra"], hj["T_surf"] - hj["Gamma"] * (hj["z_stra"] + 0.5 * (z - hj["z_stra"])) + np.sqrt(hz ** 2 + hj["dT_stra"] ** 2),
+                     hj["T_surf"] - hj["Gamma"] * hj["z_stra"] + hj["dT_stra"])
+    beta = np.where((z <= hj["z_stra"]) & (sigma > hj["sigma_stra"]), np.sin(np.pi * (sigma - hj["sigma_stra"]) / (2 * (1 - hj["sigma_stra"]))), 0.0)
+    Teq = Tvert[None, :] + beta[None, :] * hj["dT_EP"] * xyz[:, 0][:, None]
+    assert np.abs(T - Teq).max() < 1e-6
+    assert np.all(np.abs(T[:, z > hj["z_stra"]] - 1210.0) < 1e-6)
+    sub, anti = int(np.argmax(xyz[:, 0])), int(np.argmin(xyz[:, 0]))
+    assert T[sub, 0] > Tvert[0] + 250.0 and T[anti, 0] < Tvert[0] - 250.0     # ~ +-300 K day-night contrast at depth
+    k = int(np.searchsorted(z, hj["z_stra"]))
+    assert abs(Tvert[k] - Tvert[k - 1]) < 2.0 * hj["Gamma"] * G.dz            # continuous across z_stra
+    # finite step: Eq. 52 with K_T = 1/tau_rad
+    dt = 600.0
+    p2 = G.forcing_hot_jupiter(rho, p, dt, hj)
+    KT = 1.0 / hj["tau_rad"]
+    assert np.allclose(p2 / (rho * planet["Rd"]), (1600.0 + KT * dt * Teq) / (1.0 + KT * dt), rtol=1e-13, atol=0)

@@ -28,6 +28,11 @@ HOT_JUPITER = dict(radius=9.44e7, omega=2.06e-5, gravity=9.42, Rd=3779.0, Cp=132
 HELD_SUAREZ = dict(T_surf=315.0, dT_y=60.0, dth_z=10.0, T_min=200.0, k_a=1.0 / (40 * 86400.0), k_s=1.0 / (4 * 86400.0),
                    k_f=1.0 / 86400.0, sigma_b=0.7, p_star=1.0e5)
 
+# Hot-Jupiter benchmark of the paper (Table 1): forcing parameters of Eq. 59-61 and the
+# planet; the surface pressure is not printed (1e5 Pa, the reference pressure, is used).
+HOT_JUPITER_FORCING = dict(T_surf=1600.0, Gamma=2.0e-4, dT_stra=10.0, z_stra=2.0e6, sigma_stra=0.12, dT_EP=300.0, tau_rad=1.5e5)
+PAPER_HOT_JUPITER = dict(radius=1.0e8, omega=2.1e-5, gravity=8.0, Rd=3779.0, Cp=13226.5, p_ref=1.0e5, z_top=4.875e6)
+
 # BASELINE.json configs (index = config number).  n_large is the run length used for parity.
 CONFIGS = {
     0: dict(name="cfg0_level4x8_earth", level=4, nv=8, planet=EARTH, p_s=1.0e5, T0=300.0,
