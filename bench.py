@@ -41,9 +41,33 @@ SUBSTEP_DESIGN_DOUBLES = K1_DESIGN_DOUBLES + K2_DESIGN_DOUBLES
 SURVEY_GEOM_BYTES = 336       # per column, SURVEY 8(d)
 K2_GEOM_BYTES = 8 * 4 + 16 * 8    # this design: 8 int32 neighbour slots + 7x2 (+2 pad) contracted divergence weights
 K1_GEOM_BYTES = 8 * 4 + 12 * 8    # 8 int32 + 6x2 contracted gradient weights
-# HBM traffic of one k_vertical launch on config 3 from the committed ncu --set full capture
-# (profiles/r01c_substep_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum)
-K2_NCU_TRAFFIC_BYTES = {3: 200.3e6}
+# HBM traffic per launch, WARM (ncu --cache-control none over graph-replayed large steps, so every kernel finds
+# the L2 as its predecessor left it -- the situation bench.py times): raw ncu csv committed under profiles/,
+# the command that wrote it in the .md beside it.  Parsed here, never typed in.
+WARM_TRAFFIC_CSV = {3: "profiles/r02_warm_traffic_cfg3.csv", 4: "profiles/r02_warm_traffic_cfg4.csv"}
+
+
+def ncu_warm_traffic(workload, kernel_prefix):
+    """Mean dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernels whose name starts with
+    `kernel_prefix` in the committed raw ncu csv of `workload` (None if there is no such file or kernel)."""
+    import csv
+    path = os.path.join(ROOT, WARM_TRAFFIC_CSV.get(workload, ""))
+    if not os.path.isfile(path):
+        return None
+    per_launch = {}
+    with open(path, newline="") as f:
+        rows = [r for r in f if r.startswith('"')]
+    rd = csv.reader(rows)
+    head = next(rd, None)
+    if not head or "Metric Name" not in head:
+        return None
+    i_id, i_k, i_m, i_v = head.index("ID"), head.index("Kernel Name"), head.index("Metric Name"), head.index("Metric Value")
+    for r in rd:
+        name = r[i_k].split("thor::")[-1]
+        if name.startswith(kernel_prefix + "<") or name.startswith(kernel_prefix + "("):
+            if r[i_m] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                per_launch[r[i_id]] = per_launch.get(r[i_id], 0.0) + float(r[i_v].replace(",", ""))
+    return sum(per_launch.values()) / len(per_launch) if per_launch else None
 
 
 def measured_peak():
@@ -105,48 +129,73 @@ def aggregate_value(cells_per_step, steps, world, ms):
     return cells_per_step * steps * world / (ms * 1e-3)
 
 
-def sample_config(level):
-    """config 3's constants and forcing on a coarser grid (used only by the CPU legs)."""
-    cfg = dict(ti.CONFIGS[WORKLOAD])
-    cfg["dt"] = cfg["dt"] * 2 ** (cfg["level"] - level)
-    cfg["level"] = level
-    return cfg
+def oracle_sample_level(workload):
+    """Grid level of the oracle-timing legs: the workload's own up to level 6 (0.45 s per large step on 16
+    cores at config 3); config 4's level 7 x 64 costs ~5 s per step, so it is sampled at level 6 with dt doubled."""
+    return min(ti.CONFIGS[workload]["level"], 6)
 
 
-def time_oracle(level, n_steps, warmup):
-    """The oracle as it stands on the host cores.  Grid description from the oracle's own generator
-    up to level 4 is too slow beyond that, so the library's host generator supplies positions."""
+def time_oracle(workload, n_steps, warmup, threads=None):
+    """The oracle as it stands on the host cores -- nothing of the product is imported, loaded or called here.
+    The grid is the oracle's own generator WITHOUT spring smoothing (level 6 smoothing in numpy would take
+    minutes; the oracle's work per step does not depend on where the points sit).  threads=None: all cores."""
     import oracle
-    import paper_1607_05535_b200 as thor
-    cfg = sample_config(level)
-    g = thor.Grid(level, cfg["nv"], cfg["planet"])          # host-only call
-    v = g.view
-    G = oracle.Geometry(v["xyz"], v["nbr"], cfg["nv"], cfg["planet"], v["cv_vertex"])
-    ti.CONFIGS["_sample"] = cfg
-    state = ti.initial_state(WORKLOAD, v["xyz"])
-    F = ti.forcing_tables(WORKLOAD, v["xyz"])
-    for _ in range(warmup):
-        state = G.step(*state, 1, cfg["dt"], cfg["n_sub"], F)
-    t0 = time.perf_counter()
-    for _ in range(n_steps):
-        state = G.step(*state, 1, cfg["dt"], cfg["n_sub"], F)
-    dt = time.perf_counter() - t0
-    cells = v["n_cols"] * cfg["nv"] * ti.substeps_per_large_step(cfg["n_sub"])
-    return cells * n_steps / dt, dt / max(n_steps, 1), oracle.num_threads(), \
-        "config-%d constants and forcing at level %d x %d layers (%d columns), %d large steps" % (
-            WORKLOAD, level, cfg["nv"], v["n_cols"], n_steps)
+    from oracle import grid_oracle
+    cfg = dict(ti.CONFIGS[workload])
+    level = oracle_sample_level(workload)
+    dt = cfg["dt"] * 2 ** (cfg["level"] - level)
+    xyz, nbr, C, _ = grid_oracle.build(level, smooth=False)
+    G = oracle.Geometry(xyz, nbr, cfg["nv"], cfg["planet"], C)
+    state = ti.initial_state(workload, xyz)
+    F = ti.forcing_tables(workload, xyz)
+    all_threads = oracle.num_threads()
+    if threads is not None:
+        oracle.set_num_threads(threads)
+    try:
+        for _ in range(warmup):
+            state = G.step(*state, 1, dt, cfg["n_sub"], F)
+        t0 = time.perf_counter()
+        for _ in range(n_steps):
+            state = G.step(*state, 1, dt, cfg["n_sub"], F)
+        el = time.perf_counter() - t0
+        used = oracle.num_threads()
+    finally:
+        oracle.set_num_threads(all_threads)
+    cells = xyz.shape[0] * cfg["nv"] * ti.substeps_per_large_step(cfg["n_sub"])
+    sample = "config %d at level %d x %d layers (%d columns, unsmoothed bisection grid of the oracle's own generator), " \
+             "%d large steps of dt=%g s, n=%d, forcing tables on" % (workload, level, cfg["nv"], xyz.shape[0], n_steps, dt, cfg["n_sub"])
+    return cells * n_steps / el, el / max(n_steps, 1), used, sample
+
+
+def workload_config(workload, N, world):
+    """The `config` object both arms print (same workload, same words)."""
+    cfg = ti.CONFIGS[workload]
+    nv, n = cfg["nv"], cfg["n_sub"]
+    substeps = ti.substeps_per_large_step(n)
+    cells = N * nv
+    return {"workload": "config %d: level %d (%d columns) x %d layers, hot-Jupiter constants, dt=%g s, "
+                        "n=%d (%d substeps per large step), Newtonian relaxation forcing" % (
+                            workload, cfg["level"], N, nv, cfg["dt"], n, substeps),
+            "cells": cells, "substeps_per_step": substeps, "parallelism": "replicas x%d" % world}
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    value, per_step, cores, sample = time_oracle(5, args.steps, args.warmup)
+    value, per_step, cores, sample = time_oracle(WORKLOAD, args.steps, args.warmup)
+    v1, _, _, _ = time_oracle(WORKLOAD, 1, 0, threads=1)
+    level = oracle_sample_level(WORKLOAD)
+    config = workload_config(WORKLOAD, ti.n_columns(level), 1)
+    if level != ti.CONFIGS[WORKLOAD]["level"]:
+        config["workload"] += " -- SAMPLED by the oracle arm: " + sample
+    config["oracle_grid"] = "unsmoothed bisection grid of the oracle's own generator (no product code in this arm)"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config %d (hot Jupiter, n=%d) sampled: " % (WORKLOAD, ti.CONFIGS[WORKLOAD]["n_sub"]) + sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "config": config,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "value_1_thread": v1},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -202,32 +251,43 @@ def run_cuda(args):
         launches = thor.thor_launch_count() - l0
         ms = ev0.elapsed_time(ev1)
 
-        # dominant kernel alone (K2 = divergences + column solve) and K1, CUDA events on the same stream
-        def time_kernels(which, reps=60):
-            state.acoustic_substeps(5, dt / n, which)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            a.record(stream)
-            state.acoustic_substeps(reps, dt / n, which)
-            b.record(stream)
-            torch.cuda.synchronize()
-            return a.elapsed_time(b) / reps
+        # dominant kernel alone (K2 = divergences + column solve) and K1, CUDA events on the same stream.  Chunks of
+        # n launches (a stage's worth) between untimed large steps, so that the timed state stays a physical one
+        # (repeating one kernel alone for thousands of launches drives it to NaN and down another branch of
+        # eos_dev); chunks are accumulated until the timed launches cover >= 0.2 s.
+        def time_kernels(which, min_ms=200.0, chunk=n):
+            state.step(1, dt, n, forcing)
+            state.acoustic_substeps(chunk, dt / n, which)
+            total, reps = 0.0, 0
+            while total < min_ms and reps < 100000:
+                state.step(1, dt, n, forcing)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                state.acoustic_substeps(chunk, dt / n, which)
+                b.record(stream)
+                b.synchronize()
+                total += a.elapsed_time(b)
+                reps += chunk
+            return total / reps
         # config 1: the two stencils alone (Eq. 6, Eq. 7) on device arrays of this grid, 32 B/cell + geometry
         nc = N * nv
         bufs = [torch.rand(nc, dtype=torch.float64, device="cuda") for _ in range(7)]
         ptr = [b.data_ptr() for b in bufs]
 
-        def time_op(fn, reps=40):
+        def time_op(fn, min_ms=200.0, chunk=200):
             for _ in range(3):
                 fn()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            a.record(stream)
-            for _ in range(reps):
-                fn()
-            b.record(stream)
-            torch.cuda.synchronize()
-            return a.elapsed_time(b) / reps
+            total, reps = 0.0, 0
+            while total < min_ms:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(chunk):
+                    fn()
+                b.record(stream)
+                b.synchronize()
+                total += a.elapsed_time(b)
+                reps += chunk
+            return total / reps
         div_ms = time_op(lambda: thor.thor_apply_div_device(grid.handle, ptr[0], ptr[1], ptr[2], ptr[3], stream.cuda_stream))
         grad_ms = time_op(lambda: thor.thor_apply_grad_device(grid.handle, ptr[0], ptr[4], ptr[5], ptr[6], stream.cuda_stream))
         lap_ms = time_op(lambda: thor.thor_apply_lap_device(grid.handle, ptr[0], ptr[3], stream.cuda_stream))
@@ -284,7 +344,11 @@ def run_cuda(args):
     sub_design_bytes = cells * SUBSTEP_DESIGN_DOUBLES * 8 + N * (K1_GEOM_BYTES + K2_GEOM_BYTES)
     roofline = {"bound": "hbm", "kernel": "k_vertical (a5-a9: divergences + column solve + rho, rho-theta, p*)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": K2_NCU_TRAFFIC_BYTES.get(WORKLOAD),
+                "traffic": ncu_warm_traffic(WORKLOAD, "k_vertical"),
+                "traffic_kind": "dram read + write bytes per launch, mean over the k_vertical launches of %s (ncu "
+                                "--cache-control none over graph-replayed large steps: warm L2, as timed here)" % WARM_TRAFFIC_CSV.get(WORKLOAD),
+                "bytes_model": "achieved/frac: k_vertical's share (18 doubles/cell) of SURVEY 8(d)'s 27-double budget; "
+                               "achieved_design_bytes: the 19 doubles/cell this layout moves once",
                 "peak_kind": peak_kind, "ms_per_launch": k2_ms, "bytes_per_launch": k2_bytes,
                 "bytes_per_launch_design": cells * K2_DESIGN_DOUBLES * 8 + N * K2_GEOM_BYTES,
                 "achieved_design_bytes": (cells * K2_DESIGN_DOUBLES * 8 + N * K2_GEOM_BYTES) / (k2_ms * 1e-3) / 1e9,
@@ -304,12 +368,9 @@ def run_cuda(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config %d: level %d (%d columns) x %d layers, hot-Jupiter constants, dt=%g s, "
-                                   "n=%d (%d substeps per large step), Newtonian relaxation forcing" % (
-                                       WORKLOAD, cfg["level"], N, nv, dt, n, substeps),
-                       "cells": cells, "substeps_per_step": substeps, "parallelism": "replicas x%d" % world,
-                       "l2": "one large step streams the 33-row column-record slab (%d MB) > 126 MB L2; no flush" % (
-                           33 * 8 * cells * (64 if nv > 32 else 32) // nv // 1000000)},
+            "config": dict(workload_config(WORKLOAD, N, world),
+                           l2="one large step streams the 33-row column-record slab (%d MB) > 126 MB L2; no flush" % (
+                               33 * 8 * cells * (64 if nv > 32 else 32) // nv // 1000000)),
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
@@ -322,8 +383,10 @@ def run_cuda(args):
                           "lap_ms": lap_ms, "lap_GBs": (cells * 16 + N * 96) / (lap_ms * 1e-3) / 1e9,
                           "lap_what": "horizontal Laplacian of L369-L371 (NEXT-1 building block), 16 B/cell + geometry"}}
     if world == 1 and not args.no_cpu_baseline:
-        v, per, cores, sample = time_oracle(5, 4, 1)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        v, per, cores, sample = time_oracle(WORKLOAD, 4, 1)
+        v1, _, _, _ = time_oracle(WORKLOAD, 1, 0, threads=1)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                "value_1_thread": v1}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

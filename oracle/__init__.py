@@ -17,19 +17,31 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "thor_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
+# The SAME source compiled with FMA contraction allowed (a flag, not new arithmetic): the distance between
+# the two builds' answers is what a legal change of rounding does to this algorithm on these inputs -- the
+# yardstick of the parity tolerance.  Never the reference: parity is against _LIB.
+_LIB_FMA = os.path.join(_HERE, "liboracle_fma.so")
 # -ffp-contract=off: no FMA contraction, so the oracle's rounding is the plain IEEE one
 _CFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c99"]
+_CFLAGS_FMA = ["-O2", "-ffp-contract=fast", "-mfma", "-fopenmp", "-shared", "-fPIC", "-std=c99"]
 
 _lib = None
+_lib_fma = None
+
+
+def _compile(lib, flags, force):
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        tmp = lib + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc"] + flags + [_SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, lib)
+    return lib
 
 
 def build(force=False):
-    """Compile thor_oracle.c with gcc (building the checker is not using it)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + ".tmp%d" % os.getpid()
-        subprocess.check_call(["gcc"] + _CFLAGS + [_SRC, "-o", tmp, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+    """Compile thor_oracle.c with gcc (building the checker is not using it): the oracle proper and
+    its FMA-contracted twin."""
+    _compile(_LIB_FMA, _CFLAGS_FMA, force)
+    return _compile(_LIB, _CFLAGS, force)
 
 
 _D = ctypes.POINTER(ctypes.c_double)
@@ -40,47 +52,67 @@ class _Planet(ctypes.Structure):
     _fields_ = [(n, ctypes.c_double) for n in ("radius", "omega", "gravity", "Rd", "Cp", "p_ref", "z_top")]
 
 
-def _load():
-    global _lib
+def have_fma():
+    """The FMA twin needs a host CPU with the fma instruction set."""
+    try:
+        with open("/proc/cpuinfo") as f:
+            return " fma " in f.read().replace("\n", " ")
+    except OSError:
+        return False
+
+
+def _load(fma=False):
+    global _lib, _lib_fma
+    if fma:
+        if _lib_fma is None:
+            if not have_fma():
+                raise RuntimeError("oracle: the FMA-contracted twin needs a CPU with fma")
+            build()
+            _lib_fma = _declare(ctypes.CDLL(_LIB_FMA))
+        return _lib_fma
     if _lib is None:
-        L = ctypes.CDLL(build())
-        L.orc_geom_build.restype = ctypes.c_void_p
-        L.orc_geom_build.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Planet), _D, _I, _D]
-        L.orc_geom_free.argtypes = [ctypes.c_void_p]
-        for name in ("Ac", "len", "nrm", "C", "bary"):
-            f = getattr(L, "orc_geom_" + name)
-            f.restype = _D
-            f.argtypes = [ctypes.c_void_p]
-        L.orc_geom_deg.restype = _I
-        L.orc_geom_deg.argtypes = [ctypes.c_void_p]
-        L.orc_hdiv.argtypes = [ctypes.c_void_p, _D, _D]
-        L.orc_hgrad.argtypes = [ctypes.c_void_p, _D, _D]
-        L.orc_hlap.argtypes = [ctypes.c_void_p, _D, _D]
-        for name, nargs in (("orc_dbar", None), ("orc_kd", None), ("orc_tau_d", None)):
-            getattr(L, name).restype = ctypes.c_double
-        L.orc_dbar.argtypes = [ctypes.c_double, ctypes.c_int]
-        L.orc_kd.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double]
-        L.orc_tau_d.argtypes = [ctypes.c_double, ctypes.c_double]
-        L.orc_thomas.argtypes = [ctypes.c_int, _D, _D, _D, _D, _D]
-        L.orc_centroid_eq13.argtypes = [_D, ctypes.c_int, _D]
-        L.orc_step.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D]
-        L.orc_step_diffusion.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D,
-                                         ctypes.c_double, ctypes.c_double]
-        L.orc_diagnostics.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, _D, _D]
-        L.orc_tridiag_coefficients.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D, _D]
-        L.orc_slow_terms.argtypes = [ctypes.c_void_p] + [_D] * 12
-        L.orc_substep.argtypes = [ctypes.c_void_p, ctypes.c_double] + [_D] * 14
-        L.orc_diffusion_fluxes.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_double, _D, _D, _D, _D, _D]
-        L.orc_divergence_damping.argtypes = [ctypes.c_void_p, _D, _D, ctypes.c_double, _D]
-        L.orc_step_held_suarez.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
-                                           ctypes.c_double, ctypes.c_double]
-        L.orc_forcing_held_suarez.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D]
-        L.orc_step_hot_jupiter.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
-                                           ctypes.c_double, ctypes.c_double]
-        L.orc_forcing_hot_jupiter.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D]
-        L.orc_num_threads.restype = ctypes.c_int
-        _lib = L
+        _lib = _declare(ctypes.CDLL(build()))
     return _lib
+
+
+def _declare(L):
+    L.orc_geom_build.restype = ctypes.c_void_p
+    L.orc_geom_build.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Planet), _D, _I, _D]
+    L.orc_geom_free.argtypes = [ctypes.c_void_p]
+    for name in ("Ac", "len", "nrm", "C", "bary"):
+        f = getattr(L, "orc_geom_" + name)
+        f.restype = _D
+        f.argtypes = [ctypes.c_void_p]
+    L.orc_geom_deg.restype = _I
+    L.orc_geom_deg.argtypes = [ctypes.c_void_p]
+    L.orc_hdiv.argtypes = [ctypes.c_void_p, _D, _D]
+    L.orc_hgrad.argtypes = [ctypes.c_void_p, _D, _D]
+    L.orc_hlap.argtypes = [ctypes.c_void_p, _D, _D]
+    for name, nargs in (("orc_dbar", None), ("orc_kd", None), ("orc_tau_d", None)):
+        getattr(L, name).restype = ctypes.c_double
+    L.orc_dbar.argtypes = [ctypes.c_double, ctypes.c_int]
+    L.orc_kd.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_double]
+    L.orc_tau_d.argtypes = [ctypes.c_double, ctypes.c_double]
+    L.orc_thomas.argtypes = [ctypes.c_int, _D, _D, _D, _D, _D]
+    L.orc_centroid_eq13.argtypes = [_D, ctypes.c_int, _D]
+    L.orc_step.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D]
+    L.orc_step_diffusion.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D, _D, _D,
+                                     ctypes.c_double, ctypes.c_double]
+    L.orc_diagnostics.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, _D, _D]
+    L.orc_tridiag_coefficients.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D, _D]
+    L.orc_slow_terms.argtypes = [ctypes.c_void_p] + [_D] * 12
+    L.orc_substep.argtypes = [ctypes.c_void_p, ctypes.c_double] + [_D] * 14
+    L.orc_diffusion_fluxes.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_double, _D, _D, _D, _D, _D]
+    L.orc_divergence_damping.argtypes = [ctypes.c_void_p, _D, _D, ctypes.c_double, _D]
+    L.orc_step_held_suarez.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
+                                       ctypes.c_double, ctypes.c_double]
+    L.orc_forcing_held_suarez.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D, _D]
+    L.orc_step_hot_jupiter.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
+                                       ctypes.c_double, ctypes.c_double]
+    L.orc_forcing_hot_jupiter.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D]
+    L.orc_num_threads.restype = ctypes.c_int
+    L.orc_set_num_threads.argtypes = [ctypes.c_int]
+    return L
 
 
 def _p(a):
@@ -95,13 +127,20 @@ def num_threads():
     return int(_load().orc_num_threads())
 
 
+def set_num_threads(n):
+    """OpenMP threads of the following oracle calls (both builds); results do not depend on it."""
+    _load().orc_set_num_threads(int(n))
+    if _lib_fma is not None:
+        _lib_fma.orc_set_num_threads(int(n))
+
+
 class Geometry:
     """All geometric coefficients recomputed from the grid description (O2): positions xyz [N][3],
     neighbour lists nbr [N][6] and control-volume vertices C [N][6][3] (None: triangle centroids
-    of xyz)."""
+    of xyz).  fma=True: the FMA-contracted build of the same source (a rounding yardstick, never the reference)."""
 
-    def __init__(self, xyz, nbr, nv, planet, C=None):
-        L = _load()
+    def __init__(self, xyz, nbr, nv, planet, C=None, fma=False):
+        L = self._L = _load(fma)
         self.xyz = _c(xyz)
         self.nbr = np.ascontiguousarray(nbr, dtype=np.int32)
         self.N = int(self.xyz.shape[0])
@@ -127,7 +166,7 @@ class Geometry:
     def __del__(self):
         try:
             if self._h:
-                _load().orc_geom_free(self._h)
+                self._L.orc_geom_free(self._h)
                 self._h = None
         except Exception:
             pass
@@ -137,7 +176,7 @@ class Geometry:
         vec = _c(vec)
         assert vec.shape == (self.N, self.nv, 3)
         out = np.empty((self.N, self.nv))
-        _load().orc_hdiv(self._h, _p(vec), _p(out))
+        self._L.orc_hdiv(self._h, _p(vec), _p(out))
         return out
 
     # Eq. 7 (difference form, projected): horizontal gradient of s [N][nv] -> [N][nv][3]
@@ -145,7 +184,7 @@ class Geometry:
         s = _c(s)
         assert s.shape == (self.N, self.nv)
         out = np.empty((self.N, self.nv, 3))
-        _load().orc_hgrad(self._h, _p(s), _p(out))
+        self._L.orc_hgrad(self._h, _p(s), _p(out))
         return out
 
     # L369-L371: horizontal Laplacian (gradient on the triangles, then Eq. 6) of s [N][nv] at radius r_k
@@ -153,7 +192,7 @@ class Geometry:
         s = _c(s)
         assert s.shape == (self.N, self.nv)
         out = np.empty((self.N, self.nv))
-        _load().orc_hlap(self._h, _p(s), _p(out))
+        self._L.orc_hlap(self._h, _p(s), _p(out))
         return out
 
     def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None, D_hyp=0.0, D_div=0.0):
@@ -170,10 +209,10 @@ class Geometry:
             k_T = None if forcing.get("k_T") is None else _c(forcing["k_T"])
             k_v = None if forcing.get("k_v") is None else _c(forcing["k_v"])
         if D_hyp == 0.0 and D_div == 0.0:
-            _load().orc_step(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
+            self._L.orc_step(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
                              _p(T_eq), _p(k_T), _p(k_v))
         else:
-            _load().orc_step_diffusion(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
+            self._L.orc_step_diffusion(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub),
                                        _p(T_eq), _p(k_T), _p(k_v), float(D_hyp), float(D_div))
         return rho, V, W, p
 
@@ -182,54 +221,54 @@ class Geometry:
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))
         N, nv = self.N, self.nv
         Frho, FV, FW, Fp, Frt = np.empty((N, nv)), np.empty((N, nv, 3)), np.empty((N, nv + 1)), np.empty((N, nv)), np.empty((N, nv))
-        _load().orc_diffusion_fluxes(self._h, _p(rho), _p(V), _p(W), _p(p), float(Kd), _p(Frho), _p(FV), _p(FW), _p(Fp), _p(Frt))
+        self._L.orc_diffusion_fluxes(self._h, _p(rho), _p(V), _p(W), _p(p), float(Kd), _p(Frho), _p(FV), _p(FW), _p(Fp), _p(Frt))
         return Frho, FV, FW, Fp, Frt
 
     def divergence_damping(self, V, W, Kd):
         V, W = _c(V), _c(W)
         out = np.empty((self.N, self.nv, 3))
-        _load().orc_divergence_damping(self._h, _p(V), _p(W), float(Kd), _p(out))
+        self._L.orc_divergence_damping(self._h, _p(V), _p(W), float(Kd), _p(out))
         return out
 
     # NEXT-2: Held-Suarez forcing from the evolving sigma (Eq. 51-55); hs = HELD_SUAREZ-like dict
     def step_held_suarez(self, rho, V, W, p, n_large, dt, n_sub, hs, D_hyp=0.0, D_div=0.0):
         rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
         h = _c(hs_array(hs))
-        _load().orc_step_held_suarez(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
+        self._L.orc_step_held_suarez(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
                                      float(D_hyp), float(D_div))
         return rho, V, W, p
 
     def forcing_held_suarez(self, rho, V, p, dt, hs):
         rho, V, p = (_c(x).copy() for x in (rho, V, p))
         h = _c(hs_array(hs))
-        _load().orc_forcing_held_suarez(self._h, float(dt), _p(rho), _p(V), _p(p), _p(h))
+        self._L.orc_forcing_held_suarez(self._h, float(dt), _p(rho), _p(V), _p(p), _p(h))
         return V, p
 
     # NEXT-2, hot Jupiter (Eq. 59-61); hj: dict with HJ_KEYS
     def step_hot_jupiter(self, rho, V, W, p, n_large, dt, n_sub, hj, D_hyp=0.0, D_div=0.0):
         rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
         h = _c(np.array([float(hj[k]) for k in HJ_KEYS]))
-        _load().orc_step_hot_jupiter(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
+        self._L.orc_step_hot_jupiter(self._h, _p(rho), _p(V), _p(W), _p(p), int(n_large), float(dt), int(n_sub), _p(h),
                                      float(D_hyp), float(D_div))
         return rho, V, W, p
 
     def forcing_hot_jupiter(self, rho, p, dt, hj):
         rho, p = _c(rho).copy(), _c(p).copy()
         h = _c(np.array([float(hj[k]) for k in HJ_KEYS]))
-        _load().orc_forcing_hot_jupiter(self._h, float(dt), _p(rho), _p(p), _p(h))
+        self._L.orc_forcing_hot_jupiter(self._h, float(dt), _p(rho), _p(p), _p(h))
         return p
 
     def diagnostics(self, rho, V, W, p):
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))
         m = ctypes.c_double()
         e = ctypes.c_double()
-        _load().orc_diagnostics(self._h, _p(rho), _p(V), _p(W), _p(p), ctypes.byref(m), ctypes.byref(e))
+        self._L.orc_diagnostics(self._h, _p(rho), _p(V), _p(W), _p(p), ctypes.byref(m), ctypes.byref(e))
         return m.value, e.value
 
     def tridiag_coefficients(self, delta, h, gt):
         h, gt = _c(h), _c(gt)
         a, b, c = (np.zeros(self.nv + 1) for _ in range(3))
-        _load().orc_tridiag_coefficients(self._h, float(delta), _p(h), _p(gt), _p(a), _p(b), _p(c))
+        self._L.orc_tridiag_coefficients(self._h, float(delta), _p(h), _p(gt), _p(a), _p(b), _p(c))
         return a, b, c
 
     def slow_terms(self, rho, V, W, p):
@@ -238,7 +277,7 @@ class Geometry:
         out = dict(slowV=np.zeros((N, nv, 3)), slowrho=np.zeros((N, nv)), Svr=np.zeros((N, nv + 1)),
                    slowp=np.zeros((N, nv)), slowrt=np.zeros((N, nv)), h=np.zeros((N, nv)),
                    th=np.zeros((N, nv)), gt=np.zeros((N, nv + 1)))
-        _load().orc_slow_terms(self._h, _p(rho), _p(V), _p(W), _p(p), *[_p(out[k]) for k in
+        self._L.orc_slow_terms(self._h, _p(rho), _p(V), _p(W), _p(p), *[_p(out[k]) for k in
                                ("slowV", "slowrho", "Svr", "slowp", "slowrt", "h", "th", "gt")])
         return out
 
@@ -247,7 +286,7 @@ class Geometry:
         dev: dict(rho_s, V_s, W_s, p_s, rt).  Returns the updated dev (copies)."""
         st = {k: _c(v) for k, v in stage.items()}
         dv = {k: _c(v).copy() for k, v in dev.items()}
-        _load().orc_substep(self._h, float(delta), _p(st["h"]), _p(st["th"]), _p(st["gt"]), _p(st["p_t"]),
+        self._L.orc_substep(self._h, float(delta), _p(st["h"]), _p(st["th"]), _p(st["gt"]), _p(st["p_t"]),
                             _p(st["slowV"]), _p(st["slowrho"]), _p(st["Svr"]), _p(st["slowp"]), _p(st["slowrt"]),
                             _p(dv["rho_s"]), _p(dv["V_s"]), _p(dv["W_s"]), _p(dv["p_s"]), _p(dv["rt"]))
         return dv

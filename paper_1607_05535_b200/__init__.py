@@ -288,7 +288,18 @@ class State:
         thor_state_set(self._h, *[_f64(a, s) for a, s in zip((rho, mom_h, W, p), self._shapes)])
 
     def get(self, out=None):
-        out = out if out is not None else tuple(np.empty(s) for s in self._shapes)
+        """out: four caller-owned C-contiguous float64 arrays of the state's shapes (checked: the library writes
+        through their raw pointers), or None for fresh ones."""
+        if out is None:
+            out = tuple(np.empty(s) for s in self._shapes)
+        else:
+            out = tuple(out)
+            if len(out) != 4:
+                raise ThorError(THOR_EINVAL, "State.get: need four output arrays (rho, mom_h, W, p)")
+            for a, shp in zip(out, self._shapes):
+                if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.shape == tuple(shp)
+                        and a.flags["C_CONTIGUOUS"] and a.flags["WRITEABLE"]):
+                    raise ThorError(THOR_EINVAL, "State.get: output arrays must be writeable C-contiguous float64 of shape %s" % (tuple(shp),))
         thor_state_get(self._h, *out)
         return out
 

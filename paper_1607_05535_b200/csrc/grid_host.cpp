@@ -201,7 +201,7 @@ double tri_area(V3 a, V3 b, V3 c) {   // spherical excess
 
 }  // namespace
 
-int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces) {
     if (level < 0 || level > 9 || nv < 2 || nv > 128) return THOR_EINVAL;
     if (!(P.radius > 0) || !(P.z_top > 0) || !(P.Rd > 0) || !(P.Cp > P.Rd) || !(P.p_ref > 0)) return THOR_EINVAL;
     g.level = level;
@@ -435,17 +435,29 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g) {
         }
     }
 
-    // --- vertical tables (R6: uniform dz; Eq. 27's radial operator)
+    // --- vertical tables (R6: uniform dz unless interface altitudes are given; Eq. 27's radial operator;
+    // Eq. 8-9 with k = 1 for the centre -> interface interpolation)
     g.dz = P.z_top / nv;
+    g.zh.resize(nv + 1);
+    for (int k = 0; k <= nv; ++k) g.zh[k] = z_interfaces ? z_interfaces[k] : k * g.dz;
     g.rinv.resize(nv); g.dlo.resize(nv); g.dhi.resize(nv); g.vol.resize(nv); g.zc.resize(nv);
+    g.rhinv.resize(nv); g.wl.assign(nv, 0.0); g.wh.assign(nv, 0.0); g.idz.assign(nv, 0.0);
     for (int k = 0; k < nv; ++k) {
-        double zc = (k + 0.5) * g.dz, rc = P.radius + zc;
-        double rl = P.radius + k * g.dz, ru = P.radius + (k + 1) * g.dz;
+        const double zl = g.zh[k], zu = g.zh[k + 1], dzk = z_interfaces ? zu - zl : g.dz;
+        const double zc = z_interfaces ? 0.5 * (zl + zu) : (k + 0.5) * g.dz, rc = P.radius + zc;
+        const double rl = P.radius + zl, ru = P.radius + zu;
         g.zc[k] = zc;
         g.rinv[k] = 1.0 / rc;
-        g.dlo[k] = rl * rl / (rc * rc * g.dz);
-        g.dhi[k] = ru * ru / (rc * rc * g.dz);
-        g.vol[k] = rc * rc * g.dz;
+        g.dlo[k] = rl * rl / (rc * rc * dzk);
+        g.dhi[k] = ru * ru / (rc * rc * dzk);
+        g.vol[k] = rc * rc * dzk;
+        g.rhinv[k] = 1.0 / rl;
+    }
+    for (int k = 1; k < nv; ++k) {
+        const double dc = g.zc[k] - g.zc[k - 1];
+        g.wl[k] = z_interfaces ? (g.zc[k] - g.zh[k]) / dc : 0.5;
+        g.wh[k] = z_interfaces ? (g.zh[k] - g.zc[k - 1]) / dc : 0.5;
+        g.idz[k] = 1.0 / dc;
     }
     return THOR_OK;
 }

@@ -38,11 +38,17 @@ struct HostGrid {
     std::vector<double> dlo;       // [nv] r_h,k^2   / (r_k^2 dz)
     std::vector<double> dhi;       // [nv] r_h,k+1^2 / (r_k^2 dz)
     std::vector<double> vol;       // [nv] r_k^2 dz
-    std::vector<double> zc;        // [nv] centre altitude
-    double dz = 0;
+    std::vector<double> zc;        // [nv] centre altitude (midpoint of the layer's interfaces)
+    std::vector<double> zh;        // [nv+1] interface altitudes, zh[0] = 0, zh[nv] = z_top (uniform unless given)
+    std::vector<double> rhinv;     // [nv] 1/r_h,k (lower interface of layer k)
+    // Eq. 8-9 with k = 1 at the lower interface of layer k >= 1 (0 for k = 0)
+    std::vector<double> wl, wh;    // [nv] weights of the centres below / above the interface
+    std::vector<double> idz;       // [nv] 1/(z_k - z_k-1)
+    double dz = 0;                 // z_top / nv (mean thickness)
 };
 
 // Builds everything above.  Returns THOR_OK or THOR_EINVAL / THOR_ENOMEM.
-int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g);
+// z_interfaces: nullptr (uniform layers, R6) or nv+1 strictly increasing altitudes from 0 to P.z_top.
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces = nullptr);
 
 }  // namespace thor

@@ -11,6 +11,7 @@
 #include <cstring>
 #include <cstdint>
 #include <initializer_list>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -45,9 +46,10 @@ struct DeviceGeom {
     int Npad = 0;
     int* nbr = nullptr;
     int* order = nullptr;
-    double *wdiv = nullptr, *wgrad = nullptr, *rhat = nullptr, *area = nullptr;
-    double *basis = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr, *wlap = nullptr;
+    double *wdiv = nullptr, *wgrad = nullptr, *area = nullptr;
+    double *frame = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr, *wlap = nullptr;
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr, *rhinv = nullptr;
+    double *wl = nullptr, *wh = nullptr, *idz = nullptr;
     // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
     int tcol = 0, hmax = 0;
     // NEXT-1 divergence damping as ONE stencil: -lap(grad D3) composed on the host over the two rings of a column
@@ -55,6 +57,8 @@ struct DeviceGeom {
     double* dd_coef = nullptr;        // [Npad][20][2] tangent-basis coefficients of (D3_m - D3_i), unit sphere (x -K_d / r^3)
     int* tile_halo = nullptr;
     unsigned char* tile_slots = nullptr;
+    // scratch of the host wrappers thor_apply_div/grad/lap (7 x N x nv doubles), allocated on first use
+    double* op_buf = nullptr;
 };
 
 // lane-group width G and layers per lane E of the record kernels; NVP = G*E padded layers
@@ -108,9 +112,37 @@ int upload(T** dst, const std::vector<T>& src) {
 
 // device copy of the geometry, padded to Npad columns (pad columns: own neighbour, zero weights)
 // and to kMaxLayers layers (pad layers: 0)
+void free_device_geom(DeviceGeom& d) {
+    cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.frame); cudaFree(d.area);
+    cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc); cudaFree(d.rhinv);
+    cudaFree(d.wl); cudaFree(d.wh); cudaFree(d.idz);
+    cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.dd_idx); cudaFree(d.dd_coef);
+    cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap); cudaFree(d.op_buf);
+    d = DeviceGeom();
+}
+
+int upload_device_geom(const thor_grid* grid);
+
+// The device copy belongs to ONE device (the current one at first use); a call with another current device is
+// refused instead of dereferencing foreign pointers.  Serialised: two threads may share a grid.
 int ensure_device_geom(const thor_grid* grid) {
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
     DeviceGeom& d = grid->d;
-    if (d.ready) return THOR_OK;
+    int dev = -1;
+    if (d.ready) {
+        CU(cudaGetDevice(&dev));
+        if (dev != d.device)
+            return fail(THOR_EINVAL, "grid lives on CUDA device " + std::to_string(d.device) + ", current device is " + std::to_string(dev));
+        return THOR_OK;
+    }
+    const int rc = upload_device_geom(grid);
+    if (rc != THOR_OK) free_device_geom(d);              // nothing half-uploaded is kept
+    return rc;
+}
+
+int upload_device_geom(const thor_grid* grid) {
+    DeviceGeom& d = grid->d;
     int n = 0;
     cudaError_t e = cudaGetDeviceCount(&n);
     if (e != cudaSuccess || n == 0)
@@ -122,10 +154,16 @@ int ensure_device_geom(const thor_grid* grid) {
     std::vector<int> nbr(size_t(Npad) * 8);
     std::vector<double> wdiv(size_t(Npad) * 24, 0.0), wgrad(size_t(Npad) * 18, 0.0), rhat(size_t(Npad) * 4, 0.0),
         area(Npad, 0.0), basis(size_t(Npad) * 8, 0.0), wdiv2(size_t(Npad) * 16, 0.0), wgrad2(size_t(Npad) * 12, 0.0),
-        wlap(size_t(Npad) * 8, 0.0);
+        wlap(size_t(Npad) * 8, 0.0), frame(size_t(Npad) * 12, 0.0);
     for (int c = 0; c < Npad; ++c) {
         for (int k = 0; k < 8; ++k) nbr[size_t(c) * 8 + k] = (c < N && k < 6) ? h.d_nbr[size_t(c) * 6 + k] : c;
-        if (c >= N) { rhat[size_t(c) * 4 + 2] = 1.0; basis[size_t(c) * 8] = 1.0; basis[size_t(c) * 8 + 4] = 1.0; continue; }
+        if (c >= N) {
+            rhat[size_t(c) * 4 + 2] = 1.0; basis[size_t(c) * 8] = 1.0; basis[size_t(c) * 8 + 4] = 1.0;
+            frame[size_t(c) * 12] = 1.0; frame[size_t(c) * 12 + 4] = 1.0; frame[size_t(c) * 12 + 8] = 1.0;
+            continue;
+        }
+        std::copy_n(&h.d_basis[size_t(c) * 6], 6, &frame[size_t(c) * 12]);
+        std::copy_n(&h.d_rhat[size_t(c) * 3], 3, &frame[size_t(c) * 12 + 6]);
         std::copy_n(&h.d_basis[size_t(c) * 6], 6, &basis[size_t(c) * 8]);
         std::copy_n(&h.d_wdiv2[size_t(c) * 14], 14, &wdiv2[size_t(c) * 16]);
         std::copy_n(&h.d_wgrad2[size_t(c) * 12], 12, &wgrad2[size_t(c) * 12]);
@@ -145,9 +183,8 @@ int ensure_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.order, h.order))) return rc;
     if ((rc = upload(&d.wdiv, wdiv))) return rc;
     if ((rc = upload(&d.wgrad, wgrad))) return rc;
-    if ((rc = upload(&d.rhat, rhat))) return rc;
+    if ((rc = upload(&d.frame, frame))) return rc;
     if ((rc = upload(&d.area, area))) return rc;
-    if ((rc = upload(&d.basis, basis))) return rc;
     if ((rc = upload(&d.wdiv2, wdiv2))) return rc;
     if ((rc = upload(&d.wgrad2, wgrad2))) return rc;
     if ((rc = upload(&d.wlap, wlap))) return rc;
@@ -156,11 +193,10 @@ int ensure_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.dhi, padded(h.dhi)))) return rc;
     if ((rc = upload(&d.vol, padded(h.vol)))) return rc;
     if ((rc = upload(&d.zc, padded(h.zc)))) return rc;
-    {
-        std::vector<double> rh(h.nv);
-        for (int k = 0; k < h.nv; ++k) rh[k] = 1.0 / (h.P.radius + k * h.dz);
-        if ((rc = upload(&d.rhinv, padded(rh)))) return rc;
-    }
+    if ((rc = upload(&d.rhinv, padded(h.rhinv)))) return rc;
+    if ((rc = upload(&d.wl, padded(h.wl)))) return rc;
+    if ((rc = upload(&d.wh, padded(h.wh)))) return rc;
+    if ((rc = upload(&d.idz, padded(h.idz)))) return rc;
     {   // composed operator of the divergence damping (RD4): F_i = -K_d P_i lap(grad D3)_i
         //   grad D3 at column c:  G_c = sum_j wgrad_cj (D3_nbr(c,j) - D3_c)
         //   lap of each Cartesian component: sum_c wlap_ic (G_c - G_i), then Eq. 28 at i and its tangent basis
@@ -249,11 +285,12 @@ Geom make_geom(const thor_grid* grid) {
     const DeviceGeom& d = grid->d;
     Geom g;
     g.N = h.N; g.Npad = d.Npad; g.nv = h.nv;
-    g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.rhat = d.rhat; g.area = d.area;
-    g.basis = d.basis; g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
+    g.nbr = d.nbr; g.wdiv = d.wdiv; g.wgrad = d.wgrad; g.frame = d.frame; g.area = d.area;
+    g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
     g.dd_idx = d.dd_idx; g.dd_coef = d.dd_coef;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
-    g.dz = h.dz; g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
+    g.wl = d.wl; g.wh = d.wh; g.idz = d.idz;
+    g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
     g.eosq[0] = 1.0;
@@ -293,6 +330,14 @@ Geom make_geom(const thor_grid* grid) {
 
 int flat_blocks(size_t n) { return int((n + 255) / 256); }
 
+// scratch of the host wrappers thor_apply_div/grad/lap: 7 N nv doubles, kept in the grid handle
+int op_scratch(const thor_grid* grid, double** buf) {
+    DeviceGeom& d = grid->d;
+    if (!d.op_buf) CU(cudaMalloc(reinterpret_cast<void**>(&d.op_buf), 7 * size_t(grid->h.N) * grid->h.nv * sizeof(double)));
+    *buf = d.op_buf;
+    return THOR_OK;
+}
+
 // fast path of the config-1 operators: even layer count <= 64 and 16-byte aligned arrays
 bool op_fast_path(int nv, std::initializer_list<const void*> ptrs) {
     if ((nv & 1) || nv > 64) return false;
@@ -312,8 +357,9 @@ bool op_fast_path(int nv, std::initializer_list<const void*> ptrs) {
         g_launches.fetch_add(1, std::memory_order_relaxed);                                        \
     } while (0)
 
-// L2 schedule of the two acoustic kernels; THOR_B200_TUNE="rev,k1_ahead,k2_ahead,tail"
-// overrides the defaults for measurement.
+// L2 schedule of the step kernels;
+// THOR_B200_TUNE="zigzag,k1_ahead,k2_ahead,tail,tma_stages,tma_ctas,stage_ahead,graph" overrides the defaults for
+// measurement.  Read at the top of every thor_step / thor_acoustic_substeps call (never inside a graph capture).
 struct TunePair { Tune k1, k2, ks; int zigzag, tma_stages, tma_ctas, graph; };
 TunePair tune() {
     int v[8] = {1, 0, 148, 148, 0, 4, 148, 1};
@@ -384,14 +430,21 @@ int launch_vertical_staged(const Geom& g, const DeviceGeom& d, double* S, double
     const size_t smem = NS * stage_doubles * sizeof(double) + NS * sizeof(unsigned long long);
     *done = false;
     if (d.hmax <= 0 || d.tcol != TCOL || smem > kSmemPerBlockMax) return THOR_OK;
-    static size_t configured = 0;
-    static int n_sm = 0;
-    if (configured < smem) {
-        CU(cudaFuncSetAttribute(k_vertical_staged<G, E, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
-        int dev = 0;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-        configured = smem;
+    // the shared-memory opt-in is per device and per function: keyed on the device, set under a lock
+    static std::mutex mu;
+    static size_t configured[64] = {};
+    static int sm_count[64] = {};
+    int dev = 0, n_sm = 0;
+    CU(cudaGetDevice(&dev));
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        const int slot = dev & 63;
+        if (configured[slot] < smem) {
+            CU(cudaFuncSetAttribute(k_vertical_staged<G, E, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+            CU(cudaDeviceGetAttribute(&sm_count[slot], cudaDevAttrMultiProcessorCount, dev));
+            configured[slot] = smem;
+        }
+        n_sm = sm_count[slot];
     }
     const int ntiles = g.Npad / TCOL;
     const int grid = std::min(ntiles, n_sm * std::max(1, tn.tma_ctas));
@@ -459,12 +512,7 @@ int thor_grid_get(const thor_grid* grid, thor_grid_view* out) {
 
 void thor_grid_destroy(thor_grid* grid) {
     if (!grid) return;
-    DeviceGeom& d = grid->d;
-    if (d.ready) {
-        cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.rhat); cudaFree(d.area);
-        cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc); cudaFree(d.rhinv);
-        cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.dd_idx); cudaFree(d.dd_coef); cudaFree(d.basis); cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap);
-    }
+    if (grid->d.ready) free_device_geom(grid->d);
     delete grid;
 }
 
@@ -560,16 +608,19 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
     for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
         const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
         const double delta = stage == 1 ? dt / 3.0 : dt / n;
-        THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks));
-        THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks));
-        if (Kd_hyp > 0.0) {                                            // Fig. 6 large-step 2 (NEXT-1)
-            THOR_DISPATCH(k_diff0, nv, Npad, st, g, S, s->X);
-            THOR_DISPATCH(k_diff1, nv, Npad, st, g, S, s->X);
-            THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp);
+        // Fig. 6 large-steps 1-3; with NEXT-1 on, the same two kernels also produce w, the first Laplacians
+        // (RD2) and D3^[t] (RD4), so that the only extra launch per stage is the second Laplacian
+        const int dd = Kd_div > 0.0 ? (stage == 1 ? 2 : 1) : 0;
+        THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks), Kd_hyp > 0.0 ? s->X : nullptr);
+        if (Kd_hyp > 0.0) {
+            THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
+            THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks));
+        } else {
+            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
         }
-        if (Kd_div > 0.0) THOR_DISPATCH(k_dd1, nv, Npad, st, g, S, s->X);   // D3^[t] and the first substep's D3
         for (int sub = 0; sub < ns; ++sub) {
-            if (Kd_div > 0.0) THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div);   // + Fig. 6 small-step 1
+            if (Kd_div > 0.0)                                           // + Fig. 6 small-step 1
+                THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, sub == 0 ? int(X_D3N) : int(X_D3));
             else THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
             TunePair t2 = tn;
             t2.k2 = dir(tn.k2);
@@ -590,6 +641,8 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (n_large < 0 || !(dt > 0) || n < 2 || (n & 1)) return fail(THOR_EINVAL, "thor_step: need n_large >= 0, dt > 0, even n >= 2");
     cudaStream_t st = s->stream;
     if (forcing && (s->hs.on || s->hj.on)) return fail(THOR_EINVAL, "thor_step: table forcing and evolving-sigma forcing are exclusive");
+    if (forcing && forcing->resident && !(s->has_Teq || s->has_kT || s->has_kv))
+        return fail(THOR_EINVAL, "thor_step: forcing->resident is set but no table was uploaded to this state");
     if (forcing && !forcing->resident) {
         int rc;
         s->has_Teq = forcing->T_eq != nullptr; s->has_kT = forcing->k_T != nullptr; s->has_kv = forcing->k_v != nullptr;
@@ -784,7 +837,7 @@ int thor_apply_lap(const thor_grid* grid, const double* sfield, double* out) {
     const int N = h.N, nv = h.nv;
     const size_t nc = size_t(N) * nv;
     double* buf = nullptr;   // [staging][s][out]
-    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 3 * nc * sizeof(double)));
+    if (int rb = op_scratch(grid, &buf)) return rb;
     double *stg = buf, *sd = buf + nc, *od = sd + nc;
     cudaError_t e = cudaMemcpy(stg, sfield, nc * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
@@ -797,7 +850,6 @@ int thor_apply_lap(const thor_grid* grid, const double* sfield, double* out) {
             e = cudaMemcpy(out, stg, nc * sizeof(double), cudaMemcpyDeviceToHost);
         }
     }
-    cudaFree(buf);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_lap: ") + cudaGetErrorString(e));
     return THOR_OK;
@@ -812,7 +864,7 @@ int thor_apply_div(const thor_grid* grid, const double* vec, double* out) {
     const int N = h.N, nv = h.nv;
     const size_t nc = size_t(N) * nv;
     double* buf = nullptr;   // [3nc staging][vx][vy][vz][out]
-    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 7 * nc * sizeof(double)));
+    if (int rb = op_scratch(grid, &buf)) return rb;
     double *stg = buf, *vx = buf + 3 * nc, *vy = vx + nc, *vz = vy + nc, *o = vz + nc;
     cudaError_t e = cudaMemcpy(stg, vec, 3 * nc * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
@@ -827,7 +879,6 @@ int thor_apply_div(const thor_grid* grid, const double* vec, double* out) {
             e = cudaMemcpy(out, stg, nc * sizeof(double), cudaMemcpyDeviceToHost);
         }
     }
-    cudaFree(buf);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_div: ") + cudaGetErrorString(e));
     return THOR_OK;
@@ -841,7 +892,7 @@ int thor_apply_grad(const thor_grid* grid, const double* sfield, double* out) {
     const int N = h.N, nv = h.nv;
     const size_t nc = size_t(N) * nv;
     double* buf = nullptr;   // [3nc staging][s][gx][gy][gz]
-    CU(cudaMalloc(reinterpret_cast<void**>(&buf), 7 * nc * sizeof(double)));
+    if (int rb = op_scratch(grid, &buf)) return rb;
     double *stg = buf, *sd = buf + 3 * nc, *gx = sd + nc, *gy = gx + nc, *gz = gy + nc;
     cudaError_t e = cudaMemcpy(stg, sfield, nc * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
@@ -856,7 +907,6 @@ int thor_apply_grad(const thor_grid* grid, const double* sfield, double* out) {
             e = cudaMemcpy(out, stg, 3 * nc * sizeof(double), cudaMemcpyDeviceToHost);
         }
     }
-    cudaFree(buf);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_apply_grad: ") + cudaGetErrorString(e));
     return THOR_OK;

@@ -39,43 +39,53 @@ enum Field : int {
     F_RHOS, F_WS, F_RTS,         // rho*, W* = (rho v_r)*, (rho theta)*
     F_SRHO, F_SP, F_SW, F_SRT,   // slow terms of Eq. 32, 40, 42, 35
     F_FA, F_FI, F_FC,            // LU factors of the tridiagonal matrix of Eq. 37
-    F_PT,                        // p^[t]
+    F_PT,                        // p^[t]     (gathered by the slow-term kernel)
     F_SVA, F_SVB,                // slow term of Eq. 33, tangent basis
-    // --- stage reference state Phi^[t] (R1) and the un-projected velocity (L268), Cartesian
-    F_VXT, F_VYT, F_VZT, F_UX, F_UY, F_UZ, F_RHOT, F_WT,
-    // --- Phi^n (the prognostic state between large steps) and (rho theta)^n
+    // --- stage reference state Phi^[t] (R1): horizontal momentum in the tangent basis, 1/rho, W, rho.
+    //     The slow-term kernel gathers VAT, VBT, IRT, WT (+ TH, PT) from the neighbours and rebuilds the
+    //     un-projected velocity u = (V + I_c[W] r)/rho of L268 and h = Cp p/(Rd rho) from them.
+    F_VAT, F_VBT, F_IRT, F_WT, F_RHOT,
+    // --- Phi^n (the prognostic state between large steps, Cartesian momentum: what thor_state_get returns
+    //     bit-exactly) and (rho theta)^n
     F_RHON, F_VXN, F_VYN, F_VZN, F_WN, F_PN, F_RTN,
     NF
 };
 
-// rows of the NEXT-1 work slab X (hyper-diffusion and divergence damping, see k_diff0 .. k_dd3)
+// rows of the NEXT-1 work slab X (hyper-diffusion and divergence damping)
 enum XField : int {
-    X_VX = 0, X_VY, X_VZ, X_W, X_T,              // k_diff0: v = V/rho, w = W/I_h[rho], T = p/(Rd rho) of Phi^[t]
-    X_Q0, X_Q1, X_Q2, X_Q3, X_Q4, X_Q5,          // k_diff1: lap(rho), rho lap(v_x..z), rho_h lap(w), rho lap(T)
-    XF,
-    X_D3 = 0, X_D3T = 1          // divergence damping reuses rows 0-1 during the substeps
+    X_W = 0,                                     // k_stage_prepare: w = W/I_h[rho] of Phi^[t] on interior interfaces
+    X_Q0, X_Q1, X_Q2, X_Q3, X_Q4, X_Q5,          // k_slow_terms<HYP>: lap(rho), rho lap(v_x..z), rho_h lap(w), rho lap(T)
+    X_D3,                                        // 3-D divergence of the current momentum (column-solve kernel, per substep)
+    X_D3T,                                       // ... of the stage reference state (k_slow_terms, per stage)
+    X_D3N,                                       // ... of Phi^n (k_slow_terms of stage 1): the first substep's D3 of every stage
+    XF
 };
 
 struct Geom {                 // device pointers, device column order, padded to Npad columns
     int N, Npad, nv;
     const int* nbr;           // [Npad][8]   6 neighbours (pentagons, pad columns: self), 2 x self
-    const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad
-    const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)
+    const double* wdiv;       // [Npad][24]  7 x 3 divergence weights (Eq. 4-6 expanded), 3 pad        (config-1 operators)
+    const double* wgrad;      // [Npad][18]  6 x 3 gradient weights (Eq. 7, projected by Eq. 28)       (config-1 operators)
     const double* wlap;       // [Npad][8]   6 Laplacian weights (Eq. 7 on the triangles, then Eq. 6; L369-L371), 2 pad
     const int* dd_idx;        // [Npad][20]  NEXT-1 divergence damping composed over two rings: columns m ...
     const double* dd_coef;    // [Npad][20][2] ... and tangent coefficients of (D3_m - D3_i); F_dd = -K_d/r^3 sum_m coef_m (D3_m - D3_i)
-    const double* rhat;       // [Npad][4]   unit vector of the column, 1 pad
-    const double* basis;      // [Npad][8]   tangent basis e1(3), e2(3), 2 pad
+    const double* frame;      // [Npad][12]  tangent basis e1(3), e2(3), unit vector r(3) of the column, 3 pad
     const double* wdiv2;      // [Npad][16]  7 x 2 divergence weights contracted with the basis of column j, 2 pad
     const double* wgrad2;     // [Npad][12]  6 x 2 gradient weights contracted with the column's own basis
     const double* area;       // [Npad]
-    const double* rinv;       // [128] 1/r_k              (pad layers: 0)
-    const double* dlo;        // [128] r_h,k^2/(r_k^2 dz)
-    const double* dhi;        // [128] r_h,k+1^2/(r_k^2 dz)
-    const double* vol;        // [128] r_k^2 dz
-    const double* zc;         // [128]
-    const double* rhinv;      // [128] 1/r_h,k: radius of the LOWER interface of layer k (pad layers: 0)
-    double dz, omega, gravity, Rd, Cp, p_ref;
+    // per-layer tables [128]; layers need not be uniform (NEXT-3): layer k spans the interfaces z_h,k .. z_h,k+1,
+    // its centre is their midpoint
+    const double* rinv;       // 1/r_k              (pad layers: 0)
+    const double* dlo;        // r_h,k^2/(r_k^2 dz_k)
+    const double* dhi;        // r_h,k+1^2/(r_k^2 dz_k)
+    const double* vol;        // r_k^2 dz_k
+    const double* zc;         // centre altitude
+    const double* rhinv;      // 1/r_h,k: radius of the LOWER interface of layer k (pad layers: 0)
+    // Eq. 8-9 with k = 1 at the LOWER interface of layer k (0 for k = 0 and on pads):
+    const double* wl;         // weight of the centre below:  (z_k - z_h,k)/(z_k - z_k-1)
+    const double* wh;         // weight of the centre above:  (z_h,k - z_k-1)/(z_k - z_k-1)
+    const double* idz;        // 1/(z_k - z_k-1), the spacing of G_h
+    double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
 
@@ -175,17 +185,11 @@ __device__ __forceinline__ void st_row(double* p, const double (&v)[E]) {
     for (int i = 0; i < E / 2; ++i) reinterpret_cast<double2*>(p)[i] = make_double2(v[2 * i], v[2 * i + 1]);
 }
 
-__device__ __forceinline__ double3 ld_rhat(const double* rhat, int col) {   // [Npad][4]
-    const double2 a = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col));
-    const double2 b = __ldg(reinterpret_cast<const double2*>(rhat) + 2 * size_t(col) + 1);
-    return make_double3(a.x, a.y, b.x);
-}
-
-struct Basis { double3 e1, e2; };
-__device__ __forceinline__ Basis ld_basis(const double* basis, int col) {   // [Npad][8]
-    const double2* p = reinterpret_cast<const double2*>(basis) + 4 * size_t(col);
-    const double2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-    return Basis{make_double3(a.x, a.y, b.x), make_double3(b.y, c.x, c.y)};
+struct Frame { double3 e1, e2, r; };
+__device__ __forceinline__ Frame ld_frame(const double* frame, int col) {   // [Npad][12]
+    const double2* p = reinterpret_cast<const double2*>(frame) + 6 * size_t(col);
+    const double2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2), d = __ldg(p + 3), e = __ldg(p + 4);
+    return Frame{make_double3(a.x, a.y, b.x), make_double3(b.y, c.x, c.y), make_double3(d.x, d.y, e.x)};
 }
 
 // Per-column stencil weights staged once per warp in shared memory (every lane of a column group
@@ -477,24 +481,25 @@ k_lap2(Geom g, const double* __restrict__ s, double* __restrict__ out) {
 
 // ---------------------------------------------------------------------------------------------
 // S1: stage preparation (column-local).  Fig. 6 large-step 4 of the previous stage and
-// large-step 1 of this one:  Phi^[t] <- Phi^n (stage 1) or Phi^[t] + Phi* (stages 2, 3);
-// h = Cp p/(Rd rho) (Eq. 38, G9), theta, u = (V + I_c[W] r)/rho (L268), the LU factors of the
-// tridiagonal matrix of Eq. 37 (g~ of Eq. 39 inside; coefficients: DESIGN.md "tridiagonal", R8) for
-// this stage's substep length delta, and the initial deviations of Eq. 31 (R1: every stage starts
-// from t_n).  The matrix does not change between the substeps of a stage, so it is factorised
-// once here and the substeps only run the two sweeps.
+// large-step 1 of this one:  Phi^[t] <- Phi^n (stage 1) or Phi^[t] + Phi* (stages 2, 3), the
+// horizontal momentum kept as its two components in the column's tangent basis;
+// h = Cp p/(Rd rho) (Eq. 38, G9), theta, 1/rho, the LU factors of the tridiagonal matrix of Eq. 37
+// (g~ of Eq. 39 inside; coefficients: DESIGN.md "tridiagonal", R8) for this stage's substep length
+// delta, and the initial deviations of Eq. 31 (R1: every stage starts from t_n).  The matrix does not
+// change between the substeps of a stage, so it is factorised once here and the substeps only run
+// the two sweeps.  Vertical operators: Eq. 8-9 with k = 1 on possibly non-uniform layers
+// (Geom::wl, wh, idz).  Xw != null (NEXT-1 hyper-diffusion on): also w = W/I_h[rho] for its Laplacian.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn) {
+k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn, double* __restrict__ Xw) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
         prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHON, stage == 1 ? 6 : 7);
         if (stage > 1) {
             prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
-            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 3);
-            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHOT, 2);
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAT, 5);
         }
     }
     constexpr int NVP = Map<G, E>::NVP;
@@ -505,11 +510,17 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 #pragma unroll
     for (int e = 0; e < E; ++e) real[e] = (L.k0 + e < nv) && (L.col < g.N);
 
-    const Basis B = ld_basis(g.basis, L.col);
-    double rho[E], Vx[E], Vy[E], Vz[E], W[E], p[E], d[E];
+    const Frame fr = ld_frame(g.frame, L.col);
+    double rho[E], va[E], vb[E], W[E], p[E], d[E];
     if (stage == 1) {
+        double Vx[E], Vy[E], Vz[E];
         ld_rw<E>(me + F_RHON * NVP, rho); ld_rw<E>(me + F_VXN * NVP, Vx); ld_rw<E>(me + F_VYN * NVP, Vy);
         ld_rw<E>(me + F_VZN * NVP, Vz);   ld_rw<E>(me + F_WN * NVP, W);   ld_rw<E>(me + F_PN * NVP, p);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            va[e] = Vx[e] * fr.e1.x + Vy[e] * fr.e1.y + Vz[e] * fr.e1.z;
+            vb[e] = Vx[e] * fr.e2.x + Vy[e] * fr.e2.y + Vz[e] * fr.e2.z;
+        }
     } else {
         auto add = [&](int ft, int fs, double (&out)[E]) {
             ld_rw<E>(me + ft * NVP, out); ld_rw<E>(me + fs * NVP, d);
@@ -517,41 +528,31 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
             for (int e = 0; e < E; ++e) out[e] += d[e];
         };
         add(F_RHOT, F_RHOS, rho); add(F_WT, F_WS, W); add(F_PT, F_PS, p);
-        double va[E], vb[E];                                   // V^[t] += a e1 + b e2
-        ld_rw<E>(me + F_VXT * NVP, Vx); ld_rw<E>(me + F_VYT * NVP, Vy); ld_rw<E>(me + F_VZT * NVP, Vz);
-        ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, vb);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            Vx[e] += va[e] * B.e1.x + vb[e] * B.e2.x;
-            Vy[e] += va[e] * B.e1.y + vb[e] * B.e2.y;
-            Vz[e] += va[e] * B.e1.z + vb[e] * B.e2.z;
-        }
+        add(F_VAT, F_VAS, va);    add(F_VBT, F_VBS, vb);
     }
 #pragma unroll
     for (int e = 0; e < E; ++e)
-        if (!real[e]) { rho[e] = 1.0; p[e] = g.p_ref; Vx[e] = Vy[e] = Vz[e] = W[e] = 0.0; }
+        if (!real[e]) { rho[e] = 1.0; p[e] = g.p_ref; va[e] = vb[e] = W[e] = 0.0; }
 
-    const double3 rh = ld_rhat(g.rhat, L.col);
-    double h[E], th[E], rtt[E], Wup[E], ux[E], uy[E], uz[E];
-    above<G, E>(W, Wup, L.gl, 0.0);
+    double h[E], th[E], rtt[E], ir[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         h[e] = g.Cp * p[e] / (g.Rd * rho[e]);
         rtt[e] = eos_rt(p[e], g.Rd, g.p_ref, 1.0 / gam);
         th[e] = rtt[e] / rho[e];
-        const double wc = 0.5 * (W[e] + Wup[e]);                            // I_c[W]; the lid's W is the pad's 0
-        const double ir = 1.0 / rho[e];
-        ux[e] = (Vx[e] + wc * rh.x) * ir; uy[e] = (Vy[e] + wc * rh.y) * ir; uz[e] = (Vz[e] + wc * rh.z) * ir;
+        ir[e] = 1.0 / rho[e];
     }
     // interface quantities on the lower interface of each layer
-    double pb[E], rb[E], hb[E], hh[E], gt[E];
+    double pb[E], rb[E], hb[E], hh[E], gt[E], rhoh[E], wl[E], wh[E], idz[E];
     below<G, E>(p, pb, L.gl, 0.0); below<G, E>(rho, rb, L.gl, 1.0); below<G, E>(h, hb, L.gl, 0.0);
+    ld_nc<E>(g.wl + L.k0, wl); ld_nc<E>(g.wh + L.k0, wh); ld_nc<E>(g.idz + L.k0, idz);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
         const bool in = k >= 1 && k < nv;                 // interior interface
-        hh[e] = in ? 0.5 * (hb[e] + h[e]) : 0.0;          // I_h[h]
-        gt[e] = in ? ((p[e] - pb[e]) / g.dz) / (0.5 * (rb[e] + rho[e])) : 0.0;   // Eq. 39
+        rhoh[e] = in ? wl[e] * rb[e] + wh[e] * rho[e] : 1.0;                      // I_h[rho]
+        hh[e] = in ? wl[e] * hb[e] + wh[e] * h[e] : 0.0;                          // I_h[h]
+        gt[e] = in ? ((p[e] - pb[e]) * idz[e]) / rhoh[e] : 0.0;                   // Eq. 39
     }
     double hhb[E], hha[E], gtb[E], gta[E], dlo[E], dhi[E], dlob[E], dhib[E];
     below<G, E>(hh, hhb, L.gl, 0.0); above<G, E>(hh, hha, L.gl, 0.0);
@@ -559,13 +560,14 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
     ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
     below<G, E>(dlo, dlob, L.gl, 0.0); below<G, E>(dhi, dhib, L.gl, 0.0);
     double ta[E], tb[E], tc[E];
-    const double d2 = delta * delta, ck = d2 * kv / g.dz, cg = 0.5 * d2 * g.gravity;
+    const double d2 = delta * delta, d2g = d2 * g.gravity;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         // hh, g~ are 0 on the lid and on the ground: a_1 and c_(nv-1) multiply the zero boundary values
-        tc[e] = -ck * (dhi[e] * hha[e] - 0.5 * gta[e]) - cg * dhi[e];
-        ta[e] = -ck * (dlob[e] * hhb[e] + 0.5 * gtb[e]) + cg * dlob[e];
-        tb[e] = 1.0 + ck * hh[e] * (dlo[e] + dhib[e]) - cg * (dhib[e] - dlo[e]);
+        const double ck = d2 * kv * idz[e];
+        tc[e] = -ck * (dhi[e] * hha[e] - 0.5 * gta[e]) - d2g * wh[e] * dhi[e];
+        ta[e] = -ck * (dlob[e] * hhb[e] + 0.5 * gtb[e]) + d2g * wl[e] * dlob[e];
+        tb[e] = 1.0 + ck * hh[e] * (dlo[e] + dhib[e]) - d2g * (wl[e] * dhib[e] - wh[e] * dlo[e]);
     }
     // Thomas forward elimination of the matrix (L339): b'_k = b_k - a_k c_(k-1)/b'_(k-1).  The leading
     // minors theta_k = b'_1 ... b'_k obey the LINEAR recurrence theta_k = b_k theta_(k-1) - a_k c_(k-1) theta_(k-2),
@@ -619,11 +621,18 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
             fc[e] = tc[e] * fi[e];
         }
     }
-    st_row<E>(me + F_RHOT * NVP, rho); st_row<E>(me + F_VXT * NVP, Vx); st_row<E>(me + F_VYT * NVP, Vy);
-    st_row<E>(me + F_VZT * NVP, Vz);   st_row<E>(me + F_WT * NVP, W);   st_row<E>(me + F_PT * NVP, p);
+    st_row<E>(me + F_RHOT * NVP, rho); st_row<E>(me + F_IRT * NVP, ir);  st_row<E>(me + F_WT * NVP, W);
+    st_row<E>(me + F_PT * NVP, p);     st_row<E>(me + F_VAT * NVP, va);  st_row<E>(me + F_VBT * NVP, vb);
     st_row<E>(me + F_H * NVP, h);      st_row<E>(me + F_TH * NVP, th);
-    st_row<E>(me + F_UX * NVP, ux);    st_row<E>(me + F_UY * NVP, uy);  st_row<E>(me + F_UZ * NVP, uz);
-    st_row<E>(me + F_FA * NVP, fa);    st_row<E>(me + F_FI * NVP, fi);  st_row<E>(me + F_FC * NVP, fc);
+    st_row<E>(me + F_FA * NVP, fa);    st_row<E>(me + F_FI * NVP, fi);   st_row<E>(me + F_FC * NVP, fc);
+    if (Xw) {                                                    // NEXT-1: w on interior interfaces (0 elsewhere)
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int k = L.k0 + e;
+            d[e] = (k >= 1 && k < nv) ? W[e] / rhoh[e] : 0.0;
+        }
+        st_row<E>(Xw + size_t(L.col) * (size_t(XF) * NVP) + L.k0 + X_W * NVP, d);
+    }
 
     // Eq. 31: Phi*(0) = Phi^n - Phi^[t]; (rho theta)*(0) = (rho theta)^n - (rho theta)^[t]
     if (stage == 1) {
@@ -641,13 +650,14 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
             st_row<E>(me + fs * NVP, d);
         };
         dev(F_RHON, F_RHOS, rho); dev(F_WN, F_WS, W); dev(F_PN, F_PS, p); dev(F_RTN, F_RTS, rtt);
-        double dx[E], dy[E], dz[E], va[E], vb[E];              // (V^n - V^[t]) in the tangent basis
+        double dx[E], dy[E], dz[E];                             // V^n in the tangent basis, minus V^[t]
         ld_rw<E>(me + F_VXN * NVP, dx); ld_rw<E>(me + F_VYN * NVP, dy); ld_rw<E>(me + F_VZN * NVP, dz);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            dx[e] -= Vx[e]; dy[e] -= Vy[e]; dz[e] -= Vz[e];
-            va[e] = real[e] ? dx[e] * B.e1.x + dy[e] * B.e1.y + dz[e] * B.e1.z : 0.0;
-            vb[e] = real[e] ? dx[e] * B.e2.x + dy[e] * B.e2.y + dz[e] * B.e2.z : 0.0;
+            const double an = dx[e] * fr.e1.x + dy[e] * fr.e1.y + dz[e] * fr.e1.z;
+            const double bn = dx[e] * fr.e2.x + dy[e] * fr.e2.y + dz[e] * fr.e2.z;
+            va[e] = real[e] ? an - va[e] : 0.0;
+            vb[e] = real[e] ? bn - vb[e] : 0.0;
         }
         st_row<E>(me + F_VAS * NVP, va); st_row<E>(me + F_VBS * NVP, vb);
     }
@@ -655,130 +665,196 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 
 // ---------------------------------------------------------------------------------------------
 // S2: slow terms of the stage (Fig. 6 large-step 3; RHS of Eq. 32-35 and Eq. 42; O4 with R7).
-// Gathers V^[t](3), h, theta, u(3), p^[t] from the 6 neighbours.
+// Gathers six rows from the column and its 6 neighbours: V^[t] (2 tangent components), theta, p^[t],
+// 1/rho^[t], W^[t]; the neighbour's un-projected velocity u = (V + I_c[W] r)/rho (L268) is rebuilt
+// from them with the neighbour's frame (staged in shared memory per column), h = Cp p/(Rd rho) likewise.
+// The pressure gradient is accumulated directly in the column's tangent basis (wgrad2).
+// HYP (NEXT-1 hyper-diffusion on, X != null): the same loop also forms the first Laplacians of
+// rho, v = V/rho (Cartesian components), w and T (RD2) and stores them weighted for the second one.
+// dd: 1 = also store D3^[t] = div_h V^[t] + D_c[W^[t]] (RD4); 2 (stage 1, where Phi^[t] = Phi^n) = and D3^n.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
-k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
+template <int G, int E, bool HYP>
+__device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restrict__ S, const Tune& tn,
+                                                 double* __restrict__ X, int dd) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_H, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 8);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_TH, 1);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAT, 5);
     }
     constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t REC = Map<G, E>::REC;
+    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
+    constexpr int CPB = kWarpsPerBlock * 32 / G;
     double* me = S + size_t(L.col) * REC + L.k0;
     const int nv = g.nv;
-    const double kv = g.Rd / (g.Cp - g.Rd);
-    __shared__ double wsm[kWarpsPerBlock * 32 / G][24 + 18];
+    const double kv = g.Rd / (g.Cp - g.Rd), cph = g.Cp / g.Rd;
+    // per column group: 14 divergence weights (+2 pad), 12 gradient weights, the frames of the column and its
+    // 6 neighbours (7 x 12), 6 Laplacian weights (+2 pad), 8 neighbour slots
+    __shared__ double wsm[CPB][16 + 12 + 84 + 8];
+    __shared__ int nsm[CPB][8];
     double* wdv = wsm[threadIdx.x / G];
-    double* wgv = wdv + 24;
-    stage_weights<G>(g.wdiv + size_t(L.col) * 24, wdv, 12, L.gl);
-    stage_weights<G>(g.wgrad + size_t(L.col) * 18, wgv, 9, L.gl);
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
+    double* wgv = wdv + 16;
+    double* frm = wgv + 12;
+    double* wlp = frm + 84;
+    int* nbs = nsm[threadIdx.x / G];
+    stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
+    stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, wgv, 6, L.gl);
+    if (HYP) stage_weights<G>(g.wlap + size_t(L.col) * 8, wlp, 4, L.gl);
+    for (int i = L.gl; i < 8; i += G) nbs[i] = i == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 8 + i - 1);
+    __syncwarp();
+    for (int i = L.gl; i < 42; i += G)
+        reinterpret_cast<double2*>(frm)[i] = __ldg(reinterpret_cast<const double2*>(g.frame) + 6 * size_t(nbs[i / 6]) + i % 6);
+    const int nb[7] = {nbs[0], nbs[1], nbs[2], nbs[3], nbs[4], nbs[5], nbs[6]};
     __syncwarp();
 
     double p0[E];
-    ld_nc<E>(me + F_PT * NVP, p0);
-    double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], gpx[E], gpy[E], gpz[E];
+    double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], ga[E], gb[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = Ax[e] = Ay[e] = Az[e] = gpx[e] = gpy[e] = gpz[e] = 0.0;
+    for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = Ax[e] = Ay[e] = Az[e] = ga[e] = gb[e] = 0.0;
+    // NEXT-1: first Laplacians sum_j wlap_j (s_j - s_0) of rho, v_x, v_y, v_z, w, T
+    double s0[HYP ? 6 : 1][E], lp[HYP ? 6 : 1][E];
+    if (HYP) {
+#pragma unroll
+        for (int f = 0; f < 6; ++f)
+#pragma unroll
+            for (int e = 0; e < E; ++e) lp[f][e] = 0.0;
+    }
 #pragma unroll
     for (int j = 0; j < 7; ++j) {
         const double* q = S + size_t(nb[j]) * REC + L.k0;
-        const double wx = wdv[3 * j], wy = wdv[3 * j + 1], wz = wdv[3 * j + 2];
-        double x[E], y[E], z[E], hj[E], tj[E], ujx[E], ujy[E], ujz[E], pj[E];
-        ld_nc<E>(q + F_VXT * NVP, x); ld_nc<E>(q + F_VYT * NVP, y); ld_nc<E>(q + F_VZT * NVP, z);
-        ld_nc<E>(q + F_H * NVP, hj);  ld_nc<E>(q + F_TH * NVP, tj);
-        ld_nc<E>(q + F_UX * NVP, ujx); ld_nc<E>(q + F_UY * NVP, ujy); ld_nc<E>(q + F_UZ * NVP, ujz);
-        if (j > 0) {
-            ld_nc<E>(q + F_PT * NVP, pj);
-            const double gx = wgv[3 * (j - 1)], gy = wgv[3 * (j - 1) + 1], gz = wgv[3 * (j - 1) + 2];
+        const double wa = wdv[2 * j], wb = wdv[2 * j + 1];
+        const double* f = frm + 12 * j;
+        double a[E], b[E], tj[E], pj[E], irj[E], Wj[E], Wup[E];
+        ld_nc<E>(q + F_VAT * NVP, a);  ld_nc<E>(q + F_VBT * NVP, b);  ld_nc<E>(q + F_TH * NVP, tj);
+        ld_nc<E>(q + F_PT * NVP, pj);  ld_nc<E>(q + F_IRT * NVP, irj); ld_nc<E>(q + F_WT * NVP, Wj);
+        above<G, E>(Wj, Wup, L.gl, 0.0);
+        if (j == 0) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) p0[e] = pj[e];
+        } else {
+            const double g1 = wgv[2 * (j - 1)], g2 = wgv[2 * (j - 1) + 1];
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                const double d = pj[e] - p0[e];
-                gpx[e] = fma(gx, d, gpx[e]); gpy[e] = fma(gy, d, gpy[e]); gpz[e] = fma(gz, d, gpz[e]);
+                const double dp = pj[e] - p0[e];
+                ga[e] = fma(g1, dp, ga[e]); gb[e] = fma(g2, dp, gb[e]);
             }
         }
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double d = fma(wx, x[e], fma(wy, y[e], wz * z[e]));      // w_j . V_j
+            const double d = fma(wa, a[e], wb * b[e]);                        // w_j . V_j
+            const double wc = 0.5 * (Wj[e] + Wup[e]);                         // I_c[W]_j; the lid's W is the pad's 0
+            const double t = d * irj[e];
             divV[e] += d;
-            divhV[e] = fma(hj[e], d, divhV[e]);
+            divhV[e] = fma(cph * pj[e] * irj[e], d, divhV[e]);                // h_j = Cp p_j/(Rd rho_j)
             divtV[e] = fma(tj[e], d, divtV[e]);
-            Ax[e] = fma(ujx[e], d, Ax[e]); Ay[e] = fma(ujy[e], d, Ay[e]); Az[e] = fma(ujz[e], d, Az[e]);
+            Ax[e] = fma(fma(a[e], f[0], fma(b[e], f[3], wc * f[6])), t, Ax[e]);   // u_j (w_j . V_j), u = (V + I_c[W] r)/rho
+            Ay[e] = fma(fma(a[e], f[1], fma(b[e], f[4], wc * f[7])), t, Ay[e]);
+            Az[e] = fma(fma(a[e], f[2], fma(b[e], f[5], wc * f[8])), t, Az[e]);
+        }
+        if (HYP) {
+            double rj[E], wj[E], sj[6][E];
+            ld_nc<E>(q + F_RHOT * NVP, rj);
+            ld_nc<E>(X + size_t(nb[j]) * XREC + L.k0 + X_W * NVP, wj);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                sj[0][e] = rj[e];
+                sj[1][e] = fma(a[e], f[0], b[e] * f[3]) * irj[e];
+                sj[2][e] = fma(a[e], f[1], b[e] * f[4]) * irj[e];
+                sj[3][e] = fma(a[e], f[2], b[e] * f[5]) * irj[e];
+                sj[4][e] = wj[e];
+                sj[5][e] = pj[e] * irj[e] / g.Rd;
+            }
+            const double lw = j == 0 ? 0.0 : wlp[j - 1];
+#pragma unroll
+            for (int fi = 0; fi < 6; ++fi)
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    if (j == 0) s0[fi][e] = sj[fi][e];
+                    else lp[fi][e] = fma(lw, sj[fi][e] - s0[fi][e], lp[fi][e]);
+                }
         }
     }
-    double ri[E], dlo[E], dhi[E], rho[E], W[E], Wup[E];
+    double ri[E], dlo[E], dhi[E], wl[E], wh[E], idz[E];
     ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
+    ld_nc<E>(g.wl + L.k0, wl);   ld_nc<E>(g.wh + L.k0, wh);   ld_nc<E>(g.idz + L.k0, idz);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         divV[e] *= ri[e]; divhV[e] *= ri[e]; divtV[e] *= ri[e];
         Ax[e] *= ri[e]; Ay[e] *= ri[e]; Az[e] *= ri[e];
-        gpx[e] *= ri[e]; gpy[e] *= ri[e]; gpz[e] *= ri[e];
+        ga[e] *= ri[e]; gb[e] *= ri[e];
     }
+    // the column's own rows again (L1 hits), one at a time
+    double rho[E], W[E], Wup[E], a0[E], b0[E], ir0[E];
     ld_nc<E>(me + F_RHOT * NVP, rho);
-    ld_nc<E>(me + F_WT * NVP, W);
+    ld_again<E>(me + F_WT * NVP, W);
     above<G, E>(W, Wup, L.gl, 0.0);
+    ld_again<E>(me + F_VAT * NVP, a0); ld_again<E>(me + F_VBT * NVP, b0); ld_again<E>(me + F_IRT * NVP, ir0);
+    const double* f0 = frm;
+    const double e1x = f0[0], e1y = f0[1], e1z = f0[2], e2x = f0[3], e2y = f0[4], e2z = f0[5];
+    const double rx = f0[6], ry = f0[7], rz = f0[8];
+    double Mx[E], My[E], Mz[E];                                              // full momentum M = V + I_c[W] r
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const double wc = 0.5 * (W[e] + Wup[e]);
+        Mx[e] = fma(a0[e], e1x, fma(b0[e], e2x, wc * rx));
+        My[e] = fma(a0[e], e1y, fma(b0[e], e2y, wc * ry));
+        Mz[e] = fma(a0[e], e1z, fma(b0[e], e2z, wc * rz));
+    }
 
     // vertical flux divergences D_c[W I_h[q]] for q = u_x, u_y, u_z, h, theta, and D_c[W]
-    double qb[E], X[E], Xup[E];
+    double qb[E], Xf[E], Xup[E];
     auto vflux = [&](const double (&q)[E], double (&out)[E]) {
         below<G, E>(q, qb, L.gl, 0.0);
 #pragma unroll
-        for (int e = 0; e < E; ++e) X[e] = W[e] * 0.5 * (qb[e] + q[e]);    // W = 0 on the ground and on the lid
-        above<G, E>(X, Xup, L.gl, 0.0);
+        for (int e = 0; e < E; ++e) Xf[e] = W[e] * (wl[e] * qb[e] + wh[e] * q[e]);    // W = 0 on the ground and on the lid
+        above<G, E>(Xf, Xup, L.gl, 0.0);
 #pragma unroll
-        for (int e = 0; e < E; ++e) out[e] = dhi[e] * Xup[e] - dlo[e] * X[e];
+        for (int e = 0; e < E; ++e) out[e] = dhi[e] * Xup[e] - dlo[e] * Xf[e];
     };
-    double t[E], q0[E];                 // the column's own rows again (L1 hits), one at a time
-    ld_again<E>(me + F_UX * NVP, q0); vflux(q0, t);
+    double t[E], q0[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) Ax[e] += t[e];
-    ld_again<E>(me + F_UY * NVP, q0); vflux(q0, t);
+    for (int e = 0; e < E; ++e) q0[e] = Mx[e] * ir0[e];
+    vflux(q0, t);
 #pragma unroll
-    for (int e = 0; e < E; ++e) Ay[e] += t[e];
-    ld_again<E>(me + F_UZ * NVP, q0); vflux(q0, t);
+    for (int e = 0; e < E; ++e) { Ax[e] += t[e]; q0[e] = My[e] * ir0[e]; }
+    vflux(q0, t);
 #pragma unroll
-    for (int e = 0; e < E; ++e) Az[e] += t[e];
+    for (int e = 0; e < E; ++e) { Ay[e] += t[e]; q0[e] = Mz[e] * ir0[e]; }
+    vflux(q0, t);
+#pragma unroll
+    for (int e = 0; e < E; ++e) { Az[e] += t[e]; q0[e] = cph * p0[e] * ir0[e]; }
     double DhW[E], DtW[E], DW[E];
-    ld_again<E>(me + F_H * NVP, q0);  vflux(q0, DhW);
+    vflux(q0, DhW);
     ld_again<E>(me + F_TH * NVP, q0); vflux(q0, DtW);
 #pragma unroll
     for (int e = 0; e < E; ++e) DW[e] = dhi[e] * Wup[e] - dlo[e] * W[e];
 
-    const double3 rh = ld_rhat(g.rhat, L.col);
-    const double rx = rh.x, ry = rh.y, rz = rh.z;
-    double sVx[E], sVy[E], sVz[E], Fr[E], srho[E], sp[E], srt[E];
+    double sa[E], sb[E], Fr[E], srho[E], sp[E], srt[E];
     // g~ W on interfaces, then I_c
-    double pb[E], rb[E], Z[E], Zup[E];
+    double pb[E], rb[E], rhoh[E], Z[E], Zup[E];
     below<G, E>(p0, pb, L.gl, 0.0); below<G, E>(rho, rb, L.gl, 1.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
-        const double gt = (k >= 1 && k < nv) ? ((p0[e] - pb[e]) / g.dz) / (0.5 * (rb[e] + rho[e])) : 0.0;
-        Z[e] = gt * W[e];
+        const bool in = k >= 1 && k < nv;
+        rhoh[e] = in ? wl[e] * rb[e] + wh[e] * rho[e] : 1.0;
+        Z[e] = in ? ((p0[e] - pb[e]) * idz[e]) / rhoh[e] * W[e] : 0.0;
     }
     above<G, E>(Z, Zup, L.gl, 0.0);
-    double V0x[E], V0y[E], V0z[E];
-    ld_again<E>(me + F_VXT * NVP, V0x); ld_again<E>(me + F_VYT * NVP, V0y); ld_again<E>(me + F_VZT * NVP, V0z);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const bool real = (L.k0 + e < nv) && (L.col < g.N);
-        const double wc = 0.5 * (W[e] + Wup[e]);
-        const double Mx = V0x[e] + wc * rx, My = V0y[e] + wc * ry;
-        const double Cx = -2.0 * g.omega * My, Cy = 2.0 * g.omega * Mx;       // 2 Omega z x M
+        const double Cx = -2.0 * g.omega * My[e], Cy = 2.0 * g.omega * Mx[e];       // 2 Omega z x M
         const double Ar = Ax[e] * rx + Ay[e] * ry + Az[e] * rz;
         const double Cr = Cx * rx + Cy * ry;
         Fr[e] = Ar + Cr;
-        sVx[e] = real ? -gpx[e] - (Ax[e] - Ar * rx) - (Cx - Cr * rx) : 0.0;
-        sVy[e] = real ? -gpy[e] - (Ay[e] - Ar * ry) - (Cy - Cr * ry) : 0.0;
-        sVz[e] = real ? -gpz[e] - (Az[e] - Ar * rz) - (0.0 - Cr * rz) : 0.0;
+        const double sx = -(Ax[e] - Ar * rx) - (Cx - Cr * rx);                      // Eq. 28 (G5)
+        const double sy = -(Ay[e] - Ar * ry) - (Cy - Cr * ry);
+        const double sz = -(Az[e] - Ar * rz) - (0.0 - Cr * rz);
+        sa[e] = real ? (sx * e1x + sy * e1y + sz * e1z) - ga[e] : 0.0;
+        sb[e] = real ? (sx * e2x + sy * e2y + sz * e2z) - gb[e] : 0.0;
         srho[e] = real ? -divV[e] - DW[e] : 0.0;
-        const double vgp = (V0x[e] * gpx[e] + V0y[e] * gpy[e] + V0z[e] * gpz[e]) / rho[e];
+        const double vgp = (a0[e] * ga[e] + b0[e] * gb[e]) * ir0[e];               // v_h . grad_h p
         sp[e] = real ? -kv * (divhV[e] + DhW[e] - vgp - 0.5 * (Z[e] + Zup[e])) : 0.0;
         srt[e] = real ? -divtV[e] - DtW[e] : 0.0;
     }
@@ -788,21 +864,46 @@ k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
         sW[e] = (k >= 1 && k < nv && L.col < g.N)
-                    ? -(p0[e] - pb[e]) / g.dz - g.gravity * 0.5 * (rb[e] + rho[e]) - 0.5 * (Frb[e] + Fr[e])
+                    ? -(p0[e] - pb[e]) * idz[e] - g.gravity * rhoh[e] - (wl[e] * Frb[e] + wh[e] * Fr[e])
                     : 0.0;                                                    // Eq. 42
     }
-    {
-        const Basis B = ld_basis(g.basis, L.col);
-        double sa[E], sb[E];
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            sa[e] = sVx[e] * B.e1.x + sVy[e] * B.e1.y + sVz[e] * B.e1.z;
-            sb[e] = sVx[e] * B.e2.x + sVy[e] * B.e2.y + sVz[e] * B.e2.z;
-        }
-        st_row<E>(me + F_SVA * NVP, sa); st_row<E>(me + F_SVB * NVP, sb);
-    }
+    st_row<E>(me + F_SVA * NVP, sa);    st_row<E>(me + F_SVB * NVP, sb);
     st_row<E>(me + F_SRHO * NVP, srho); st_row<E>(me + F_SW * NVP, sW); st_row<E>(me + F_SP * NVP, sp);
     st_row<E>(me + F_SRT * NVP, srt);
+    if (dd) {                                                                 // NEXT-1 divergence damping (RD4)
+        double* xe = X + size_t(L.col) * XREC + L.k0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) t[e] = divV[e] + DW[e];
+        st_row<E>(xe + X_D3T * NVP, t);
+        if (dd == 2) st_row<E>(xe + X_D3N * NVP, t);
+    }
+    if (HYP) {                                                                // q = lap(rho) | rho lap(v_j) | rho_h lap(w) | rho lap(T)
+        double* xe = X + size_t(L.col) * XREC + L.k0;
+        double rhi[E];
+        ld_nc<E>(g.rhinv + L.k0, rhi);
+#pragma unroll
+        for (int fi = 0; fi < 6; ++fi) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int k = L.k0 + e;
+                const double sc = fi == 4 ? rhi[e] * rhi[e] : ri[e] * ri[e];
+                const double wgt = fi == 0 ? 1.0 : (fi == 4 ? rhoh[e] : rho[e]);
+                t[e] = wgt * (lp[fi][e] * sc);
+                if (fi == 4 && !(k >= 1 && k < nv)) t[e] = 0.0;
+            }
+            st_row<E>(xe + (X_Q0 + fi) * NVP, t);
+        }
+    }
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
+k_slow_terms(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
+    slow_terms_block<G, E, false>(g, S, tn, X, dd);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
+k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
+    slow_terms_block<G, E, true>(g, S, tn, X, dd);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -811,7 +912,7 @@ k_slow_terms(Geom g, double* __restrict__ S, Tune tn) {
 // ---------------------------------------------------------------------------------------------
 template <int G, int E, bool DD>
 __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict__ S, double delta, const Tune& tn,
-                                               const double* __restrict__ Xdd, double Kd_div) {
+                                               const double* __restrict__ Xdd, double Kd_div, int d3row) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -855,7 +956,7 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
         const int* di = g.dd_idx + size_t(L.col) * 20;
         const double2* dc = reinterpret_cast<const double2*>(g.dd_coef + size_t(L.col) * 40);
         double d0[E], fa[E], fb[E];
-        ld_nc<E>(Xdd + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d0);
+        ld_nc<E>(Xdd + size_t(L.col) * XREC + L.k0 + d3row * NVP, d0);
 #pragma unroll
         for (int e = 0; e < E; ++e) fa[e] = fb[e] = 0.0;
 #pragma unroll 6
@@ -863,7 +964,7 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
             const int m = __ldg(di + q);
             const double2 c = __ldg(dc + q);
             double dm[E];
-            ld_nc<E>(Xdd + size_t(m) * XREC + L.k0 + X_D3 * NVP, dm);
+            ld_nc<E>(Xdd + size_t(m) * XREC + L.k0 + d3row * NVP, dm);
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const double dd = dm[e] - d0[e];
@@ -886,13 +987,14 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
-    momentum_block<G, E, false>(g, S, delta, tn, nullptr, 0.0);
+    momentum_block<G, E, false>(g, S, delta, tn, nullptr, 0.0, 0);
 }
-// the same kernel with NEXT-1's divergence damping added to Eq. 33
+// the same kernel with NEXT-1's divergence damping added to Eq. 33; d3row: the X row that holds the 3-D
+// divergence of the current momentum (X_D3N in the first substep of a stage, where V^[t] + V*(0) = V^n; X_D3 after)
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum_dd(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div) {
-    momentum_block<G, E, true>(g, S, delta, tn, Xdd, Kd_div);
+k_momentum_dd(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div, int d3row) {
+    momentum_block<G, E, true>(g, S, delta, tn, Xdd, Kd_div, d3row);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -945,8 +1047,9 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
             divtV[e] = fma(tj[e], d, divtV[e]);
         }
     }
-    double ri[E], dlo[E], dhi[E];
+    double ri[E], dlo[E], dhi[E], wl[E], wh[E];
     ld_nc<E>(g.rinv + k0, ri); ld_nc<E>(g.dlo + k0, dlo); ld_nc<E>(g.dhi + k0, dhi);
+    ld_nc<E>(g.wl + k0, wl);   ld_nc<E>(g.wh + k0, wh);
 
     double rho_s[E], p_s[E], W_s[E], rts[E], srho[E], sp[E], sW[E], srt[E], pt[E], irt[E];
     ld_rw<E>(own + F_RHOS * NVP, rho_s); ld_rw<E>(own + F_WS * NVP, W_s); ld_rw<E>(own + F_RTS * NVP, rts);
@@ -975,12 +1078,15 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
     // right-hand side d_k on interior interfaces, already scaled by 1/b'_k (fi = 0 on the ground and on pads)
     double fa[E], fi[E], fc[E], A[E], B[E], zf[E], Wn[E];
     ld_rw<E>(own + F_FA * NVP, fa); ld_rw<E>(own + F_FI * NVP, fi); ld_rw<E>(own + F_FC * NVP, fc);
-    const double cdz = delta / g.dz, cg = 0.5 * delta * g.gravity;
+    {
+        double idz[E];
+        ld_nc<E>(g.idz + k0, idz);
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const double d = W_s[e] + delta * sW[e] - cdz * (pq[e] - pqb[e]) - cg * (rqb[e] + rq[e]);
-        A[e] = -fa[e];            // z_k = d_k/b'_k - (a_k/b'_k) z_(k-1)
-        B[e] = fi[e] * d;
+        for (int e = 0; e < E; ++e) {     // G_h and I_h of Eq. 8-9 (k = 1) on the lower interface of layer k
+            const double d = W_s[e] + delta * (sW[e] - idz[e] * (pq[e] - pqb[e]) - g.gravity * (wl[e] * rqb[e] + wh[e] * rq[e]));
+            A[e] = -fa[e];            // z_k = d_k/b'_k - (a_k/b'_k) z_(k-1)
+            B[e] = fi[e] * d;
+        }
     }
     affine_scan<G, E, false>(A, B, zf, gl);
 #pragma unroll
@@ -991,7 +1097,7 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
     above<G, E>(Wn, Wup, gl, 0.0);
     below<G, E>(th0, thb, gl, 0.0);
 #pragma unroll
-    for (int e = 0; e < E; ++e) X[e] = 0.5 * (thb[e] + th0[e]) * Wn[e];  // I_h[theta] W'
+    for (int e = 0; e < E; ++e) X[e] = (wl[e] * thb[e] + wh[e] * th0[e]) * Wn[e];  // I_h[theta] W'
     above<G, E>(X, Xup, gl, 0.0);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -1045,7 +1151,8 @@ k_vertical_dd(Geom g, double* __restrict__ S, double delta, int first, Tune tn, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2, TMA-staged (the production path where the shape has one): persistent blocks of kTmaWarps warps
+// K2, TMA-staged (NOT the default: measured slower than the direct-load kernel, profiles/r01c_substep_kernels.md;
+// selected with THOR_B200_TUNE tma_stages = 1 or 2 and kept as a tested variant): persistent blocks of kTmaWarps warps
 // walk tiles of TCOL = kTmaWarps*32/G consecutive columns -- 2x2 / 2x4 / 4x4 patches of the rhombus
 // lattice in the Morton device order.  EVERYTHING a tile reads is brought into shared memory by
 // cp.async.bulk (TMA) and signalled through an mbarrier: the own rows F_VAS..F_PT of its columns
@@ -1165,8 +1272,7 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
         prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VXT, 3);
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHOT, 2);
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAT, 5);
     }
     constexpr int NVP = Map<G, E>::NVP;
     double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
@@ -1178,16 +1284,15 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
         for (int e = 0; e < E; ++e) out[e] += d[e];
     };
     sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p);
+    const Frame fr = ld_frame(g.frame, L.col);
     {
-        const Basis B = ld_basis(g.basis, L.col);
-        double va[E];
-        ld_rw<E>(me + F_VXT * NVP, vx); ld_rw<E>(me + F_VYT * NVP, vy); ld_rw<E>(me + F_VZT * NVP, vz);
-        ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, d);
+        double va[E], vb[E];
+        sum(F_VAT, F_VAS, va); sum(F_VBT, F_VBS, vb);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            vx[e] += va[e] * B.e1.x + d[e] * B.e2.x;
-            vy[e] += va[e] * B.e1.y + d[e] * B.e2.y;
-            vz[e] += va[e] * B.e1.z + d[e] * B.e2.z;
+            vx[e] = va[e] * fr.e1.x + vb[e] * fr.e2.x;
+            vy[e] = va[e] * fr.e1.y + vb[e] * fr.e2.y;
+            vz[e] = va[e] * fr.e1.z + vb[e] * fr.e2.z;
         }
     }
     sum(F_WT, F_WS, a);
@@ -1196,7 +1301,7 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
         // Eq. 59-61 (G15, RJ1): T_eq = T_vert(z) + beta_trop(sigma, z) dT_EP cos(lon) cos(lat); cos(lon) cos(lat) = x of the unit vector
         const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
         const double ps = p0 * exp(g.gravity * __ldg(g.zc) / (g.Rd * (p0 / (rho0 * g.Rd))));
-        const double mu = ld_rhat(g.rhat, L.col).x, KT = 1.0 / J.tau_rad;
+        const double mu = fr.r.x, KT = 1.0 / J.tau_rad;
         double z[E];
         ld_nc<E>(g.zc + L.k0, z);
 #pragma unroll
@@ -1221,7 +1326,7 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
         const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
         const double T0 = p0 / (rho0 * g.Rd);
         const double ps = p0 * exp(g.gravity * __ldg(g.zc) / (g.Rd * T0));
-        const double sphi = ld_rhat(g.rhat, L.col).z, cphi2 = 1.0 - sphi * sphi, kappa = g.Rd / g.Cp;
+        const double sphi = fr.r.z, cphi2 = 1.0 - sphi * sphi, kappa = g.Rd / g.Cp;
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double sigma = p[e] / ps;
@@ -1263,7 +1368,9 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
 // hyper-diffusion of rho, v_h (Cartesian components), v_r and T per Runge-Kutta stage, and the 3-D
 // divergence damping per acoustic substep.  Every nabla_h^2 is the 7-point stencil of L369-L371
 // (Geom::wlap).  Work rows live in a second slab X[column][XF][layer], allocated only when a
-// diffusion coefficient is set; the base path and its slab are untouched.
+// diffusion coefficient is set.  The first Laplacians are formed inside the slow-term kernel's gather
+// loop (k_slow_terms_hyp), w by the stage-preparation kernel, D3^[t] by the slow-term kernel, D3 per
+// substep by the column-solve kernel: the only extra launch per stage is k_diff2 below.
 // ---------------------------------------------------------------------------------------------
 
 template <int G, int E>
@@ -1290,76 +1397,13 @@ __device__ __forceinline__ void ld_lap_weights(const Geom& g, int col, int (&nb)
     w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x; w[5] = c.y;
 }
 
-// column-local: the diffused quantities of the stage reference state
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_diff0(Geom g, const double* __restrict__ S, double* __restrict__ X) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    const double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
-    double* xe = X + size_t(L.col) * (size_t(XF) * NVP) + L.k0;
-    double rho[E], rb[E], v[E], W[E], p[E];
-    ld_nc<E>(me + F_RHOT * NVP, rho); ld_nc<E>(me + F_WT * NVP, W); ld_nc<E>(me + F_PT * NVP, p);
-    below<G, E>(rho, rb, L.gl, 1.0);
-    const int fv[3] = {F_VXT, F_VYT, F_VZT};
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-        ld_nc<E>(me + fv[j] * NVP, v);
-#pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = v[e] / rho[e];
-        st_row<E>(xe + (X_VX + j) * NVP, v);
-    }
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int k = L.k0 + e;
-        v[e] = (k >= 1 && k < g.nv) ? W[e] / (0.5 * (rb[e] + rho[e])) : 0.0;       // w on interior interfaces
-    }
-    st_row<E>(xe + X_W * NVP, v);
-#pragma unroll
-    for (int e = 0; e < E; ++e) v[e] = p[e] / (g.Rd * rho[e]);
-    st_row<E>(xe + X_T * NVP, v);
-}
-
-// first Laplacian, weighted for the second: q = lap(rho) | rho lap(v_j) | rho_h lap(w) | rho lap(T)
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_diff1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
-    int nb[6]; double w[6];
-    ld_lap_weights(g, L.col, nb, w);
-    double* xe = X + size_t(L.col) * XREC + L.k0;
-    double rho[E], rb[E], ri[E], rhi[E], q[E];
-    ld_nc<E>(S + size_t(L.col) * REC + L.k0 + F_RHOT * NVP, rho);
-    below<G, E>(rho, rb, L.gl, 1.0);
-    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.rhinv + L.k0, rhi);
-    lap_gather<G, E>(S + F_RHOT * NVP, REC, nb, w, L.col, L.k0, q);
-#pragma unroll
-    for (int e = 0; e < E; ++e) q[e] = q[e] * ri[e] * ri[e];
-    st_row<E>(xe + X_Q0 * NVP, q);
-    const int src[4] = {X_VX, X_VY, X_VZ, X_T}, dst[4] = {X_Q1, X_Q2, X_Q3, X_Q5};
-#pragma unroll
-    for (int f = 0; f < 4; ++f) {
-        lap_gather<G, E>(X + src[f] * NVP, XREC, nb, w, L.col, L.k0, q);
-#pragma unroll
-        for (int e = 0; e < E; ++e) q[e] = rho[e] * (q[e] * ri[e] * ri[e]);
-        st_row<E>(xe + dst[f] * NVP, q);
-    }
-    lap_gather<G, E>(X + X_W * NVP, XREC, nb, w, L.col, L.k0, q);
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const int k = L.k0 + e;
-        q[e] = (k >= 1 && k < g.nv) ? (0.5 * (rb[e] + rho[e])) * (q[e] * rhi[e] * rhi[e]) : 0.0;
-    }
-    st_row<E>(xe + X_Q4 * NVP, q);
-}
-
 // second Laplacian; the fluxes are added to the slow terms of the stage (RD2, RD3)
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd) {
-    Map<G, E> L;
+k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd, Tune tn) {
+    const Walk wk(tn);
+    Map<G, E> L(wk.bid);
+    if (wk.ahead_bid >= 0) { prefetch_block_rows<G, E>(S, wk.ahead_bid, F_SRHO, 4); prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 3); }
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
     int nb[6]; double w[6];
@@ -1380,18 +1424,17 @@ k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd)
     lap_gather<G, E>(X + X_Q1 * NVP, XREC, nb, w, L.col, L.k0, Fx);
     lap_gather<G, E>(X + X_Q2 * NVP, XREC, nb, w, L.col, L.k0, Fy);
     lap_gather<G, E>(X + X_Q3 * NVP, XREC, nb, w, L.col, L.k0, Fz);
-    const double3 rh = ld_rhat(g.rhat, L.col);
-    const Basis B = ld_basis(g.basis, L.col);
+    const Frame fr = ld_frame(g.frame, L.col);
     double sa[E], sb[E];
     ld_rw<E>(me + F_SVA * NVP, sa); ld_rw<E>(me + F_SVB * NVP, sb);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const double s2 = ri[e] * ri[e];
         double fx = -Kd * (Fx[e] * s2), fy = -Kd * (Fy[e] * s2), fz = -Kd * (Fz[e] * s2);
-        const double fr = fx * rh.x + fy * rh.y + fz * rh.z;
-        fx -= fr * rh.x; fy -= fr * rh.y; fz -= fr * rh.z;
-        sa[e] = real(e) ? sa[e] + (fx * B.e1.x + fy * B.e1.y + fz * B.e1.z) : 0.0;
-        sb[e] = real(e) ? sb[e] + (fx * B.e2.x + fy * B.e2.y + fz * B.e2.z) : 0.0;
+        const double frr = fx * fr.r.x + fy * fr.r.y + fz * fr.r.z;
+        fx -= frr * fr.r.x; fy -= frr * fr.r.y; fz -= frr * fr.r.z;
+        sa[e] = real(e) ? sa[e] + (fx * fr.e1.x + fy * fr.e1.y + fz * fr.e1.z) : 0.0;
+        sb[e] = real(e) ? sb[e] + (fx * fr.e2.x + fy * fr.e2.y + fz * fr.e2.z) : 0.0;
     }
     st_row<E>(me + F_SVA * NVP, sa); st_row<E>(me + F_SVB * NVP, sb);
     // vertical momentum on interior interfaces
@@ -1415,50 +1458,6 @@ k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd)
         u[e] = real(e) ? u[e] + Fp * eos_rt(p[e], g.Rd, g.p_ref, 1.0 / gam) / (gam * p[e]) : 0.0;
     }
     st_row<E>(me + F_SP * NVP, t); st_row<E>(me + F_SRT * NVP, u);
-}
-
-// divergence damping, once per stage: D3^[t] = div_h(V^[t]) + D_c[W^[t]] (constant over the stage) and the
-// first substep's D3 = D3^[t] + div_h(V*(0)) + D_c[W*(0)]  (RD4); later substeps get D3 from the column-solve kernel
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_dd1(Geom g, const double* __restrict__ S, double* __restrict__ X) {
-    Map<G, E> L;
-    constexpr int NVP = Map<G, E>::NVP;
-    constexpr size_t REC = Map<G, E>::REC, XREC = size_t(XF) * NVP;
-    const double* me = S + size_t(L.col) * REC + L.k0;
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    const double* wc = g.wdiv + size_t(L.col) * 24;
-    const double* wt = g.wdiv2 + size_t(L.col) * 16;
-    double d[E], ds[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = ds[e] = 0.0;
-#pragma unroll
-    for (int j = 0; j < 7; ++j) {
-        const double* q = S + size_t(nb[j]) * REC + L.k0;
-        double x[E], y[E], z[E], a[E], b[E];
-        ld_nc<E>(q + F_VXT * NVP, x); ld_nc<E>(q + F_VYT * NVP, y); ld_nc<E>(q + F_VZT * NVP, z);
-        ld_nc<E>(q + F_VAS * NVP, a); ld_nc<E>(q + F_VBS * NVP, b);
-        const double wx = __ldg(wc + 3 * j), wy = __ldg(wc + 3 * j + 1), wz = __ldg(wc + 3 * j + 2);
-        const double wa = __ldg(wt + 2 * j), wb = __ldg(wt + 2 * j + 1);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            d[e] += fma(wx, x[e], fma(wy, y[e], wz * z[e]));
-            ds[e] += fma(wa, a[e], wb * b[e]);
-        }
-    }
-    double ri[E], dlo[E], dhi[E], W[E], Ws[E], Wup[E];
-    ld_nc<E>(g.rinv + L.k0, ri); ld_nc<E>(g.dlo + L.k0, dlo); ld_nc<E>(g.dhi + L.k0, dhi);
-    ld_nc<E>(me + F_WT * NVP, W); ld_nc<E>(me + F_WS * NVP, Ws);
-    above<G, E>(W, Wup, L.gl, 0.0);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] = d[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * W[e]);
-    st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3T * NVP, d);
-    above<G, E>(Ws, Wup, L.gl, 0.0);
-#pragma unroll
-    for (int e = 0; e < E; ++e) d[e] += ds[e] * ri[e] + (dhi[e] * Wup[e] - dlo[e] * Ws[e]);
-    st_row<E>(X + size_t(L.col) * XREC + L.k0 + X_D3 * NVP, d);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -275,24 +275,106 @@ def test_vertical_slow_term_is_second_order_hydrostatic_residual(ogrid):
 
 
 # ------------------------------------------------------------------------------------------ P14
-def test_p14_rk3_split_explicit_is_second_order_in_dt(ogrid):
-    cfg = ti.CONFIGS[0]
+def test_p14_rk3_stage_weights_give_third_order_on_rotation_dominated_flow(ogrid):
+    """Pin of reading R1 (stage reference state, the 1/3, 1/2, 1 weights and the restart from t_n of
+    Eq. 30-31).  Three step sizes against a much finer reference, observed order asserted
+    for V and for p separately.
+
+    The HE-VI coupling of the fast modes (forward-backward in the horizontal, backward Euler in the
+    vertical, Eq. 33-37) is first order in the substep delta BY CONSTRUCTION; a flow dominated by
+    acoustic/gravity-wave adjustment therefore shows order ~1 at fixed n whatever the stage weights
+    are (measured: 1.04-1.10 on a warm anomaly at rest), which is why this pin uses a flow whose
+    evolution is carried by the SLOW terms: solid-body rotation about a tilted axis on a fast
+    rotator (Omega = 3e-4 1/s, inertial period ~3 h, Coriolis and advection in slowV), many substeps
+    (n = 32) so that the first-order fast-mode error is far below the Runge-Kutta error.  Eq. 30 is
+    then a three-stage Runge-Kutta scheme on a nearly linear slow operator: third order.  A wrong
+    second-stage weight or restart gives order 1, a wrong first-stage weight order 2 (both outside
+    the asserted windows); L243 claims second order at least."""
     xyz, nbr, C = ogrid(2, True)
-    nv = 6
-    planet = cfg["planet"]
+    nv, n, Ttot = 6, 32, 7200.0
+    planet = dict(ti.EARTH, omega=3.0e-4)
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1e5, 300.0)
+    vel = 10.0 * np.cross(np.array([0.3, 0.2, 1.0]), xyz)[:, None, :] * np.ones((1, nv, 1))
+    V = rho[..., None] * vel
+    ref = G.step(rho, V, W, p, 64, Ttot / 64, n)
+    eV, ep = [], []
+    for k in (2, 4, 8):
+        out = G.step(rho, V, W, p, k, Ttot / k, n)
+        eV.append(np.abs(out[1] - ref[1]).max())
+        ep.append(np.abs(out[3] - ref[3]).max())
+    assert eV[0] > 0.1 * np.abs(ref[1] - V).max()                # the coarse run is far from converged: a real test
+    oV = [math.log2(eV[i] / eV[i + 1]) for i in range(2)]
+    op = [math.log2(ep[i] / ep[i + 1]) for i in range(2)]
+    assert all(2.6 < o < 3.3 for o in oV), (oV, eV)
+    assert all(2.0 < o < 3.0 for o in op), (op, ep)
+
+
+def test_p14b_fast_mode_coupling_is_first_order_in_the_substep(ogrid):
+    """The complement of P14, stated so that nobody reads L243's "second-order accuracy" into the whole
+    scheme: on an adjustment problem (warm anomaly at rest, Earth rotation, n = 4) the error falls
+    ~2x per halving of dt -- the backward-Euler vertical solve and the forward-backward horizontal
+    coupling of Eq. 33-37 are first order in delta = dt/n."""
+    xyz, nbr, C = ogrid(2, True)
+    nv, n, Ttot = 6, 4, 3600.0
+    planet = ti.EARTH
     G = oracle.Geometry(xyz, nbr, nv, planet, C)
     rho, V, W, p = ti.rest_state(planet, nv, G.N, 1e5, 300.0)
     x, y, z = xyz[:, 0:1], xyz[:, 1:2], xyz[:, 2:3]
-    T = 300.0 * (1 + 0.01 * x * z + 0.005 * y)               # smooth warm anomaly drives a flow
-    rho = p / (287.0 * T)
-    Ttot, n = 3600.0, 4
-    ref = G.step(rho, V, W, p, 16, Ttot / 16, n)
-    e = []
-    for k in (2, 4):
-        out = G.step(rho, V, W, p, k, Ttot / k, n)
-        e.append(max(np.abs(out[1] - ref[1]).max() / np.abs(ref[1]).max(),
-                     np.abs(out[3] - ref[3]).max() / np.abs(ref[3] - p).max()))
-    assert e[1] < 0.45 * e[0], e                               # ~4x per halving (second order, L243)
+    rho = p / (287.0 * 300.0 * (1 + 0.01 * x * z + 0.005 * y))
+    ref = G.step(rho, V, W, p, 64, Ttot / 64, n)
+    e = [np.abs(G.step(rho, V, W, p, k, Ttot / k, n)[1] - ref[1]).max() for k in (2, 4, 8)]
+    o = [math.log2(e[i] / e[i + 1]) for i in range(2)]
+    assert all(0.8 < x < 1.4 for x in o), (o, e)
+
+
+# ------------------------------------------------------------------------------------------ R10
+def test_total_energy_closed_forms(ogrid):
+    """Pin of the energy half of orc_diagnostics (R10: E = sum (Cv p/Rd + (|V|^2 + I_c[W]^2)/(2 rho)
+    + rho g z_c) A_c r_c^2 dz; L215, L339 only name "total energy").  Four states whose energy is a
+    one-line closed form, each isolating one term, so that Cp for Cv, a missing 1/2, z_h for z_c,
+    r_h for r_c or a wrong I_c fails one of them.  The expected values are written out here with
+    math.fsum from the layer tables; sum(A_c) = 4 pi is pin P2."""
+    xyz, nbr, C = ogrid(2, True)
+    nv = 5
+    planet = dict(ti.EARTH, z_top=20.0e3)
+    Rd, Cp, g, A = planet["Rd"], planet["Cp"], planet["gravity"], planet["radius"]
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    N = G.N
+    dz = planet["z_top"] / nv
+    zc = [(k + 0.5) * dz for k in range(nv)]
+    rc = [A + zk for zk in zc]
+    area = math.fsum(G.Ac)
+    assert abs(area - 4 * math.pi) < 1e-12
+    pk = ti.hydrostatic_isothermal(planet, nv, 1.0e5, 250.0)           # the P12 recurrence
+    rk = [float(x) / (Rd * 250.0) for x in pk]
+    rho, p = np.tile(np.array(rk), (N, 1)), np.tile(pk, (N, 1))
+    V0, W0 = np.zeros((N, nv, 3)), np.zeros((N, nv + 1))
+    # (a) internal + potential energy of the discretely hydrostatic isothermal rest column
+    E_int = area * math.fsum((Cp - Rd) * float(pk[k]) / Rd * rc[k] ** 2 * dz for k in range(nv))
+    E_pot = area * math.fsum(rk[k] * g * zc[k] * rc[k] ** 2 * dz for k in range(nv))
+    _, E = G.diagnostics(rho, V0, W0, p)
+    assert abs(E - (E_int + E_pot)) <= 1e-13 * (E_int + E_pot)
+    # (b) no gravity: the internal term alone (Cv, not Cp: they differ by 40 %)
+    G0 = oracle.Geometry(xyz, nbr, nv, dict(planet, gravity=0.0), C)
+    _, E = G0.diagnostics(rho, V0, W0, p)
+    assert abs(E - E_int) <= 1e-13 * E_int
+    assert abs(E_pot) > 0.05 * E_int                                    # (a) did test the potential term
+    # (c) horizontal kinetic energy of solid-body rotation in ONE layer: 1/2 rho |w x r|^2, |w x r|^2 = w^2 r^2 (1 - z^2)
+    k0, wrot = 3, 2.0e-6
+    V = V0.copy()
+    V[:, k0, :] = rk[k0] * wrot * rc[k0] * np.cross(np.array([0.0, 0.0, 1.0]), xyz)
+    S = math.fsum(float(a) * (1.0 - float(zz) ** 2) for a, zz in zip(G.Ac, xyz[:, 2]))
+    E_kh = 0.5 * rk[k0] * (wrot * rc[k0]) ** 2 * S * rc[k0] ** 2 * dz
+    _, E = G0.diagnostics(rho, V, W0, p)
+    assert abs((E - E_int) - E_kh) <= 1e-9 * E_kh                      # E_kh ~ 1e-6 E_int: 1e-9 of it is the rounding of the sum
+    # (d) vertical kinetic energy of W on ONE interface k1: I_c[W] = W/2 in the layers below and above it
+    k1, Wv = 2, 0.7
+    W = W0.copy()
+    W[:, k1] = Wv
+    E_kv = area * 0.5 * (0.5 * Wv) ** 2 * (rc[k1 - 1] ** 2 / rk[k1 - 1] + rc[k1] ** 2 / rk[k1]) * dz
+    _, E = G0.diagnostics(rho, V0, W, p)
+    assert abs((E - E_int) - E_kv) <= 1e-8 * E_kv
 
 
 # ------------------------------------------------------------------------------------- forcing R9
