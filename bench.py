@@ -233,6 +233,8 @@ def run_cuda(args):
     substeps = ti.substeps_per_large_step(n)
     cells_per_step = N * nv * substeps
 
+    if args.next1:
+        state.set_diffusion(0.01992)
     with torch.cuda.stream(stream):
         for _ in range(max(args.warmup, 3)):
             state.step(1, dt, n, forcing)
@@ -250,6 +252,17 @@ def run_cuda(args):
         barrier()
         launches = thor.thor_launch_count() - l0
         ms = ev0.elapsed_time(ev1)
+        if args.step_only:                       # the profiling entry: nothing but large steps after set-up
+            sampler.stop_flag.set()
+            sampler.join()
+            if rank == 0:
+                print(json.dumps({"metric": METRIC, "value": aggregate_value(cells_per_step, args.steps, 1, ms), "unit": UNIT,
+                                  "ms_per_step": ms / args.steps, "steps": args.steps, "gpu_launches": int(launches),
+                                  "config": dict(workload_config(WORKLOAD, N, world), next1=bool(args.next1)),
+                                  "note": "--step-only: the timed large steps alone (profiling entry), not a bench line"}), flush=True)
+            if world > 1:
+                dist.destroy_process_group()
+            return
 
         # dominant kernel alone (K2 = divergences + column solve) and K1, CUDA events on the same stream.  Chunks of
         # n launches (a stage's worth) between untimed large steps, so that the timed state stays a physical one
@@ -399,6 +412,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--step-only", action="store_true",
+                    help="profiling entry: set up, warm up, run --steps large steps, print a short line and stop "
+                         "(no kernel-alone loops, operators, NEXT-1 or e2e legs); the ncu commands under profiles/ use it")
+    ap.add_argument("--next1", action="store_true", help="with --step-only: NEXT-1 on (D = 0.01992) in the timed steps")
     ap.add_argument("--workload", type=int, default=3, choices=[3, 4],
                     help="BASELINE.json config: 3 = level 6 x 32 (default, the configuration the target is stated on), "
                          "4 = level 7 x 64 (throughput at scale)")

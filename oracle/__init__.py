@@ -79,6 +79,9 @@ def _declare(L):
     L.orc_geom_build.restype = ctypes.c_void_p
     L.orc_geom_build.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Planet), _D, _I, _D]
     L.orc_geom_free.argtypes = [ctypes.c_void_p]
+    L.orc_vertical_ops.argtypes = [ctypes.c_void_p, ctypes.c_int, _D, _D, _D, _D, _D, _D]
+    L.orc_geom_set_vertical.restype = ctypes.c_int
+    L.orc_geom_set_vertical.argtypes = [ctypes.c_void_p, _D, ctypes.c_int]
     for name in ("Ac", "len", "nrm", "C", "bary"):
         f = getattr(L, "orc_geom_" + name)
         f.restype = _D
@@ -137,9 +140,11 @@ def set_num_threads(n):
 class Geometry:
     """All geometric coefficients recomputed from the grid description (O2): positions xyz [N][3],
     neighbour lists nbr [N][6] and control-volume vertices C [N][6][3] (None: triangle centroids
-    of xyz).  fma=True: the FMA-contracted build of the same source (a rounding yardstick, never the reference)."""
+    of xyz).  fma=True: the FMA-contracted build of the same source (a rounding yardstick, never the reference).
+    NEXT-3: z_interfaces = nv+1 increasing interface altitudes from 0 to z_top (None: uniform layers, R6);
+    vert_order = the k of Eq. 8-9 (odd; 1 = linear, the paper's choice)."""
 
-    def __init__(self, xyz, nbr, nv, planet, C=None, fma=False):
+    def __init__(self, xyz, nbr, nv, planet, C=None, fma=False, z_interfaces=None, vert_order=1):
         L = self._L = _load(fma)
         self.xyz = _c(xyz)
         self.nbr = np.ascontiguousarray(nbr, dtype=np.int32)
@@ -160,8 +165,18 @@ class Geometry:
         self.deg = np.ctypeslib.as_array(L.orc_geom_deg(self._h), (N,)).copy()
         self.dz = planet["z_top"] / nv
         self.z_c = (np.arange(nv) + 0.5) * self.dz
+        self.z_h = np.arange(nv + 1) * self.dz
+        self.vert_order = int(vert_order)
+        if z_interfaces is not None or vert_order != 1:
+            zi = None if z_interfaces is None else _c(z_interfaces)
+            assert zi is None or zi.shape == (nv + 1,)
+            if L.orc_geom_set_vertical(self._h, _p(zi), int(vert_order)) != 0:
+                raise ValueError("oracle: bad z_interfaces / vert_order")
+            if zi is not None:
+                self.z_h = zi.copy()
+                self.z_c = 0.5 * (zi[:-1] + zi[1:])
         self.r_c = planet["radius"] + self.z_c
-        self.r_h = planet["radius"] + np.arange(nv + 1) * self.dz
+        self.r_h = planet["radius"] + self.z_h
 
     def __del__(self):
         try:
@@ -257,6 +272,15 @@ class Geometry:
         h = _c(np.array([float(hj[k]) for k in HJ_KEYS]))
         self._L.orc_forcing_hot_jupiter(self._h, float(dt), _p(rho), _p(p), _p(h))
         return p
+
+    def vertical_ops(self, Yc, Xh, order_k=True):
+        """NEXT-3 pins: (I_h[Yc], G_h[Yc], I_c[Xh], D_c[Xh]) of one column; order_k: Eq. 8-9 at the order of the
+        run, else the linear interpolations of the acoustic system."""
+        Yc, Xh = _c(Yc), _c(Xh)
+        assert Yc.shape == (self.nv,) and Xh.shape == (self.nv + 1,)
+        Ih, Gh, Ic, Dc = np.empty(self.nv + 1), np.empty(self.nv + 1), np.empty(self.nv), np.empty(self.nv)
+        self._L.orc_vertical_ops(self._h, int(bool(order_k)), _p(Yc), _p(Xh), _p(Ih), _p(Gh), _p(Ic), _p(Dc))
+        return Ih, Gh, Ic, Dc
 
     def diagnostics(self, rho, V, W, p):
         rho, V, W, p = (_c(x) for x in (rho, V, W, p))

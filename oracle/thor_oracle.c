@@ -41,6 +41,10 @@ typedef struct {
     double *r_c;  /* [nv]   centre radii     r_k   = A + (k+1/2) dz   (R6: uniform dz, L339, L432) */
     double *r_h;  /* [nv+1] interface radii  r_h,k = A + k dz */
     double *z_c;  /* [nv]   centre altitudes */
+    /* NEXT-3 (orc_geom_set_vertical; readings RV1-RV3 of DESIGN.md): layers of unequal thickness and Eq. 8-9 of
+     * order kord > 1.  uniform != 0 (the default) is the path above, arithmetic untouched. */
+    int uniform, kord;
+    double *z_h;  /* [nv+1] interface altitudes, z_h[0] = 0, z_h[nv] = z_top; the centre is the midpoint of its layer */
     double *xyz;  /* [N][3] unit-sphere positions P_i */
     int *nbr;     /* [N][6] neighbours, counter-clockwise seen from outside; -1 pads pentagons */
     int *deg;     /* [N] 5 or 6 */
@@ -97,7 +101,7 @@ static void centroid_eq13(const double *r, int n, double *out) {
 
 void orc_geom_free(orc_geom *G) {
     if (!G) return;
-    free(G->r_c); free(G->r_h); free(G->z_c); free(G->xyz); free(G->nbr); free(G->deg);
+    free(G->r_c); free(G->r_h); free(G->z_c); free(G->z_h); free(G->xyz); free(G->nbr); free(G->deg);
     free(G->C); free(G->len); free(G->nrm); free(G->bary); free(G->Ac);
     free(G->tv); free(G->tE); free(G->tbw);
     free(G);
@@ -117,6 +121,9 @@ orc_geom *orc_geom_build(int N, int nv, const orc_planet *P, const double *xyz, 
     G->r_h = (double *)malloc(sizeof(double) * (nv + 1));
     for (int k = 0; k < nv; k++) { G->z_c[k] = (k + 0.5) * G->dz; G->r_c[k] = P->radius + G->z_c[k]; }
     for (int k = 0; k <= nv; k++) G->r_h[k] = P->radius + k * G->dz;
+    G->uniform = 1; G->kord = 1;
+    G->z_h = (double *)malloc(sizeof(double) * (nv + 1));
+    for (int k = 0; k <= nv; k++) G->z_h[k] = k * G->dz;
     G->xyz = (double *)malloc(sizeof(double) * 3 * N);
     memcpy(G->xyz, xyz, sizeof(double) * 3 * N);
     G->nbr = (int *)malloc(sizeof(int) * 6 * N);
@@ -356,12 +363,77 @@ double orc_tau_d(double dbar, double kd) { return dbar * dbar * dbar * dbar / (3
  * Vertical operators (O3; Eq. 8-9 with k = 1, L88-L94; Eq. 27's radial part, L227).
  * Centre arrays are [nv]; interface arrays are [nv+1] with index 0 = bottom, nv = top.
  * ------------------------------------------------------------------------------------------- */
-static double I_h(const double *Y, int k) { return 0.5 * (Y[k - 1] + Y[k]); }            /* k=1..nv-1 */
+static double I_h_uniform(const double *Y, int k) { return 0.5 * (Y[k - 1] + Y[k]); }    /* k=1..nv-1 */
 static double I_c(const double *X, int k) { return 0.5 * (X[k] + X[k + 1]); }            /* k=0..nv-1 */
-static double G_h(const double *Y, int k, double dz) { return (Y[k] - Y[k - 1]) / dz; }  /* k=1..nv-1 */
+
+/* Eq. 8-9 (L90-L94) written out: sum_j Phi_j L_j(zt), L_j(zt) = prod_(i != j) (zt - z_i)/(z_j - z_i), over the
+ * n nodes z[0..n-1] with values Y[0..n-1]. */
+static double lagrange(const double *z, const double *Y, int n, double zt) {
+    double s = 0.0;
+    for (int j = 0; j < n; j++) {
+        double L = 1.0;
+        for (int i = 0; i < n; i++)
+            if (i != j) L = L * (zt - z[i]) / (z[j] - z[i]);
+        s = s + Y[j] * L;
+    }
+    return s;
+}
+/* RV1: the nodes of Eq. 8-9 at a target between nodes m-1 and m of an array of n_nodes: the (kord+1)/2 nearest
+ * nodes on each side; where the column ends first, the missing ones are dropped (the order falls by one per
+ * missing node: kord = 3 is quadratic at the first and last interior interface).  kord = 1: the two neighbours. */
+static void window(int kord, int m, int n_nodes, int *first, int *count) {
+    int half = (kord + 1) / 2;
+    int lo = m - half, hi = m + half - 1;
+    if (lo < 0) lo = 0;
+    if (hi > n_nodes - 1) hi = n_nodes - 1;
+    *first = lo; *count = hi - lo + 1;
+}
+/* centre -> interface k (k = 1..nv-1), linear (Eq. 8-9 with k = 1): what the acoustic system uses (RV2) */
+static double I_h(const orc_geom *G, const double *Y, int k) {
+    if (G->uniform) return I_h_uniform(Y, k);
+    return lagrange(G->z_c + k - 1, Y + k - 1, 2, G->z_h[k]);
+}
+/* centre -> interface k at the order of the run (RV2: the explicit slow terms) */
+static double I_hk(const orc_geom *G, const double *Y, int k) {
+    if (G->kord <= 1) return I_h(G, Y, k);
+    int f, n;
+    window(G->kord, k, G->nv, &f, &n);
+    return lagrange(G->z_c + f, Y + f, n, G->z_h[k]);
+}
+/* interface -> centre k (k = 0..nv-1) at the order of the run: nodes are the interfaces 0..nv (RV2: the
+ * vertical momentum at the layer centre, L88); order 1 = the mean of the layer's two interfaces */
+static double I_ck(const orc_geom *G, const double *X, int k) {
+    if (G->kord <= 1) return I_c(X, k);
+    int f, n;
+    window(G->kord, k + 1, G->nv + 1, &f, &n);
+    return lagrange(G->z_h + f, X + f, n, G->z_c[k]);
+}
+static double G_h(const orc_geom *G, const double *Y, int k) {                            /* k=1..nv-1 */
+    if (G->uniform) return (Y[k] - Y[k - 1]) / G->dz;
+    return (Y[k] - Y[k - 1]) / (G->z_c[k] - G->z_c[k - 1]);
+}
 static double D_c(const orc_geom *G, const double *X, int k) {                            /* k=0..nv-1 */
     const double *rh = G->r_h;
-    return (rh[k + 1] * rh[k + 1] * X[k + 1] - rh[k] * rh[k] * X[k]) / (G->r_c[k] * G->r_c[k] * G->dz);
+    const double dzk = G->uniform ? G->dz : G->z_h[k + 1] - G->z_h[k];
+    return (rh[k + 1] * rh[k + 1] * X[k + 1] - rh[k] * rh[k] * X[k]) / (G->r_c[k] * G->r_c[k] * dzk);
+}
+
+/* NEXT-3: layers of unequal thickness (z_h: nv+1 increasing interface altitudes from 0 to z_top, NULL = keep)
+ * and the order of Eq. 8-9 (odd, >= 1).  Returns 0, or -1 for a bad argument (nothing changed). */
+int orc_geom_set_vertical(orc_geom *G, const double *z_h, int kord) {
+    const int nv = G->nv;
+    if (kord < 1 || kord % 2 == 0) return -1;
+    if (z_h) {
+        if (z_h[0] != 0.0) return -1;
+        for (int k = 0; k < nv; k++) if (!(z_h[k + 1] > z_h[k])) return -1;
+        G->uniform = 0;
+        for (int k = 0; k <= nv; k++) { G->z_h[k] = z_h[k]; G->r_h[k] = G->P.radius + z_h[k]; }
+        for (int k = 0; k < nv; k++) { G->z_c[k] = 0.5 * (z_h[k] + z_h[k + 1]); G->r_c[k] = G->P.radius + G->z_c[k]; }
+        G->P.z_top = z_h[nv];
+        G->dz = z_h[nv] / nv;
+    }
+    G->kord = kord;
+    return 0;
 }
 
 /* Eq. 24 (L210) and its inverse */
@@ -452,7 +524,7 @@ static void stage_coefficients(const orc_geom *G, orc_work *w) {
             th[k] = eos_rt(P, p[k]) / rho[k];
         }
         gt[0] = 0.0; gt[nv] = 0.0;
-        for (int k = 1; k < nv; k++) gt[k] = G_h(p, k, G->dz) / I_h(rho, k);
+        for (int k = 1; k < nv; k++) gt[k] = G_h(G, p, k) / I_h(G, rho, k);
     }
 }
 
@@ -470,7 +542,7 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
         const double *W = w->W_t + (size_t)i * (nv + 1);
         for (int k = 0; k < nv; k++) {
             size_t c = (size_t)i * nv + k;
-            double wc = I_c(W, k);
+            double wc = I_ck(G, W, k);
             w->Wc[c] = wc;
             for (int d = 0; d < 3; d++) w->u[3 * c + d] = (w->V_t[3 * c + d] + wc * rh[d]) / w->rho_t[c];
         }
@@ -491,7 +563,7 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
                 const double *W = w->W_t + (size_t)i * (nv + 1);
                 for (int k = 0; k < nv; k++) uj[k] = w->u[3 * ((size_t)i * nv + k) + j];
                 X[0] = 0.0; X[nv] = 0.0;
-                for (int k = 1; k < nv; k++) X[k] = W[k] * I_h(uj, k);
+                for (int k = 1; k < nv; k++) X[k] = W[k] * I_hk(G, uj, k);
                 for (int k = 0; k < nv; k++) {
                     size_t c = (size_t)i * nv + k;
                     w->Avec[3 * c + j] = w->sc1[c] + D_c(G, X, k);
@@ -546,10 +618,10 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
             for (int k = 0; k < nv; k++) w->slowrho[(size_t)i * nv + k] = -w->sc1[(size_t)i * nv + k] - D_c(G, W, k);
             /* Eq. 42 at interior interfaces */
             Svr[0] = 0.0; Svr[nv] = 0.0;
-            for (int k = 1; k < nv; k++) Svr[k] = -G_h(p, k, G->dz) - P->gravity * I_h(rho, k) - I_h(Fr, k);
+            for (int k = 1; k < nv; k++) Svr[k] = -G_h(G, p, k) - P->gravity * I_hk(G, rho, k) - I_hk(G, Fr, k);
             /* slow part of the pressure equation (Eq. 40 with the signs of G10) */
             X[0] = 0.0; X[nv] = 0.0;
-            for (int k = 1; k < nv; k++) X[k] = I_h(h, k) * W[k];
+            for (int k = 1; k < nv; k++) X[k] = I_hk(G, h, k) * W[k];
             for (int k = 0; k < nv; k++) {
                 size_t c = (size_t)i * nv + k;
                 double vgp = 0.0;
@@ -558,7 +630,7 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
                 w->slowp[c] = -kv * (w->sc2[c] + D_c(G, X, k) - vgp - gW);
             }
             /* slow part of Eq. 35 (G7: with the r^2 factors of Eq. 27) */
-            for (int k = 1; k < nv; k++) X[k] = I_h(th, k) * W[k];
+            for (int k = 1; k < nv; k++) X[k] = I_hk(G, th, k) * W[k];
             for (int k = 0; k < nv; k++) {
                 size_t c = (size_t)i * nv + k;
                 w->slowrt[c] = -w->sc3[c] - D_c(G, X, k);
@@ -619,7 +691,7 @@ static void hyper_diffusion(const orc_geom *G, orc_work *w) {
         const double *rho = w->rho_t + (size_t)i * nv, *W = w->W_t + (size_t)i * (nv + 1);
         double *wv = a + (size_t)i * (nv + 1);
         wv[0] = 0.0; wv[nv] = 0.0;
-        for (int k = 1; k < nv; k++) wv[k] = W[k] / I_h(rho, k);
+        for (int k = 1; k < nv; k++) wv[k] = W[k] / I_hk(G, rho, k);
     }
     hlap_interfaces(G, a, b);
 #pragma omp parallel for schedule(static)
@@ -627,7 +699,7 @@ static void hyper_diffusion(const orc_geom *G, orc_work *w) {
         const double *rho = w->rho_t + (size_t)i * nv;
         double *x = b + (size_t)i * (nv + 1);
         x[0] = 0.0; x[nv] = 0.0;
-        for (int k = 1; k < nv; k++) x[k] = I_h(rho, k) * x[k];
+        for (int k = 1; k < nv; k++) x[k] = I_hk(G, rho, k) * x[k];
     }
     hlap_interfaces(G, b, c);
 #pragma omp parallel for schedule(static)
@@ -702,10 +774,30 @@ static void tridiag_coefficients(const orc_geom *G, double delta, const double *
     const double kv = P->Rd / (P->Cp - P->Rd), dz = G->dz, g = P->gravity;
     const double *rc = G->r_c, *rh = G->r_h;
     const double d2 = delta * delta;
+    if (!G->uniform) {
+        /* the same elimination with layers of unequal thickness: t_k = z_h,k+1 - z_h,k (layer), s_k = z_k - z_k-1
+         * (centre spacing of G_h), I_h[Y]_k = wl Y_k-1 + wu Y_k (Eq. 8-9, k = 1) */
+        const double *zh = G->z_h, *zc = G->z_c;
+        for (int k = 1; k < nv; k++) {
+            double hk = I_h(G, h, k);
+            double hkp = (k + 1 < nv) ? I_h(G, h, k + 1) : 0.0;
+            double hkm = (k - 1 > 0) ? I_h(G, h, k - 1) : 0.0;
+            double rk2 = rc[k] * rc[k], rkm2 = rc[k - 1] * rc[k - 1];
+            double tk = zh[k + 1] - zh[k], tkm = zh[k] - zh[k - 1], sk = zc[k] - zc[k - 1];
+            double wl = (zc[k] - zh[k]) / sk, wu = (zh[k] - zc[k - 1]) / sk;
+            c[k] = -(d2 * kv / sk) * (rh[k + 1] * rh[k + 1] * hkp / (rk2 * tk) - gt[k + 1] / 2.0)
+                   - d2 * g * wu * rh[k + 1] * rh[k + 1] / (rk2 * tk);
+            a[k] = -(d2 * kv / sk) * (rh[k - 1] * rh[k - 1] * hkm / (rkm2 * tkm) + gt[k - 1] / 2.0)
+                   + d2 * g * wl * rh[k - 1] * rh[k - 1] / (rkm2 * tkm);
+            b[k] = 1.0 + (d2 * kv / sk) * rh[k] * rh[k] * hk * (1.0 / (rk2 * tk) + 1.0 / (rkm2 * tkm))
+                   - d2 * g * rh[k] * rh[k] * (wl / (rkm2 * tkm) - wu / (rk2 * tk));
+        }
+        return;
+    }
     for (int k = 1; k < nv; k++) {
-        double hk = I_h(h, k);
-        double hkp = (k + 1 < nv) ? I_h(h, k + 1) : 0.0;   /* multiplies W_nv = 0 */
-        double hkm = (k - 1 > 0) ? I_h(h, k - 1) : 0.0;    /* multiplies W_0  = 0 */
+        double hk = I_h(G, h, k);
+        double hkp = (k + 1 < nv) ? I_h(G, h, k + 1) : 0.0;   /* multiplies W_nv = 0 */
+        double hkm = (k - 1 > 0) ? I_h(G, h, k - 1) : 0.0;    /* multiplies W_0  = 0 */
         double rk2 = rc[k] * rc[k], rkm2 = rc[k - 1] * rc[k - 1];
         c[k] = -(d2 * kv / dz) * (rh[k + 1] * rh[k + 1] * hkp / (rk2 * dz) - gt[k + 1] / 2.0)
                - (d2 * g / (2.0 * dz)) * rh[k + 1] * rh[k + 1] / rk2;
@@ -720,7 +812,7 @@ static void tridiag_coefficients(const orc_geom *G, double delta, const double *
 static void substep(const orc_geom *G, orc_work *w, double delta) {
     const int N = G->N, nv = G->nv;
     const orc_planet *P = &G->P;
-    const double kv = P->Rd / (P->Cp - P->Rd), dz = G->dz, g = P->gravity;
+    const double kv = P->Rd / (P->Cp - P->Rd), g = P->gravity;
     const size_t nc = w->nc;
 
     /* Fig. 6 small-step 1 (NEXT-1, only when K_d > 0) */
@@ -768,14 +860,14 @@ static void substep(const orc_geom *G, orc_work *w, double delta) {
             /* a6: assemble and solve (Eq. 37 as defined by elimination, R8; L339) */
             tridiag_coefficients(G, delta, h, gt, a, b, c);
             for (int k = 1; k < nv; k++)
-                d[k] = Ws[k] + delta * Svr[k] - delta * G_h(pq, k, dz) - delta * g * I_h(rq, k);
+                d[k] = Ws[k] + delta * Svr[k] - delta * G_h(G, pq, k) - delta * g * I_h(G, rq, k);
             Wn[0] = 0.0; Wn[nv] = 0.0;
             if (nv > 1) orc_thomas(nv - 1, a, b, c, d, Wn);
             /* a7: Eq. 32 with the new momenta (L341) */
             for (int k = 0; k < nv; k++) w->rho_s[c0 + k] = w->rho_s[c0 + k] + delta * (Srho[k] - D_c(G, Wn, k));
             /* a8: Eq. 35 (G7) */
             X[0] = 0.0; X[nv] = 0.0;
-            for (int k = 1; k < nv; k++) X[k] = I_h(th, k) * Wn[k];
+            for (int k = 1; k < nv; k++) X[k] = I_h(G, th, k) * Wn[k];
             for (int k = 0; k < nv; k++)
                 w->rt[c0 + k] = w->rt[c0 + k] + delta * (w->slowrt[c0 + k] - w->sc3[c0 + k] - D_c(G, X, k));
             /* a9: Eq. 36 */
@@ -987,7 +1079,7 @@ void orc_diagnostics(const orc_geom *G, const double *rho, const double *V, cons
     for (int i = 0; i < N; i++)
         for (int k = 0; k < nv; k++) {
             size_t c = (size_t)i * nv + k;
-            double vol = G->Ac[i] * G->r_c[k] * G->r_c[k] * G->dz;
+            double vol = G->Ac[i] * G->r_c[k] * G->r_c[k] * (G->uniform ? G->dz : G->z_h[k + 1] - G->z_h[k]);
             double wc = I_c(W + (size_t)i * (nv + 1), k);
             double ke = 0.5 * (V[3 * c] * V[3 * c] + V[3 * c + 1] * V[3 * c + 1] + V[3 * c + 2] * V[3 * c + 2] + wc * wc) / rho[c];
             double e = Cv * p[c] / P->Rd + ke + rho[c] * P->gravity * G->z_c[k];
@@ -1001,6 +1093,23 @@ void orc_diagnostics(const orc_geom *G, const double *rho, const double *V, cons
 /* ---------------------------------------------------------------------------------------------
  * Pieces exposed one at a time for the pins (same code the step runs)
  * ------------------------------------------------------------------------------------------- */
+
+/* NEXT-3 pins: the vertical operators alone on one column.  order_k != 0: the interpolations at the order of
+ * the run (I_hk, I_ck), else the linear ones of the acoustic system.  Yc [nv] -> Ih [nv+1] (ends 0), Gh [nv+1]
+ * (ends 0); Xh [nv+1] -> Ic [nv], Dc [nv]. */
+void orc_vertical_ops(const orc_geom *G, int order_k, const double *Yc, const double *Xh,
+                      double *Ih, double *Gh, double *Ic, double *Dc) {
+    const int nv = G->nv;
+    Ih[0] = Ih[nv] = Gh[0] = Gh[nv] = 0.0;
+    for (int k = 1; k < nv; k++) {
+        Ih[k] = order_k ? I_hk(G, Yc, k) : I_h(G, Yc, k);
+        Gh[k] = G_h(G, Yc, k);
+    }
+    for (int k = 0; k < nv; k++) {
+        Ic[k] = order_k ? I_ck(G, Xh, k) : I_c(Xh, k);
+        Dc[k] = D_c(G, Xh, k);
+    }
+}
 
 /* P10: tridiagonal coefficients of one column, arrays [nv+1] indexed by interface */
 void orc_tridiag_coefficients(const orc_geom *G, double delta, const double *h, const double *gt,

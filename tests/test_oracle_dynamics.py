@@ -39,11 +39,17 @@ def _dense_column_solve(G, delta, col, stage, dev, divV, divhV):
     nv = G.nv
     P = G.planet
     kv = P["Rd"] / (P["Cp"] - P["Rd"])
-    g, dz = P["gravity"], G.dz
+    g = P["gravity"]
     rc, rh = G.r_c, G.r_h
+    # layer thickness t_j, centre spacing s_k and the linear (Eq. 8-9, k = 1) weights of interface k between the
+    # centres k-1 and k; equal layers: t = s = dz, weights 1/2
+    t = np.diff(G.z_h)
+    sp = np.concatenate([[1.0], np.diff(G.z_c)])
+    wl = np.concatenate([[0.0], (G.z_c[1:] - G.z_h[1:nv]) / np.diff(G.z_c)])
+    wu = np.concatenate([[0.0], (G.z_h[1:nv] - G.z_c[:-1]) / np.diff(G.z_c)])
     h, gt = stage["h"][col], stage["gt"][col]
     hh = np.zeros(nv + 1)
-    hh[1:nv] = 0.5 * (h[:-1] + h[1:])
+    hh[1:nv] = wl[1:] * h[:-1] + wu[1:] * h[1:]
     nW = nv - 1
     n = nW + 2 * nv
     A = np.zeros((n, n))
@@ -57,24 +63,24 @@ def _dense_column_solve(G, delta, col, stage, dev, divV, divhV):
         # Eq. 32: rho' + delta * D_c[W'] = rho* + delta S_rho
         A[iR(j), iR(j)] = 1.0
         if j + 1 <= nv - 1:
-            A[iR(j), iW(j + 1)] += delta * rh[j + 1] ** 2 / (rc[j] ** 2 * dz)
+            A[iR(j), iW(j + 1)] += delta * rh[j + 1] ** 2 / (rc[j] ** 2 * t[j])
         if j >= 1:
-            A[iR(j), iW(j)] -= delta * rh[j] ** 2 / (rc[j] ** 2 * dz)
+            A[iR(j), iW(j)] -= delta * rh[j] ** 2 / (rc[j] ** 2 * t[j])
         b[iR(j)] = dev["rho_s"][col, j] + delta * S_rho[j]
         # pressure: p' + delta kv (D_c[h_h W'] - I_c[g~ W']) = p* + delta S_p
         A[iP(j), iP(j)] = 1.0
         if j + 1 <= nv - 1:
-            A[iP(j), iW(j + 1)] += delta * kv * (rh[j + 1] ** 2 * hh[j + 1] / (rc[j] ** 2 * dz) - 0.5 * gt[j + 1])
+            A[iP(j), iW(j + 1)] += delta * kv * (rh[j + 1] ** 2 * hh[j + 1] / (rc[j] ** 2 * t[j]) - 0.5 * gt[j + 1])
         if j >= 1:
-            A[iP(j), iW(j)] += delta * kv * (-rh[j] ** 2 * hh[j] / (rc[j] ** 2 * dz) - 0.5 * gt[j])
+            A[iP(j), iW(j)] += delta * kv * (-rh[j] ** 2 * hh[j] / (rc[j] ** 2 * t[j]) - 0.5 * gt[j])
         b[iP(j)] = dev["p_s"][col, j] + delta * S_p[j]
     for k in range(1, nv):
         # Eq. 34: (W' - W*)/delta + G_h[p'] + g I_h[rho'] = S_vr
         A[iW(k), iW(k)] = 1.0 / delta
-        A[iW(k), iP(k)] += 1.0 / dz
-        A[iW(k), iP(k - 1)] -= 1.0 / dz
-        A[iW(k), iR(k)] += 0.5 * g
-        A[iW(k), iR(k - 1)] += 0.5 * g
+        A[iW(k), iP(k)] += 1.0 / sp[k]
+        A[iW(k), iP(k - 1)] -= 1.0 / sp[k]
+        A[iW(k), iR(k)] += wu[k] * g
+        A[iW(k), iR(k - 1)] += wl[k] * g
         b[iW(k)] = stage["Svr"][col, k] + dev["W_s"][col, k] / delta
     x = np.linalg.solve(A, b)
     return x[:nW], x[nW:nW + nv], x[nW + nv:]

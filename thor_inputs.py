@@ -77,6 +77,34 @@ def hydrostatic_isothermal(planet, nv, p_s, T0):
     return p
 
 
+def stretched_interfaces(planet, nv, ratio):
+    """nv+1 interface altitudes from 0 to z_top whose layer thickness grows geometrically, top/bottom = ratio
+    (NEXT-3 workloads: thin layers near the surface)."""
+    t = ratio ** (np.arange(nv) / max(nv - 1, 1))
+    z = np.concatenate([[0.0], np.cumsum(t)])
+    z *= planet["z_top"] / z[-1]
+    z[-1] = planet["z_top"]
+    return z
+
+
+def hydrostatic_column(planet, z_h, p_s, T_c):
+    """Pressure column in DISCRETE hydrostatic balance for layer-centre temperatures T_c on layers bounded by
+    z_h (centres at the midpoints): (p_k - p_k-1)/(z_k - z_k-1) + g (wl rho_k-1 + wu rho_k) = 0 with
+    rho = p/(Rd T) and the linear weights of the interface between the two centres; p_0 from the surface
+    pressure with the lowest layer's temperature.  Uniform layers and constant T: hydrostatic_isothermal."""
+    z_h = np.asarray(z_h, dtype=np.float64)
+    z_c = 0.5 * (z_h[:-1] + z_h[1:])
+    g, Rd = planet["gravity"], planet["Rd"]
+    nv = z_c.size
+    p = np.empty(nv)
+    p[0] = p_s * math.exp(-g * z_c[0] / (Rd * T_c[0]))
+    for k in range(1, nv):
+        s = z_c[k] - z_c[k - 1]
+        wl, wu = (z_c[k] - z_h[k]) / s, (z_h[k] - z_c[k - 1]) / s
+        p[k] = p[k - 1] * (1.0 / s - g * wl / (Rd * T_c[k - 1])) / (1.0 / s + g * wu / (Rd * T_c[k]))
+    return p
+
+
 def rest_state(planet, nv, n_cols, p_s, T0):
     p_col = hydrostatic_isothermal(planet, nv, p_s, T0)
     p = np.tile(p_col, (n_cols, 1))
