@@ -1,40 +1,40 @@
 """Held-Suarez benchmark driver (section 7.1): the base HE-VI step + the hyper-diffusion and
 divergence damping of section 4 (NEXT-1) + the forcing of Eq. 51-55 from the evolving sigma (NEXT-2).
 
-    python -m paper_1607_05535_b200.held_suarez_run [days] [level] [layers]
+    python examples/held_suarez_run.py [days] [level] [layers]
 
-Level 5 x 32 layers, dt = 1000 s, n = 6 acoustic substeps, D = 0.004837 (Table 1), rest state at 300 K
-with 0.1 K noise, lid at 32 km.  Prints the zonal-mean zonal wind maximum every 50 days.  Everything
-runs in the CUDA library; this file only sets the run up and bins the output by latitude."""
+The paper's set-up (L452-L454): level 5 x 37 layers from 0 to 32 km, dt = 1000 s, D = 0.004837 (Table 1: 6.46e3 s),
+at rest, every column with the temperature profile of T_eq at the equator in (discrete) hydrostatic balance.
+n = 6 acoustic substeps (L252's example) and p_s = 1e5 Pa are not printed for this run.  Prints the zonal-mean
+zonal wind maximum every 50 days.  Everything runs in the CUDA library; this file only sets the run up and bins
+the output by latitude."""
+import os
 import sys
 import time
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
 import numpy as np
 import torch
 
 import paper_1607_05535_b200 as thor
+import thor_inputs as ti
 
-EARTH = dict(radius=6.371e6, omega=7.292e-5, gravity=9.8, Rd=287.0, Cp=1005.0, p_ref=1.0e5, z_top=32.0e3)
-HELD_SUAREZ = dict(T_surf=315.0, dT_y=60.0, dth_z=10.0, T_min=200.0, k_a=1.0 / (40 * 86400.0), k_s=1.0 / (4 * 86400.0),
-                   k_f=1.0 / 86400.0, sigma_b=0.7, p_star=1.0e5)
+EARTH = dict(ti.EARTH, z_top=32.0e3)
+HELD_SUAREZ = ti.HELD_SUAREZ
 
 
 def main():
     days = int(sys.argv[1]) if len(sys.argv) > 1 else 300
     level = int(sys.argv[2]) if len(sys.argv) > 2 else 5
-    nv = int(sys.argv[3]) if len(sys.argv) > 3 else 32
+    nv = int(sys.argv[3]) if len(sys.argv) > 3 else 37
     g = thor.Grid(level, nv, EARTH)
     xyz, N = g.view["xyz"], g.n_cols
-    # isothermal column in discrete hydrostatic balance, 300 K, p_s = 1e5 Pa, plus 0.1 K noise
-    dz = EARTH["z_top"] / nv
-    q = EARTH["gravity"] * dz / (2.0 * EARTH["Rd"] * 300.0)
-    pcol = np.empty(nv)
-    pcol[0] = 1.0e5 * np.exp(-EARTH["gravity"] * 0.5 * dz / (EARTH["Rd"] * 300.0))
-    for k in range(1, nv):
-        pcol[k] = pcol[k - 1] * (1.0 - q) / (1.0 + q)
+    # L452: the equatorial T_eq profile in discrete hydrostatic balance, the same in every column, at rest
+    _, _, z_h = ti.vertical_grid(EARTH, nv)
+    pcol, Tcol = ti.benchmark_column(EARTH, z_h, 1.0e5, ti.held_suarez_equator_profile(EARTH, HELD_SUAREZ))
     p = np.tile(pcol, (N, 1))
-    T = 300.0 + np.random.default_rng(1).uniform(-0.1, 0.1, size=p.shape)
-    rho = p / (EARTH["Rd"] * T)
+    rho = p / (EARTH["Rd"] * np.tile(Tcol, (N, 1)))
     stream = torch.cuda.Stream()
     st = thor.State(g, rho, np.zeros((N, nv, 3)), np.zeros((N, nv + 1)), p, cuda_stream=stream.cuda_stream)
     st.set_diffusion(0.004837)

@@ -1,37 +1,35 @@
 """Tidally locked hot-Jupiter benchmark driver (section 7.2): base HE-VI step + NEXT-1 + the
 forcing of Eq. 59-61.
 
-    python -m paper_1607_05535_b200.hot_jupiter_run [days] [level] [layers]
+    python examples/hot_jupiter_run.py [days] [level] [layers]
 
-Table 1's planet, level 5, 0-4875 km, dt = 600 s, n = 6, D = 0.01992 (Table 1: 941.2 s), isothermal
-1600 K at rest (L529); surface pressure 1e5 Pa (not printed in the paper).  Prints the zonal-mean zonal
-wind every 50 Earth days.  Everything runs in the CUDA library."""
+The paper's set-up (L529): Table 1's planet, level 5 x 37 layers from 0 to 4875 km, dt = 600 s, D = 0.01992
+(Table 1: 941.2 s), isothermal 1600 K in (discrete) hydrostatic balance, at rest.  n = 6 and the surface pressure
+1e5 Pa are not printed in the paper.  Prints the zonal-mean zonal wind every 50 Earth days.  Everything runs in
+the CUDA library."""
+import os
 import sys
 import time
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
 import numpy as np
 import torch
 
 import paper_1607_05535_b200 as thor
+import thor_inputs as ti
 
-PLANET = dict(radius=1.0e8, omega=2.1e-5, gravity=8.0, Rd=3779.0, Cp=13226.5, p_ref=1.0e5, z_top=4.875e6)
-FORCING = dict(T_surf=1600.0, Gamma=2.0e-4, dT_stra=10.0, z_stra=2.0e6, sigma_stra=0.12, dT_EP=300.0, tau_rad=1.5e5)
+PLANET = ti.PAPER_HOT_JUPITER
+FORCING = ti.HOT_JUPITER_FORCING
 
 
 def main():
     days = int(sys.argv[1]) if len(sys.argv) > 1 else 300
     level = int(sys.argv[2]) if len(sys.argv) > 2 else 5
-    nv = int(sys.argv[3]) if len(sys.argv) > 3 else 32
+    nv = int(sys.argv[3]) if len(sys.argv) > 3 else 37
     g = thor.Grid(level, nv, PLANET)
     xyz, N = g.view["xyz"], g.n_cols
-    T0, dz = 1600.0, PLANET["z_top"] / nv
-    q = PLANET["gravity"] * dz / (2.0 * PLANET["Rd"] * T0)
-    pcol = np.empty(nv)
-    pcol[0] = 1.0e5 * np.exp(-PLANET["gravity"] * 0.5 * dz / (PLANET["Rd"] * T0))
-    for k in range(1, nv):
-        pcol[k] = pcol[k - 1] * (1.0 - q) / (1.0 + q)
-    p = np.tile(pcol, (N, 1))
-    rho = p / (PLANET["Rd"] * T0)
+    rho, _, _, p = ti.rest_state(PLANET, nv, N, 1.0e5, 1600.0)
     stream = torch.cuda.Stream()
     st = thor.State(g, rho, np.zeros((N, nv, 3)), np.zeros((N, nv + 1)), p, cuda_stream=stream.cuda_stream)
     st.set_diffusion(0.01992)

@@ -105,6 +105,36 @@ def hydrostatic_column(planet, z_h, p_s, T_c):
     return p
 
 
+def benchmark_column(planet, z_h, p_s, T_of):
+    """Initial column of the paper's Earth benchmark ("the same temperature profile in every column
+    taken from the function T_eq at the equator in hydrostatic equilibrium"): layer-centre temperatures
+    T_k = T_of(z_k, p_k, p_s) with the pressure in DISCRETE hydrostatic balance (hydrostatic_column).
+    T_eq depends on the pressure itself (Eq. 54), so the pair is found by fixed-point iteration (a contraction:
+    the profile moves p by O(dT/T) per sweep); returns (p, T)."""
+    z_h = np.asarray(z_h, dtype=np.float64)
+    z_c = 0.5 * (z_h[:-1] + z_h[1:])
+    T = np.full(z_c.size, T_of(z_c[:1], np.array([p_s]), p_s)[0])
+    p = hydrostatic_column(planet, z_h, p_s, T)
+    for _ in range(200):
+        T_new = T_of(z_c, p, p_s)
+        p_new = hydrostatic_column(planet, z_h, p_s, T_new)
+        done = np.abs(p_new - p).max() <= 1e-14 * p_s
+        p, T = p_new, T_new
+        if done:
+            break
+    return p, T
+
+
+def held_suarez_equator_profile(planet, hs):
+    """T_eq of Eq. 54 at the equator (latitude 0) as a function of pressure: the initial profile of L452."""
+    kappa = planet["Rd"] / planet["Cp"]
+
+    def T_of(z, p, p_s):
+        pr = p / hs["p_star"]
+        return np.maximum(hs["T_min"], (hs["T_surf"] - hs["dth_z"] * np.log(pr)) * pr ** kappa)
+    return T_of
+
+
 def rest_state(planet, nv, n_cols, p_s, T0):
     p_col = hydrostatic_isothermal(planet, nv, p_s, T0)
     p = np.tile(p_col, (n_cols, 1))
