@@ -167,6 +167,28 @@ def time_oracle(workload, n_steps, warmup, threads=None):
     return cells * n_steps / el, el / max(n_steps, 1), used, sample
 
 
+def time_oracle_operators(workload, reps=3):
+    """Config 1's stencils (Eq. 6, Eq. 7) as the oracle evaluates them, timed alone on the host cores on the
+    grid size of `workload`: seconds per application, all cores; oracle/ only."""
+    import oracle
+    from oracle import grid_oracle
+    cfg = ti.CONFIGS[workload]
+    level = oracle_sample_level(workload)
+    xyz, nbr, C, _ = grid_oracle.build(level, smooth=False)
+    G = oracle.Geometry(xyz, nbr, cfg["nv"], cfg["planet"], C)
+    rng = np.random.default_rng(ti.SEED0)
+    s = rng.standard_normal((xyz.shape[0], cfg["nv"]))
+    v = rng.standard_normal((xyz.shape[0], cfg["nv"], 3))
+    out = {}
+    for name, fn, arg in (("div", G.hdiv, v), ("grad", G.hgrad, s), ("lap", G.hlap, s)):
+        fn(arg)
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            fn(arg)
+        out[name] = (time.perf_counter() - t0) / reps
+    return out, oracle.num_threads(), level
+
+
 def workload_config(workload, N, world):
     """The `config` object both arms print (same workload, same words)."""
     cfg = ti.CONFIGS[workload]
@@ -400,6 +422,11 @@ def run_cuda(args):
         v1, _, _, _ = time_oracle(WORKLOAD, 1, 0, threads=1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                 "value_1_thread": v1}
+        ops, op_cores, op_level = time_oracle_operators(WORKLOAD)
+        line["operators"].update({"oracle_div_ms": ops["div"] * 1e3, "oracle_grad_ms": ops["grad"] * 1e3,
+                                  "oracle_lap_ms": ops["lap"] * 1e3, "oracle_cores": op_cores,
+                                  "oracle_what": "the oracle's orc_hdiv / orc_hgrad / orc_hlap alone on level %d x %d "
+                                                 "(unsmoothed grid of its own generator), all host cores" % (op_level, nv)})
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -619,12 +619,19 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
             THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
         }
         for (int sub = 0; sub < ns; ++sub) {
-            if (Kd_div > 0.0)                                           // + Fig. 6 small-step 1
-                THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, sub == 0 ? int(X_D3N) : int(X_D3));
-            else THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
+            // stage 1: Phi*(0) = 0 exactly (Eq. 31 with Phi^[t] = Phi^n), so its substep reads no deviation row
+            if (Kd_div > 0.0) {                                         // + Fig. 6 small-step 1
+                if (stage == 1) THOR_DISPATCH(k_momentum_dd_stage1, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, int(X_D3N));
+                else THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, sub == 0 ? int(X_D3N) : int(X_D3));
+            } else if (stage == 1) {
+                THOR_DISPATCH(k_momentum_stage1, nv, Npad, st, g, S, delta, dir(tn.k1));
+            } else {
+                THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
+            }
             TunePair t2 = tn;
             t2.k2 = dir(tn.k2);
-            if (int rc = launch_vertical(s->grid, g, S, delta, sub == 0 ? 1 : 0, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
+            const int first = stage == 1 ? 2 : (sub == 0 ? 1 : 0);
+            if (int rc = launch_vertical(s->grid, g, S, delta, first, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
         }
     }
     THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, s->hs, s->hj, dt, dir(tn.ks));

@@ -636,12 +636,9 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 
     // Eq. 31: Phi*(0) = Phi^n - Phi^[t]; (rho theta)*(0) = (rho theta)^n - (rho theta)^[t]
     if (stage == 1) {
+        // Phi*(0) = 0 exactly: the six deviation rows are neither written here nor read by the stage's single
+        // substep (k_momentum_stage1, k_vertical with first = 2), which overwrites all of them
         st_row<E>(me + F_RTN * NVP, rtt);
-#pragma unroll
-        for (int e = 0; e < E; ++e) d[e] = 0.0;
-        st_row<E>(me + F_RHOS * NVP, d); st_row<E>(me + F_VAS * NVP, d); st_row<E>(me + F_VBS * NVP, d);
-        st_row<E>(me + F_WS * NVP, d);   st_row<E>(me + F_PS * NVP, d);
-        st_row<E>(me + F_RTS * NVP, d);
     } else {
         auto dev = [&](int fn, int fs, const double (&t)[E]) {
             ld_rw<E>(me + fn * NVP, d);
@@ -910,14 +907,18 @@ k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X
 // K1 (a4): explicit horizontal momentum, Eq. 33 (Fig. 6 small-step 2):
 //   V*' = V* + delta (-grad_h p* / r + slowV).  Gathers p* from the 6 neighbours.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E, bool DD>
+// ZERO: the substep of stage 1, where V*(0) = 0 and p*(0) = 0 exactly (Eq. 31 with Phi^[t] = Phi^n): nothing of the
+// deviation rows is read and there is no gradient to gather; V*' = delta slowV.
+template <int G, int E, bool DD, bool ZERO = false>
 __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict__ S, double delta, const Tune& tn,
                                                const double* __restrict__ Xdd, double Kd_div, int d3row) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 1);
+        if (!ZERO) {
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 1);
+        }
         prefetch_block_rows<G, E>(S, wk.ahead_bid, F_SVA, 2);
     }
     if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_H, F_PT - F_H + 1);   // the column-solve kernel starts here
@@ -931,24 +932,26 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
     const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
     __syncwarp();
-    double p0[E], pj[6][E], ga[E], gb[E];
-    ld_nc<E>(me + F_PS * NVP, p0);
+    double ga[E], gb[E], ri[E], va[E], vb[E], sa[E], sb[E];
 #pragma unroll
-    for (int j = 0; j < 6; ++j) ld_nc<E>(S + size_t(nb[j]) * REC + L.k0 + F_PS * NVP, pj[j]);
-    double ri[E], va[E], vb[E], sa[E], sb[E];
-    ld_nc<E>(g.rinv + L.k0, ri);
-    ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, vb);
-    ld_nc<E>(me + F_SVA * NVP, sa); ld_nc<E>(me + F_SVB * NVP, sb);
+    for (int e = 0; e < E; ++e) ga[e] = gb[e] = va[e] = vb[e] = 0.0;
+    if constexpr (!ZERO) {
+        double p0[E], pj[6][E];
+        ld_nc<E>(me + F_PS * NVP, p0);
 #pragma unroll
-    for (int e = 0; e < E; ++e) ga[e] = gb[e] = 0.0;
+        for (int j = 0; j < 6; ++j) ld_nc<E>(S + size_t(nb[j]) * REC + L.k0 + F_PS * NVP, pj[j]);
+        ld_rw<E>(me + F_VAS * NVP, va); ld_rw<E>(me + F_VBS * NVP, vb);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) {
+        for (int j = 0; j < 6; ++j) {
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const double d = pj[j][e] - p0[e];
-            ga[e] = fma(wgv[2 * j], d, ga[e]); gb[e] = fma(wgv[2 * j + 1], d, gb[e]);
+            for (int e = 0; e < E; ++e) {
+                const double d = pj[j][e] - p0[e];
+                ga[e] = fma(wgv[2 * j], d, ga[e]); gb[e] = fma(wgv[2 * j + 1], d, gb[e]);
+            }
         }
     }
+    ld_nc<E>(g.rinv + L.k0, ri);
+    ld_nc<E>(me + F_SVA * NVP, sa); ld_nc<E>(me + F_SVB * NVP, sb);
     if constexpr (DD) {
         // NEXT-1, Fig. 6 small-step 1: divergence damping F_dd = -K_d lap(grad_h D3) (RD4) as ONE two-ring
         // stencil on the D3 row (composed on the host: thor_api.cu), already projected and in the tangent basis
@@ -989,6 +992,11 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
     momentum_block<G, E, false>(g, S, delta, tn, nullptr, 0.0, 0);
 }
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_momentum_stage1(Geom g, double* __restrict__ S, double delta, Tune tn) {
+    momentum_block<G, E, false, true>(g, S, delta, tn, nullptr, 0.0, 0);
+}
 // the same kernel with NEXT-1's divergence damping added to Eq. 33; d3row: the X row that holds the 3-D
 // divergence of the current momentum (X_D3N in the first substep of a stage, where V^[t] + V*(0) = V^n; X_D3 after)
 template <int G, int E>
@@ -996,13 +1004,19 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_momentum_dd(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div, int d3row) {
     momentum_block<G, E, true>(g, S, delta, tn, Xdd, Kd_div, d3row);
 }
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_momentum_dd_stage1(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div, int d3row) {
+    momentum_block<G, E, true, true>(g, S, delta, tn, Xdd, Kd_div, d3row);
+}
 
 // ---------------------------------------------------------------------------------------------
 // K2 (a5-a9): horizontal divergences of the new momentum, the implicit vertical momentum
 // (Eq. 37; two sweeps with the stage's LU factors), density (Eq. 32), rho*theta (Eq. 35, G7) and
 // the pressure deviation (Eq. 36).  Fig. 6 small-steps 3-6.  Gathers V*', h, theta from the 6
-// neighbours; everything else is column-local.  `first`: p*(tau) is read (first substep of a
-// stage, p* = p^n - p^[t]); otherwise it is re-evaluated from (rho theta)* exactly as the previous
+// neighbours; everything else is column-local.  `first` = 1: p*(tau) is read (first substep of
+// stages 2 and 3, p* = p^n - p^[t]); 2: the substep of stage 1, where every deviation is exactly 0 and
+// no deviation row is read; 0: p* is re-evaluated from (rho theta)* exactly as the previous
 // substep stored it, which saves one row of HBM reads.
 //
 // vertical_column is the work of one lane group on one column.  `own` points at row 0 (layer k0)
@@ -1052,7 +1066,12 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
     ld_nc<E>(g.wl + k0, wl);   ld_nc<E>(g.wh + k0, wh);
 
     double rho_s[E], p_s[E], W_s[E], rts[E], srho[E], sp[E], sW[E], srt[E], pt[E], irt[E];
-    ld_rw<E>(own + F_RHOS * NVP, rho_s); ld_rw<E>(own + F_WS * NVP, W_s); ld_rw<E>(own + F_RTS * NVP, rts);
+    if (first == 2) {                     // stage 1: Phi*(0) = 0 exactly, the rows hold nothing yet
+#pragma unroll
+        for (int e = 0; e < E; ++e) rho_s[e] = W_s[e] = rts[e] = 0.0;
+    } else {
+        ld_rw<E>(own + F_RHOS * NVP, rho_s); ld_rw<E>(own + F_WS * NVP, W_s); ld_rw<E>(own + F_RTS * NVP, rts);
+    }
     ld_rw<E>(own + F_SRHO * NVP, srho);  ld_rw<E>(own + F_SP * NVP, sp);  ld_rw<E>(own + F_SW * NVP, sW);
     ld_rw<E>(own + F_SRT * NVP, srt);    ld_rw<E>(own + F_PT * NVP, pt);
     {   // 1/(rho theta)^[t] from rows already here: h/theta = Cp p/(Rd rho theta)
@@ -1060,7 +1079,10 @@ __device__ __forceinline__ void vertical_column(const Geom& g, double* __restric
 #pragma unroll
         for (int e = 0; e < E; ++e) irt[e] = kap * h0[e] / (th0[e] * pt[e]);
     }
-    if (first) {
+    if (first == 2) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) p_s[e] = 0.0;
+    } else if (first) {
         ld_rw<E>(own + F_PS * NVP, p_s);
     } else {
 #pragma unroll
@@ -1121,7 +1143,11 @@ __device__ __forceinline__ void vertical_block(const Geom& g, double* __restrict
                                                double* __restrict__ Xdd) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
-    if (wk.ahead_bid >= 0) prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, F_PT + 1);
+    if (wk.ahead_bid >= 0) {                        // only the rows this launch reads (see `first`)
+        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, first == 1 ? F_PT + 1 : int(F_PS));
+        if (first == 0) prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHOS, F_PT - F_RHOS + 1);
+        if (first == 2) prefetch_block_rows<G, E>(S, wk.ahead_bid, F_SRHO, F_PT - F_SRHO + 1);
+    }
     if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_SVA, 2);               // the next momentum kernel starts here
     __shared__ double wsm[kWarpsPerBlock * 32 / G][16];
     double* wdv = wsm[threadIdx.x / G];
