@@ -21,7 +21,8 @@
  *                                 both ends are the rigid lid (L339) and are forced to 0.
  *    The device keeps a different, locality-preserving column order; it is internal
  *    (thor_grid_view.device_order documents it for the *_device entry points).
- *  - Layers are uniform in altitude: dz = z_top / n_layers, centre k at (k+1/2) dz (R6).
+ *  - Layers are uniform in altitude unless thor_grid_create_vertical says otherwise: dz = z_top / n_layers,
+ *    centre k at (k+1/2) dz (R6).
  *  - thor_step and thor_acoustic_substeps are asynchronous on the stream given to thor_state_init;
  *    thor_state_get, thor_state_set and thor_diagnostics synchronise that stream.
  *  - On a non-default stream thor_step replays a large step as a CUDA graph after the first directly
@@ -87,6 +88,15 @@ typedef struct { double total_mass, total_energy; } thor_diag;
  * n_cols = 10*4^level + 2) -> spring dynamics (Eq. 10-12, beta = 1.15) -> centroid move (Eq. 13);
  * then the finite-volume stencil weights of Eq. 4-7 and the device column order.  Host only. */
 int thor_grid_create(int level, int n_layers, const thor_planet *planet, thor_grid **out);
+/* NEXT-3 (section 2.2, Eq. 8-9): the same grid with layers of unequal thickness and/or the vertical
+ * Lagrange interpolation of order k > 1.  z_interfaces: n_layers+1 strictly increasing altitudes, z_interfaces[0] = 0,
+ * the last one is the rigid lid and REPLACES planet->z_top; NULL = uniform layers.  Layer centres sit midway between
+ * their interfaces.  order_k: 1 (the paper's choice, L94) or 3; it enters the explicit slow terms (vertical fluxes of
+ * u, h, theta; I_h[rho] and I_h[F_r] of Eq. 42; I_c[W]; w = W/I_h[rho] of the hyper-diffusion), while the implicit
+ * acoustic system keeps k = 1 and stays tridiagonal (reading RV2).  Order 3 uses the two nearest nodes on each side
+ * of the target; where the column ends first the missing nodes are dropped (RV1).  Other orders: THOR_EINVAL. */
+int thor_grid_create_vertical(int level, int n_layers, const thor_planet *planet, const double *z_interfaces,
+                              int order_k, thor_grid **out);
 int thor_grid_get(const thor_grid *grid, thor_grid_view *out);
 void thor_grid_destroy(thor_grid *grid);
 

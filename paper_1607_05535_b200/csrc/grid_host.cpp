@@ -143,16 +143,12 @@ bool neighbour_table(int N, const std::vector<Tri>& tris, std::vector<int>& nbr,
     return true;
 }
 
-// Eq. 10-12.  Returns the number of steps taken.
-int spring_dynamics(std::vector<V3>& x, const std::vector<int>& nbr, const std::vector<int>& deg, int level) {
-    const int N = int(x.size());
-    const double dspr = kBeta * 2 * kPi / (10.0 * std::pow(2.0, level - 1));   // Eq. 12, A = 1
-    std::vector<V3> v(N, V3{0, 0, 0}), xn(N);
-    // the tolerance follows the grid spacing above level 4 (a fixed displacement is a smaller and
-    // smaller fraction of an edge there, and the long waves were already relaxed on the coarser levels)
-    const double tol = kSpringTol * std::pow(kSpringTolGrowth, std::max(0, level - 4));
+// Eq. 10-12 on the host.  Returns the number of steps taken.
+int spring_dynamics_host(int N, double* xyz, const int* nbr, const int* deg, const SpringParams& sp) {
+    std::vector<V3> x(N), v(N, V3{0, 0, 0}), xn(N);
+    for (int i = 0; i < N; ++i) x[i] = V3{xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2]};
     int it = 0;
-    for (; it < kSpringMaxIter; ++it) {
+    for (; it < sp.max_iter; ++it) {
         double worst = 0.0;
 #pragma omp parallel for schedule(static) reduction(max : worst)
         for (int i = 0; i < N; ++i) {
@@ -166,22 +162,35 @@ int spring_dynamics(std::vector<V3>& x, const std::vector<int>& nbr, const std::
                 const V3 pj = x[nbr[size_t(i) * 6 + k]];
                 double d = arc(p0, pj);
                 V3 e = unit(pj - dot(pj, p0) * p0);               // unit tangent at P_0 towards P_j
-                f = f + (kSpringK * (d - dspr)) * e;
+                f = f + (sp.k * (d - sp.dspr)) * e;
             }
-            f = f - kAlpha * v[i];                                // Eq. 10
-            V3 vi = v[i] + kSpringDt * f;
-            V3 pn = unit(p0 + kSpringDt * vi);                    // Eq. 11, back onto the sphere
+            f = f - sp.alpha * v[i];                              // Eq. 10
+            V3 vi = v[i] + sp.dt * f;
+            V3 pn = unit(p0 + sp.dt * vi);                        // Eq. 11, back onto the sphere
             v[i] = vi - dot(vi, pn) * pn;
             xn[i] = pn;
             worst = std::max(worst, norm(pn - p0));
         }
         x.swap(xn);
-        if (it >= kSpringMinIter && worst < tol) {
+        if (it >= sp.min_iter && worst < sp.tol) {
             ++it;
             break;
         }
     }
+    for (int i = 0; i < N; ++i) { xyz[3 * i] = x[i].x; xyz[3 * i + 1] = x[i].y; xyz[3 * i + 2] = x[i].z; }
     return it;
+}
+
+// the constants of one level's relaxation
+SpringParams spring_params(int level) {
+    SpringParams sp;
+    sp.dspr = kBeta * 2 * kPi / (10.0 * std::pow(2.0, level - 1));   // Eq. 12, A = 1
+    sp.k = kSpringK; sp.alpha = kAlpha; sp.dt = kSpringDt;
+    // the tolerance follows the grid spacing above level 4 (a fixed displacement is a smaller and
+    // smaller fraction of an edge there, and the long waves were already relaxed on the coarser levels)
+    sp.tol = kSpringTol * std::pow(kSpringTolGrowth, std::max(0, level - 4));
+    sp.min_iter = kSpringMinIter; sp.max_iter = kSpringMaxIter;
+    return sp;
 }
 
 // Eq. 13 (G4): sum_i (r_i x r_i+1)/|r_i x r_i+1| * arc(r_i, r_i+1), normalised.
@@ -201,12 +210,20 @@ double tri_area(V3 a, V3 b, V3 c) {   // spherical excess
 
 }  // namespace
 
-int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces) {
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces, int kord,
+                    SpringFn spring) {
     if (level < 0 || level > 9 || nv < 2 || nv > 128) return THOR_EINVAL;
+    if (kord != 1 && kord != 3) return THOR_EINVAL;
+    if (z_interfaces) {
+        if (z_interfaces[0] != 0.0) return THOR_EINVAL;
+        for (int k = 0; k < nv; ++k)
+            if (!(z_interfaces[k + 1] > z_interfaces[k])) return THOR_EINVAL;
+    }
     if (!(P.radius > 0) || !(P.z_top > 0) || !(P.Rd > 0) || !(P.Cp > P.Rd) || !(P.p_ref > 0)) return THOR_EINVAL;
     g.level = level;
     g.nv = nv;
     g.P = P;
+    if (z_interfaces) g.P.z_top = z_interfaces[nv];      // the lid is the last interface
 
     std::vector<V3> pts;
     std::vector<Tri> tris;
@@ -216,7 +233,10 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
     for (int l = 1; l <= level; ++l) {
         bisect(pts, tris);
         if (!neighbour_table(int(pts.size()), tris, nbr, deg)) return THOR_EINVAL;
-        g.spring_iterations += spring_dynamics(pts, nbr, deg, l);
+        static_assert(sizeof(V3) == 3 * sizeof(double), "V3 is three packed doubles");
+        const int its = (spring ? spring : spring_dynamics_host)(int(pts.size()), &pts[0].x, nbr.data(), deg.data(), spring_params(l));
+        if (its < 0) return THOR_ECUDA;
+        g.spring_iterations += its;
     }
     if (level == 0 && !neighbour_table(int(pts.size()), tris, nbr, deg)) return THOR_EINVAL;
     const int N = int(pts.size());
@@ -437,7 +457,7 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
 
     // --- vertical tables (R6: uniform dz unless interface altitudes are given; Eq. 27's radial operator;
     // Eq. 8-9 with k = 1 for the centre -> interface interpolation)
-    g.dz = P.z_top / nv;
+    g.dz = g.P.z_top / nv;
     g.zh.resize(nv + 1);
     for (int k = 0; k <= nv; ++k) g.zh[k] = z_interfaces ? z_interfaces[k] : k * g.dz;
     g.rinv.resize(nv); g.dlo.resize(nv); g.dhi.resize(nv); g.vol.resize(nv); g.zc.resize(nv);
@@ -458,6 +478,25 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
         g.wl[k] = z_interfaces ? (g.zc[k] - g.zh[k]) / dc : 0.5;
         g.wh[k] = z_interfaces ? (g.zh[k] - g.zc[k - 1]) / dc : 0.5;
         g.idz[k] = 1.0 / dc;
+    }
+    // Eq. 8-9 (L90-L94) at order 3: L_j(zt) = prod_(i != j) (zt - z_i)/(z_j - z_i) over the window of RV1 -- the two
+    // nearest nodes on each side of the target, cut at the ends of the column
+    g.kord = kord;
+    g.ihw.assign(size_t(4) * nv, 0.0);
+    g.icw.assign(size_t(4) * nv, 0.0);
+    auto lagrange = [](const double* z, int n, double zt, int j) {
+        double L = 1.0;
+        for (int i = 0; i < n; ++i)
+            if (i != j) L = L * (zt - z[i]) / (z[j] - z[i]);
+        return L;
+    };
+    for (int k = 1; k < nv; ++k) {                         // centres lo..hi -> interface k
+        const int lo = std::max(k - 2, 0), hi = std::min(k + 1, nv - 1);
+        for (int j = lo; j <= hi; ++j) g.ihw[size_t(j - (k - 2)) * nv + k] = lagrange(&g.zc[lo], hi - lo + 1, g.zh[k], j - lo);
+    }
+    for (int k = 0; k < nv; ++k) {                         // interfaces lo..hi -> centre k
+        const int lo = std::max(k - 1, 0), hi = std::min(k + 2, nv);
+        for (int j = lo; j <= hi; ++j) g.icw[size_t(j - (k - 1)) * nv + k] = lagrange(&g.zh[lo], hi - lo + 1, g.zc[k], j - lo);
     }
     return THOR_OK;
 }

@@ -45,10 +45,26 @@ struct HostGrid {
     std::vector<double> wl, wh;    // [nv] weights of the centres below / above the interface
     std::vector<double> idz;       // [nv] 1/(z_k - z_k-1)
     double dz = 0;                 // z_top / nv (mean thickness)
+    // NEXT-3: Eq. 8-9 of order kord (1 or 3) in the explicit slow terms (RV1, RV2).  kord = 3: Lagrange weights of
+    // the four nearest nodes, 0 for the nodes the column's end cuts off (the order falls by one per missing node)
+    int kord = 1;
+    std::vector<double> ihw;       // [4][nv] centre k-2, k-1, k, k+1 -> lower interface of layer k (0 for k = 0)
+    std::vector<double> icw;       // [4][nv] interface k-1, k, k+1, k+2 -> centre of layer k
 };
 
-// Builds everything above.  Returns THOR_OK or THOR_EINVAL / THOR_ENOMEM.
+// One spring-dynamics relaxation (Eq. 10-12) of the N points xyz [N][3] (in place) on the refinement level whose
+// neighbour table is nbr [N][6] / deg [N]; returns the number of steps taken, < 0 on failure.  The constants of the
+// iteration are passed in so that the host loop (grid_host.cpp) and the device loop (thor_api.cu, NEXT-3) share them.
+struct SpringParams {
+    double dspr, k, alpha, dt, tol;   // Eq. 12 natural length (unit sphere), spring constant, drag, time step, stop test
+    int min_iter, max_iter;
+};
+using SpringFn = int (*)(int N, double* xyz, const int* nbr, const int* deg, const SpringParams& sp);
+
+// Builds everything above.  Returns THOR_OK or THOR_EINVAL / THOR_ENOMEM (THOR_ECUDA from a device `spring`).
+// kord: order of Eq. 8-9 in the explicit slow terms, 1 (the paper's choice, L94) or 3.  spring: nullptr = the host loop.
 // z_interfaces: nullptr (uniform layers, R6) or nv+1 strictly increasing altitudes from 0 to P.z_top.
-int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces = nullptr);
+int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces = nullptr, int kord = 1,
+                    SpringFn spring = nullptr);
 
 }  // namespace thor

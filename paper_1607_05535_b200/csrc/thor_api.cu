@@ -49,7 +49,7 @@ struct DeviceGeom {
     double *wdiv = nullptr, *wgrad = nullptr, *area = nullptr;
     double *frame = nullptr, *wdiv2 = nullptr, *wgrad2 = nullptr, *wlap = nullptr;
     double *rinv = nullptr, *dlo = nullptr, *dhi = nullptr, *vol = nullptr, *zc = nullptr, *rhinv = nullptr;
-    double *wl = nullptr, *wh = nullptr, *idz = nullptr;
+    double *wl = nullptr, *wh = nullptr, *idz = nullptr, *vk = nullptr;
     // tiles of the TMA-staged column-solve kernel (kTmaWarps * 32/G consecutive columns each)
     int tcol = 0, hmax = 0;
     // NEXT-1 divergence damping as ONE stencil: -lap(grad D3) composed on the host over the two rings of a column
@@ -115,7 +115,7 @@ int upload(T** dst, const std::vector<T>& src) {
 void free_device_geom(DeviceGeom& d) {
     cudaFree(d.nbr); cudaFree(d.order); cudaFree(d.wdiv); cudaFree(d.wgrad); cudaFree(d.frame); cudaFree(d.area);
     cudaFree(d.rinv); cudaFree(d.dlo); cudaFree(d.dhi); cudaFree(d.vol); cudaFree(d.zc); cudaFree(d.rhinv);
-    cudaFree(d.wl); cudaFree(d.wh); cudaFree(d.idz);
+    cudaFree(d.wl); cudaFree(d.wh); cudaFree(d.idz); cudaFree(d.vk);
     cudaFree(d.tile_halo); cudaFree(d.tile_slots); cudaFree(d.dd_idx); cudaFree(d.dd_coef);
     cudaFree(d.wdiv2); cudaFree(d.wgrad2); cudaFree(d.wlap); cudaFree(d.op_buf);
     d = DeviceGeom();
@@ -197,6 +197,15 @@ int upload_device_geom(const thor_grid* grid) {
     if ((rc = upload(&d.wl, padded(h.wl)))) return rc;
     if ((rc = upload(&d.wh, padded(h.wh)))) return rc;
     if ((rc = upload(&d.idz, padded(h.idz)))) return rc;
+    {   // NEXT-3: the order-3 weights of Eq. 8-9, [8][kMaxLayers]
+        std::vector<double> vk(size_t(8) * kMaxLayers, 0.0);
+        for (int r = 0; r < 4; ++r)
+            for (int k = 0; k < h.nv; ++k) {
+                vk[size_t(r) * kMaxLayers + k] = h.ihw[size_t(r) * h.nv + k];
+                vk[size_t(4 + r) * kMaxLayers + k] = h.icw[size_t(r) * h.nv + k];
+            }
+        if ((rc = upload(&d.vk, vk))) return rc;
+    }
     {   // composed operator of the divergence damping (RD4): F_i = -K_d P_i lap(grad D3)_i
         //   grad D3 at column c:  G_c = sum_j wgrad_cj (D3_nbr(c,j) - D3_c)
         //   lap of each Cartesian component: sum_c wlap_ic (G_c - G_i), then Eq. 28 at i and its tangent basis
@@ -289,7 +298,7 @@ Geom make_geom(const thor_grid* grid) {
     g.wdiv2 = d.wdiv2; g.wgrad2 = d.wgrad2; g.wlap = d.wlap;
     g.dd_idx = d.dd_idx; g.dd_coef = d.dd_coef;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
-    g.wl = d.wl; g.wh = d.wh; g.idz = d.idz;
+    g.wl = d.wl; g.wh = d.wh; g.idz = d.idz; g.vk = d.vk; g.kord = h.kord;
     g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
@@ -480,23 +489,34 @@ extern "C" {
 const char* thor_last_error(void) { return g_err.c_str(); }
 long long thor_launch_count(void) { return g_launches.load(); }
 
-int thor_grid_create(int level, int n_layers, const thor_planet* planet, thor_grid** out) {
+static int grid_create(int level, int n_layers, const thor_planet* planet, const double* z_interfaces, int order_k,
+                       SpringFn spring, thor_grid** out) {
     if (!planet || !out) return fail(THOR_EINVAL, "thor_grid_create: null argument");
     thor_grid* g = new (std::nothrow) thor_grid();
     if (!g) return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
     int rc;
     try {
-        rc = build_host_grid(level, n_layers, *planet, g->h);
+        rc = build_host_grid(level, n_layers, *planet, g->h, z_interfaces, order_k, spring);
     } catch (const std::bad_alloc&) {
         delete g;
         return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
     }
     if (rc != THOR_OK) {
         delete g;
-        return fail(rc, "thor_grid_create: invalid level, layer count or planet parameters");
+        if (rc == THOR_ECUDA) return rc;                 // the device spring loop has set the message
+        return fail(rc, "thor_grid_create: invalid level, layer count, planet parameters, interface altitudes or order");
     }
     *out = g;
     return THOR_OK;
+}
+
+int thor_grid_create(int level, int n_layers, const thor_planet* planet, thor_grid** out) {
+    return grid_create(level, n_layers, planet, nullptr, 1, nullptr, out);
+}
+
+int thor_grid_create_vertical(int level, int n_layers, const thor_planet* planet, const double* z_interfaces,
+                              int order_k, thor_grid** out) {
+    return grid_create(level, n_layers, planet, z_interfaces, order_k, nullptr, out);
 }
 
 int thor_grid_get(const thor_grid* grid, thor_grid_view* out) {
@@ -613,8 +633,11 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         const int dd = Kd_div > 0.0 ? (stage == 1 ? 2 : 1) : 0;
         THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks), Kd_hyp > 0.0 ? s->X : nullptr);
         if (Kd_hyp > 0.0) {
-            THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
+            if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
+            else THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
             THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks));
+        } else if (g.kord == 3) {
+            THOR_DISPATCH(k_slow_terms_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
         } else {
             THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
         }

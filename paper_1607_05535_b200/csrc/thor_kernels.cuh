@@ -85,6 +85,11 @@ struct Geom {                 // device pointers, device column order, padded to
     const double* wl;         // weight of the centre below:  (z_k - z_h,k)/(z_k - z_k-1)
     const double* wh;         // weight of the centre above:  (z_h,k - z_k-1)/(z_k - z_k-1)
     const double* idz;        // 1/(z_k - z_k-1), the spacing of G_h
+    // NEXT-3 (RV1, RV2): Eq. 8-9 of order 3 in the explicit slow terms, [8][128]: rows 0-3 the weights of the centres
+    // k-2, k-1, k, k+1 at the lower interface of layer k; rows 4-7 those of the interfaces k-1, k, k+1, k+2 at the
+    // centre of layer k (0 for the nodes the column's end cuts off, and on pads); used when kord == 3
+    const double* vk;
+    int kord;
     double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
@@ -218,6 +223,46 @@ __device__ __forceinline__ void above(const double (&v)[E], double (&out)[E], in
 #pragma unroll
     for (int e = 0; e < E - 1; ++e) out[e] = v[e + 1];
     out[E - 1] = next;
+}
+
+// value at layer k-2 / k+2
+template <int G, int E>
+__device__ __forceinline__ void below2(const double (&v)[E], double (&out)[E], int gl, double fill) {
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const double prev = __shfl_up_sync(kFull, v[E - 2 + e], 1, G);
+        out[e] = gl == 0 ? fill : prev;
+    }
+#pragma unroll
+    for (int e = 2; e < E; ++e) out[e] = v[e - 2];
+}
+template <int G, int E>
+__device__ __forceinline__ void above2(const double (&v)[E], double (&out)[E], int gl, double fill) {
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const double next = __shfl_down_sync(kFull, v[e], 1, G);
+        out[E - 2 + e] = gl == G - 1 ? fill : next;
+    }
+#pragma unroll
+    for (int e = 0; e < E - 2; ++e) out[e] = v[e + 2];
+}
+// NEXT-3, Eq. 8-9 of order 3 (RV1): centres -> lower interface of each layer, and interfaces -> centres;
+// w points at the lane's first layer of Geom::vk rows 0-3 (resp. 4-7), row stride 128
+template <int G, int E>
+__device__ __forceinline__ void interp_h3(const double* w, const double (&q)[E], double (&out)[E], int gl) {
+    double b2[E], b1[E], a1[E], w0[E], w1[E], w2[E], w3[E];
+    below2<G, E>(q, b2, gl, 0.0); below<G, E>(q, b1, gl, 0.0); above<G, E>(q, a1, gl, 0.0);
+    ld_nc<E>(w, w0); ld_nc<E>(w + 128, w1); ld_nc<E>(w + 256, w2); ld_nc<E>(w + 384, w3);
+#pragma unroll
+    for (int e = 0; e < E; ++e) out[e] = fma(a1[e], w3[e], fma(q[e], w2[e], fma(b1[e], w1[e], b2[e] * w0[e])));
+}
+template <int G, int E>
+__device__ __forceinline__ void interp_c3(const double* w, const double (&X)[E], double (&out)[E], int gl) {
+    double b1[E], a1[E], a2[E], w0[E], w1[E], w2[E], w3[E];
+    below<G, E>(X, b1, gl, 0.0); above<G, E>(X, a1, gl, 0.0); above2<G, E>(X, a2, gl, 0.0);
+    ld_nc<E>(w, w0); ld_nc<E>(w + 128, w1); ld_nc<E>(w + 256, w2); ld_nc<E>(w + 384, w3);
+#pragma unroll
+    for (int e = 0; e < E; ++e) out[e] = fma(a2[e], w3[e], fma(a1[e], w2[e], fma(X[e], w1[e], b1[e] * w0[e])));
 }
 
 // Eq. 24 (L210) and its inverse
@@ -626,6 +671,7 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
     st_row<E>(me + F_H * NVP, h);      st_row<E>(me + F_TH * NVP, th);
     st_row<E>(me + F_FA * NVP, fa);    st_row<E>(me + F_FI * NVP, fi);   st_row<E>(me + F_FC * NVP, fc);
     if (Xw) {                                                    // NEXT-1: w on interior interfaces (0 elsewhere)
+        if (g.kord == 3) interp_h3<G, E>(g.vk + L.k0, rho, rhoh, L.gl);   // RV2: I_h of the order of the run
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int k = L.k0 + e;
@@ -670,7 +716,7 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 // rho, v = V/rho (Cartesian components), w and T (RD2) and stores them weighted for the second one.
 // dd: 1 = also store D3^[t] = div_h V^[t] + D_c[W^[t]] (RD4); 2 (stage 1, where Phi^[t] = Phi^n) = and D3^n.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E, bool HYP>
+template <int G, int E, bool HYP, bool K3>
 __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restrict__ S, const Tune& tn,
                                                  double* __restrict__ X, int dd) {
     const Walk wk(tn);
@@ -724,7 +770,8 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
         double a[E], b[E], tj[E], pj[E], irj[E], Wj[E], Wup[E];
         ld_nc<E>(q + F_VAT * NVP, a);  ld_nc<E>(q + F_VBT * NVP, b);  ld_nc<E>(q + F_TH * NVP, tj);
         ld_nc<E>(q + F_PT * NVP, pj);  ld_nc<E>(q + F_IRT * NVP, irj); ld_nc<E>(q + F_WT * NVP, Wj);
-        above<G, E>(Wj, Wup, L.gl, 0.0);
+        if (K3) interp_c3<G, E>(g.vk + 512 + L.k0, Wj, Wup, L.gl);           // RV2: Wup holds I_c[W]_j itself
+        else above<G, E>(Wj, Wup, L.gl, 0.0);
         if (j == 0) {
 #pragma unroll
             for (int e = 0; e < E; ++e) p0[e] = pj[e];
@@ -739,7 +786,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const double d = fma(wa, a[e], wb * b[e]);                        // w_j . V_j
-            const double wc = 0.5 * (Wj[e] + Wup[e]);                         // I_c[W]_j; the lid's W is the pad's 0
+            const double wc = K3 ? Wup[e] : 0.5 * (Wj[e] + Wup[e]);           // I_c[W]_j; the lid's W is the pad's 0
             const double t = d * irj[e];
             divV[e] += d;
             divhV[e] = fma(cph * pj[e] * irj[e], d, divhV[e]);                // h_j = Cp p_j/(Rd rho_j)
@@ -785,6 +832,8 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     ld_nc<E>(me + F_RHOT * NVP, rho);
     ld_again<E>(me + F_WT * NVP, W);
     above<G, E>(W, Wup, L.gl, 0.0);
+    double Wc3[K3 ? E : 1];
+    if constexpr (K3) interp_c3<G, E>(g.vk + 512 + L.k0, W, Wc3, L.gl);
     ld_again<E>(me + F_VAT * NVP, a0); ld_again<E>(me + F_VBT * NVP, b0); ld_again<E>(me + F_IRT * NVP, ir0);
     const double* f0 = frm;
     const double e1x = f0[0], e1y = f0[1], e1z = f0[2], e2x = f0[3], e2y = f0[4], e2z = f0[5];
@@ -792,7 +841,8 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     double Mx[E], My[E], Mz[E];                                              // full momentum M = V + I_c[W] r
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-        const double wc = 0.5 * (W[e] + Wup[e]);
+        double wc = 0.5 * (W[e] + Wup[e]);
+        if constexpr (K3) wc = Wc3[e];
         Mx[e] = fma(a0[e], e1x, fma(b0[e], e2x, wc * rx));
         My[e] = fma(a0[e], e1y, fma(b0[e], e2y, wc * ry));
         Mz[e] = fma(a0[e], e1z, fma(b0[e], e2z, wc * rz));
@@ -801,9 +851,15 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     // vertical flux divergences D_c[W I_h[q]] for q = u_x, u_y, u_z, h, theta, and D_c[W]
     double qb[E], Xf[E], Xup[E];
     auto vflux = [&](const double (&q)[E], double (&out)[E]) {
-        below<G, E>(q, qb, L.gl, 0.0);
+        if constexpr (K3) {
+            interp_h3<G, E>(g.vk + L.k0, q, qb, L.gl);
 #pragma unroll
-        for (int e = 0; e < E; ++e) Xf[e] = W[e] * (wl[e] * qb[e] + wh[e] * q[e]);    // W = 0 on the ground and on the lid
+            for (int e = 0; e < E; ++e) Xf[e] = W[e] * qb[e];
+        } else {
+            below<G, E>(q, qb, L.gl, 0.0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) Xf[e] = W[e] * (wl[e] * qb[e] + wh[e] * q[e]);    // W = 0 on the ground and on the lid
+        }
         above<G, E>(Xf, Xup, L.gl, 0.0);
 #pragma unroll
         for (int e = 0; e < E; ++e) out[e] = dhi[e] * Xup[e] - dlo[e] * Xf[e];
@@ -856,12 +912,19 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
         srt[e] = real ? -divtV[e] - DtW[e] : 0.0;
     }
     double Frb[E], sW[E];
-    below<G, E>(Fr, Frb, L.gl, 0.0);
+    if constexpr (K3) {                                      // RV2: I_h[rho] and I_h[F_r] of Eq. 42 at the order of the run
+        interp_h3<G, E>(g.vk + L.k0, rho, rhoh, L.gl);       // (g~ above keeps the acoustic system's linear one)
+        interp_h3<G, E>(g.vk + L.k0, Fr, Frb, L.gl);
+    } else {
+        below<G, E>(Fr, Frb, L.gl, 0.0);
+#pragma unroll
+        for (int e = 0; e < E; ++e) Frb[e] = wl[e] * Frb[e] + wh[e] * Fr[e];
+    }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const int k = L.k0 + e;
         sW[e] = (k >= 1 && k < nv && L.col < g.N)
-                    ? -(p0[e] - pb[e]) * idz[e] - g.gravity * rhoh[e] - (wl[e] * Frb[e] + wh[e] * Fr[e])
+                    ? -(p0[e] - pb[e]) * idz[e] - g.gravity * rhoh[e] - Frb[e]
                     : 0.0;                                                    // Eq. 42
     }
     st_row<E>(me + F_SVA * NVP, sa);    st_row<E>(me + F_SVB * NVP, sb);
@@ -895,12 +958,23 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
 k_slow_terms(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, false>(g, S, tn, X, dd);
+    slow_terms_block<G, E, false, false>(g, S, tn, X, dd);
 }
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
 k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, true>(g, S, tn, X, dd);
+    slow_terms_block<G, E, true, false>(g, S, tn, X, dd);
+}
+// NEXT-3: the same two kernels with Eq. 8-9 of order 3 in the vertical interpolations (RV2)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
+k_slow_terms_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
+    slow_terms_block<G, E, false, true>(g, S, tn, X, dd);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
+k_slow_terms_hyp_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
+    slow_terms_block<G, E, true, true>(g, S, tn, X, dd);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -45,6 +45,23 @@ def test_error_codes_and_messages():
         thor.thor_grid_create(2, 8, dict(ti.EARTH, Cp=100.0))     # Cp <= Rd
 
 
+def test_vertical_grid_arguments():
+    """thor_grid_create_vertical (NEXT-3): interface altitudes must start at 0 and increase strictly; orders 1 and 3."""
+    nv = 6
+    z = ti.stretched_interfaces(ti.EARTH, nv, 3.0)
+    g = thor.Grid(1, nv, ti.EARTH, z_interfaces=z, order_k=3)
+    assert g.n_layers == nv
+    g.close()
+    bad = z.copy()
+    bad[3] = bad[2]
+    for args in ((bad, 1), (z + 1.0, 1), (z, 2), (z, 5), (z, 0)):
+        with pytest.raises(thor.ThorError) as e:
+            thor.Grid(1, nv, ti.EARTH, z_interfaces=args[0], order_k=args[1])
+        assert e.value.code == thor.THOR_EINVAL
+    with pytest.raises(thor.ThorError):
+        thor.Grid(1, nv, ti.EARTH, z_interfaces=z[:-1])            # wrong length is caught by the binding
+
+
 @pytest.mark.skipif(have_cuda(), reason="checks the no-device behaviour")
 def test_device_entry_points_fail_loudly_without_a_gpu():
     g = thor.Grid(1, 4, ti.EARTH)

@@ -432,6 +432,49 @@ def test_held_suarez_benchmark_spins_up_midlatitude_jets():
     g.close()
 
 
+@pytest.mark.parametrize("D", [0.0, 0.004837])
+@pytest.mark.parametrize("nv,order_k,ratio", [(32, 1, 6.0), (32, 3, 6.0), (37, 3, 1.0), (8, 3, 3.0), (70, 3, 4.0), (5, 3, 2.0)])
+def test_next3_stretched_layers_and_order_k(nv, order_k, ratio, D):
+    """NEXT-3 (Eq. 8-9): layers of unequal thickness (geometric stretching, top/bottom = ratio; 1 = uniform
+    altitudes passed explicitly) and the vertical interpolation of order k in the explicit slow terms, against the
+    oracle's orc_geom_set_vertical path, after 1 and 5 large steps, with and without NEXT-1."""
+    level, planet = 3, ti.EARTH
+    z_h = ti.stretched_interfaces(planet, nv, ratio)
+    g = thor.Grid(level, nv, planet, z_interfaces=z_h, order_k=order_k)
+    v = g.view
+    G = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], z_interfaces=z_h, vert_order=order_k)
+    Gf = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], fma=True, z_interfaces=z_h, vert_order=order_k)
+    rng = np.random.default_rng(31 + nv)
+    N = g.n_cols
+    T = 290.0 * (1 + rng.uniform(-1e-2, 1e-2, size=(N, nv)))
+    pcol = ti.hydrostatic_column(planet, z_h, 1.0e5, np.full(nv, 290.0))
+    p = np.tile(pcol, (N, 1))
+    rho = p / (planet["Rd"] * T)
+    u = rng.uniform(-3.0, 3.0, size=(N, nv, 3))
+    u -= np.sum(u * v["xyz"][:, None, :], axis=-1, keepdims=True) * v["xyz"][:, None, :]
+    V = rho[..., None] * u
+    W = np.zeros((N, nv + 1))
+    W[:, 1:nv] = rng.uniform(-0.3, 0.3, size=(N, nv - 1))
+    s = (rho, V, W, p)
+    dt, n = 300.0, 4
+    st = thor.State(g, *s)
+    st.set_diffusion(D, D)
+    Y = Yardstick(G, Gf, s, _base_run(n, dt, None, (D, D)))
+    st.step(1, dt, n)
+    _compare(st.get(), Y.advance(1), TOL_1, "next3 nv=%d k=%d ratio=%g D=%g, 1 step" % (nv, order_k, ratio, D))
+    st.step(4, dt, n)
+    _compare(st.get(), Y.advance(4), TOL_1 * 5, "next3 nv=%d k=%d ratio=%g D=%g, 5 steps" % (nv, order_k, ratio, D))
+    if order_k == 3:                                    # the order does change the answer (far above the tolerance)
+        G1 = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], z_interfaces=z_h, vert_order=1)
+        lin = G1.step(*s, 5, dt, n, None, D, D)
+        assert np.abs(lin[2] - Y.ref[2]).max() > 1e3 * np.abs(st.get()[2] - Y.ref[2]).max()
+    m, _ = st.diagnostics()
+    mr, _ = G.diagnostics(*Y.ref)
+    assert abs(m - mr) <= 1e-13 * mr
+    st.close()
+    g.close()
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""
