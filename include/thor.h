@@ -97,6 +97,13 @@ int thor_grid_create(int level, int n_layers, const thor_planet *planet, thor_gr
  * of the target; where the column ends first the missing nodes are dropped (RV1).  Other orders: THOR_EINVAL. */
 int thor_grid_create_vertical(int level, int n_layers, const thor_planet *planet, const double *z_interfaces,
                               int order_k, thor_grid **out);
+/* NEXT-3 (section 2.3, Eq. 10-12): the same grid with the spring-dynamics relaxation -- by far the slowest
+ * part of set-up from level 6 on -- iterated on the current CUDA device (one kernel launch per step, the same update
+ * and the same stopping test as the host loop; positions agree with thor_grid_create's to rounding accumulated over the
+ * iteration, far inside the stopping tolerance).  Bisection, centroid move, stencil weights and the device column order
+ * stay on the host.  Arguments as thor_grid_create_vertical.  THOR_ECUDA without a usable device. */
+int thor_grid_create_device(int level, int n_layers, const thor_planet *planet, const double *z_interfaces,
+                            int order_k, thor_grid **out);
 int thor_grid_get(const thor_grid *grid, thor_grid_view *out);
 void thor_grid_destroy(thor_grid *grid);
 

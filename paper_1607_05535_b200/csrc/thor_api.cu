@@ -482,6 +482,53 @@ int launch_vertical(const thor_grid* grid, const Geom& g, double* S, double delt
     return THOR_OK;
 }
 
+// NEXT-3: the spring-dynamics relaxation of one refinement level on the current CUDA device (SpringFn of
+// grid_host.h).  Same iteration and the same stopping test as the host loop, checked after every step (one 8-byte
+// read back per step); positions in and out through the host array.
+int spring_dynamics_device(int N, double* xyz, const int* nbr, const int* deg, const SpringParams& sp) {
+    double *x = nullptr, *xn = nullptr, *v = nullptr;
+    int *dn = nullptr, *dd = nullptr;
+    unsigned long long* worst = nullptr;
+    const size_t b3 = size_t(N) * 3 * sizeof(double);
+    auto cleanup = [&]() { cudaFree(x); cudaFree(xn); cudaFree(v); cudaFree(dn); cudaFree(dd); cudaFree(worst); };
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&x), b3);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&xn), b3);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&v), b3);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&dn), size_t(N) * 6 * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&dd), size_t(N) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&worst), sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemcpy(x, xyz, b3, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(v, 0, b3);
+    if (e == cudaSuccess) e = cudaMemcpy(dn, nbr, size_t(N) * 6 * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dd, deg, size_t(N) * sizeof(int), cudaMemcpyHostToDevice);
+    int it = 0;
+    for (; e == cudaSuccess && it < sp.max_iter; ++it) {
+        e = cudaMemsetAsync(worst, 0, sizeof(unsigned long long), nullptr);
+        if (e != cudaSuccess) break;
+        k_spring_step<<<(N + 127) / 128, 128>>>(N, x, xn, v, dn, dd, sp.dspr, sp.k, sp.alpha, sp.dt, worst);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        std::swap(x, xn);
+        if (it >= sp.min_iter) {
+            unsigned long long bits = 0;
+            e = cudaMemcpy(&bits, worst, sizeof(bits), cudaMemcpyDeviceToHost);
+            double w;
+            std::memcpy(&w, &bits, sizeof(w));
+            if (e == cudaSuccess && w < sp.tol) {
+                ++it;
+                break;
+            }
+        }
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpy(xyz, x, b3, cudaMemcpyDeviceToHost);
+    cleanup();
+    if (e != cudaSuccess) {
+        fail(THOR_ECUDA, std::string("thor_grid_create_device: spring dynamics: ") + cudaGetErrorString(e));
+        return -1;
+    }
+    return it;
+}
+
 }  // namespace
 
 extern "C" {
@@ -517,6 +564,14 @@ int thor_grid_create(int level, int n_layers, const thor_planet* planet, thor_gr
 int thor_grid_create_vertical(int level, int n_layers, const thor_planet* planet, const double* z_interfaces,
                               int order_k, thor_grid** out) {
     return grid_create(level, n_layers, planet, z_interfaces, order_k, nullptr, out);
+}
+
+int thor_grid_create_device(int level, int n_layers, const thor_planet* planet, const double* z_interfaces,
+                            int order_k, thor_grid** out) {
+    int n = 0;
+    const cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) return fail(THOR_ECUDA, std::string("thor_grid_create_device: no CUDA device: ") + cudaGetErrorString(e));
+    return grid_create(level, n_layers, planet, z_interfaces, order_k, spring_dynamics_device, out);
 }
 
 int thor_grid_get(const thor_grid* grid, thor_grid_view* out) {

@@ -1598,6 +1598,53 @@ k_diag(Geom g, const double* __restrict__ S, double* __restrict__ col_mass, doub
 }
 
 // ---------------------------------------------------------------------------------------------
+// NEXT-3: one step of the spring dynamics of the grid generator (Eq. 10-12) for all points at once
+// (Jacobi: new positions from the old ones), one thread per point.  x, xn: [N][3] unit vectors; v: [N][3] velocities
+// (tangent); the twelve pentagon centres stay fixed (L109).  worst: the largest displacement of the step as the bit
+// pattern of a non-negative double (atomicMax on the integer order, which is the same).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_spring_step(int N, const double* __restrict__ x, double* __restrict__ xn, double* __restrict__ v,
+              const int* __restrict__ nbr, const int* __restrict__ deg, double dspr, double kspr, double alpha, double dt,
+              unsigned long long* __restrict__ worst) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double moved = 0.0;
+    if (i < N) {
+        const double px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2];
+        if (deg[i] == 5) {
+            xn[3 * i] = px; xn[3 * i + 1] = py; xn[3 * i + 2] = pz;
+        } else {
+            double fx = 0.0, fy = 0.0, fz = 0.0;
+            for (int k = 0; k < 6; ++k) {
+                const int j = nbr[size_t(i) * 6 + k];
+                const double qx = x[3 * j], qy = x[3 * j + 1], qz = x[3 * j + 2];
+                const double cx = py * qz - pz * qy, cy = pz * qx - px * qz, cz = px * qy - py * qx;
+                const double dt0 = qx * px + qy * py + qz * pz;
+                const double d = atan2(sqrt(cx * cx + cy * cy + cz * cz), dt0);             // geodesic distance
+                double ex = qx - dt0 * px, ey = qy - dt0 * py, ez = qz - dt0 * pz;           // tangent at P_0 towards P_j
+                const double inv = 1.0 / sqrt(ex * ex + ey * ey + ez * ez);
+                const double a = kspr * (d - dspr) * inv;
+                fx += a * ex; fy += a * ey; fz += a * ez;
+            }
+            double vx = v[3 * i], vy = v[3 * i + 1], vz = v[3 * i + 2];
+            fx -= alpha * vx; fy -= alpha * vy; fz -= alpha * vz;                           // Eq. 10
+            vx += dt * fx; vy += dt * fy; vz += dt * fz;
+            double nx = px + dt * vx, ny = py + dt * vy, nz = pz + dt * vz;                  // Eq. 11, back onto the sphere
+            const double in = 1.0 / sqrt(nx * nx + ny * ny + nz * nz);
+            nx *= in; ny *= in; nz *= in;
+            const double vr = vx * nx + vy * ny + vz * nz;
+            v[3 * i] = vx - vr * nx; v[3 * i + 1] = vy - vr * ny; v[3 * i + 2] = vz - vr * nz;
+            xn[3 * i] = nx; xn[3 * i + 1] = ny; xn[3 * i + 2] = nz;
+            const double mx = nx - px, my = ny - py, mz = nz - pz;
+            moved = sqrt(mx * mx + my * my + mz * mz);
+        }
+    }
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) moved = fmax(moved, __shfl_xor_sync(kFull, moved, s));
+    if ((threadIdx.x & 31) == 0 && moved > 0.0) atomicMax(worst, static_cast<unsigned long long>(__double_as_longlong(moved)));
+}
+
+// ---------------------------------------------------------------------------------------------
 // Canonical (host order, as uploaded) <-> device rows.  One thread per (device column, layer).
 //   rows:   dst[d*dst_col + k] for d < Npad, k < NVP  (a record row: dst_col = NF*NVP; a table: NVP)
 //   canon:  src[order[d]*row_len + k*cs + c0]         (real columns and layers only; pads get `pad`)

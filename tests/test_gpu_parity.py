@@ -475,6 +475,40 @@ def test_next3_stretched_layers_and_order_k(nv, order_k, ratio, D):
     g.close()
 
 
+@pytest.mark.parametrize("level", [3, 5, 6])
+def test_next3_spring_dynamics_on_the_device(level):
+    """NEXT-3: thor_grid_create_device iterates Eq. 10-12 on the GPU.  Same update, same stopping test: the points agree
+    with the host generator's far inside the stopping tolerance (1e-9 per step), the step counts agree, the exported
+    geometry agrees, and the oracle's own generator (pin P3) agrees with it as it does with the host grid."""
+    import time
+    t0 = time.perf_counter()
+    gh = thor.Grid(level, 8, ti.EARTH)
+    t1 = time.perf_counter()
+    gd = thor.Grid(level, 8, ti.EARTH, on_device=True)
+    t2 = time.perf_counter()
+    vh, vd = gh.view, gd.view
+    _report("spring dynamics level %d: host %.2f s (%d steps), device %.2f s (%d steps), max |dP| %.2e" % (
+        level, t1 - t0, vh["spring_iterations"], t2 - t1, vd["spring_iterations"], np.abs(vh["xyz"] - vd["xyz"]).max()))
+    assert np.array_equal(vh["nbr"], vd["nbr"]) and np.array_equal(vh["device_order"], vd["device_order"])
+    assert np.abs(vh["xyz"] - vd["xyz"]).max() < 1e-8
+    assert abs(vh["spring_iterations"] - vd["spring_iterations"]) <= 0.02 * vh["spring_iterations"] + 2
+    assert np.abs(vh["area"] - vd["area"]).max() < 1e-8 * vh["area"].max()
+    assert abs(vd["area"].sum() - 4 * np.pi) < 1e-11
+    assert np.abs(np.linalg.norm(vd["xyz"], axis=1) - 1).max() < 1e-14
+    if level <= 5:                                     # a step on the device-made grid against the oracle on the same grid
+        nv = 8
+        G = oracle.Geometry(vd["xyz"], vd["nbr"], nv, ti.EARTH, vd["cv_vertex"])
+        Gf = oracle.Geometry(vd["xyz"], vd["nbr"], nv, ti.EARTH, vd["cv_vertex"], fma=True)
+        s = _random_state(G, ti.EARTH, 5)
+        st = thor.State(gd, *s)
+        st.step(1, 600.0, 4)
+        Y = Yardstick(G, Gf, s, _base_run(4, 600.0)).advance(1)
+        _compare(st.get(), Y, TOL_1, "device-made grid level %d, 1 step" % level)
+        st.close()
+    gh.close()
+    gd.close()
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""
