@@ -24,7 +24,20 @@
 namespace thor {
 
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int kWarpsPerBlock = 4;
+// measurement knobs (compile time; the defaults are the measured best, profiles/r02*_variants.md)
+#ifndef THOR_WPB
+#define THOR_WPB 4
+#endif
+#ifndef THOR_K2_MINB
+#define THOR_K2_MINB 1
+#endif
+#ifndef THOR_KS_MINB
+#define THOR_KS_MINB 4
+#endif
+#ifndef THOR_KP_MINB
+#define THOR_KP_MINB 1
+#endif
+constexpr int kWarpsPerBlock = THOR_WPB;
 constexpr int kColPad = 64;      // columns are padded to a multiple of this (>= columns per block of any shape)
 constexpr int kEosTerms = 11;    // degree of the binomial series of Eq. 36 in deviation form
 constexpr double kEosSmall = 0.03125;   // |x| <= 2^-5: series; beyond: expm1/log1p
@@ -536,7 +549,7 @@ k_lap2(Geom g, const double* __restrict__ s, double* __restrict__ out) {
 // (Geom::wl, wh, idz).  Xw != null (NEXT-1 hyper-diffusion on): also w = W/I_h[rho] for its Laplacian.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, THOR_KP_MINB)
 k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn, double* __restrict__ Xw) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
@@ -956,7 +969,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     }
 }
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 4)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, THOR_KS_MINB)
 k_slow_terms(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
     slow_terms_block<G, E, false, false>(g, S, tn, X, dd);
 }
@@ -1239,7 +1252,7 @@ __device__ __forceinline__ void vertical_block(const Geom& g, double* __restrict
         vertical_column<G, E>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first);
 }
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, THOR_K2_MINB)
 k_vertical(Geom g, double* __restrict__ S, double delta, int first, Tune tn) {
     vertical_block<G, E, false>(g, S, delta, first, tn, nullptr);
 }
