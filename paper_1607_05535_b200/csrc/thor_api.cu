@@ -371,7 +371,7 @@ bool op_fast_path(int nv, std::initializer_list<const void*> ptrs) {
 // measurement.  Read at the top of every thor_step / thor_acoustic_substeps call (never inside a graph capture).
 struct TunePair { Tune k1, k2, ks; int zigzag, tma_stages, tma_ctas, graph; };
 TunePair tune() {
-    int v[8] = {1, 0, 148, 148, 0, 4, 148, 1};
+    int v[8] = {1, 148, 148, 148, 0, 4, 148, 1};
     if (const char* e = std::getenv("THOR_B200_TUNE"))
         std::sscanf(e, "%d,%d,%d,%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4], &v[5], &v[6], &v[7]);
     TunePair p;
