@@ -687,14 +687,18 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         // (RD2) and D3^[t] (RD4), so that the only extra launch per stage is the second Laplacian
         const int dd = Kd_div > 0.0 ? (stage == 1 ? 2 : 1) : 0;
         THOR_DISPATCH(k_stage_prepare, nv, Npad, st, g, S, stage, delta, dir(tn.ks), Kd_hyp > 0.0 ? s->X : nullptr);
+        // stage 1 without divergence damping: its explicit horizontal step V*' = delta slowV (Phi*(0) = 0) is written
+        // by the kernel that holds the finished slow term (k_slow_terms, or k_diff2 with the hyper-diffusion on)
+        const bool fuse1 = stage == 1 && !(Kd_div > 0.0);
+        const double d1s = (fuse1 && !(Kd_hyp > 0.0)) ? delta : 0.0, d1d = (fuse1 && Kd_hyp > 0.0) ? delta : 0.0;
         if (Kd_hyp > 0.0) {
-            if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
-            else THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
-            THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks));
+            if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
+            else THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
+            THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks), d1d);
         } else if (g.kord == 3) {
-            THOR_DISPATCH(k_slow_terms_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
+            THOR_DISPATCH(k_slow_terms_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);
         } else {
-            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks), s->X, dd);
+            THOR_DISPATCH(k_slow_terms, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);
         }
         for (int sub = 0; sub < ns; ++sub) {
             // stage 1: Phi*(0) = 0 exactly (Eq. 31 with Phi^[t] = Phi^n), so its substep reads no deviation row
@@ -702,7 +706,7 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
                 if (stage == 1) THOR_DISPATCH(k_momentum_dd_stage1, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, int(X_D3N));
                 else THOR_DISPATCH(k_momentum_dd, nv, Npad, st, g, S, delta, dir(tn.k1), s->X, Kd_div, sub == 0 ? int(X_D3N) : int(X_D3));
             } else if (stage == 1) {
-                THOR_DISPATCH(k_momentum_stage1, nv, Npad, st, g, S, delta, dir(tn.k1));
+                // done by k_slow_terms / k_diff2 above
             } else {
                 THOR_DISPATCH(k_momentum, nv, Npad, st, g, S, delta, dir(tn.k1));
             }

@@ -768,7 +768,8 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
     // Eq. 31: Phi*(0) = Phi^n - Phi^[t]; (rho theta)*(0) = (rho theta)^n - (rho theta)^[t]
     if (stage == 1) {
         // Phi*(0) = 0 exactly: the six deviation rows are neither written here nor read by the stage's single
-        // substep (k_momentum_stage1, k_vertical with first = 2), which overwrites all of them
+        // substep (V*' = delta slowV written by k_slow_terms / k_diff2 / k_momentum_dd_stage1; k_vertical with first = 2),
+        // which overwrites all of them
         st_row<E>(me + F_RTN * NVP, rtt);
     } else {
         auto dev = [&](int fn, int fs, const double (&t)[E]) {
@@ -800,10 +801,12 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 // HYP (NEXT-1 hyper-diffusion on, X != null): the same loop also forms the first Laplacians of
 // rho, v = V/rho (Cartesian components), w and T (RD2) and stores them weighted for the second one.
 // dd: 1 = also store D3^[t] = div_h V^[t] + D_c[W^[t]] (RD4); 2 (stage 1, where Phi^[t] = Phi^n) = and D3^n.
+// delta1 > 0 (stage 1 of the base path): also the stage's explicit horizontal step, which with V*(0) = 0 and
+// p*(0) = 0 is V*' = delta1 slowV (Eq. 33) -- the slow term is in registers here, so no k_momentum launch.
 // ---------------------------------------------------------------------------------------------
 template <int G, int E, bool HYP, bool K3>
 __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restrict__ S, const Tune& tn,
-                                                 double* __restrict__ X, int dd) {
+                                                 double* __restrict__ X, int dd, double delta1) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -1033,6 +1036,11 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
                     : 0.0;                                                    // Eq. 42
     }
     st_row<E>(me + F_SVA * NVP, sa);    st_row<E>(me + F_SVB * NVP, sb);
+    if (delta1 > 0.0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) { sa[e] *= delta1; sb[e] *= delta1; }
+        st_row<E>(me + F_VAS * NVP, sa); st_row<E>(me + F_VBS * NVP, sb);
+    }
     st_row<E>(me + F_SRHO * NVP, srho); st_row<E>(me + F_SW * NVP, sW); st_row<E>(me + F_SP * NVP, sp);
     st_row<E>(me + F_SRT * NVP, srt);
     if (dd) {                                                                 // NEXT-1 divergence damping (RD4)
@@ -1062,24 +1070,24 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
 }
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, THOR_KS_MINB)
-k_slow_terms(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, false, false>(g, S, tn, X, dd);
+k_slow_terms(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, false, false>(g, S, tn, X, dd, delta1);
 }
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
-k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, true, false>(g, S, tn, X, dd);
+k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, true, false>(g, S, tn, X, dd, delta1);
 }
 // NEXT-3: the same two kernels with Eq. 8-9 of order 3 in the vertical interpolations (RV2)
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
-k_slow_terms_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, false, true>(g, S, tn, X, dd);
+k_slow_terms_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, false, true>(g, S, tn, X, dd, delta1);
 }
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
-k_slow_terms_hyp_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd) {
-    slow_terms_block<G, E, true, true>(g, S, tn, X, dd);
+k_slow_terms_hyp_k3(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, true, true>(g, S, tn, X, dd, delta1);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1183,11 +1191,6 @@ template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
     momentum_block<G, E, false>(g, S, delta, tn, nullptr, 0.0, 0);
-}
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_momentum_stage1(Geom g, double* __restrict__ S, double delta, Tune tn) {
-    momentum_block<G, E, false, true>(g, S, delta, tn, nullptr, 0.0, 0);
 }
 // the same kernel with NEXT-1's divergence damping added to Eq. 33; d3row: the X row that holds the 3-D
 // divergence of the current momentum (X_D3N in the first substep of a stage, where V^[t] + V*(0) = V^n; X_D3 after)
@@ -1635,10 +1638,10 @@ __device__ __forceinline__ void ld_lap_weights(const Geom& g, int col, int (&nb)
     w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x; w[5] = c.y;
 }
 
-// second Laplacian; the fluxes are added to the slow terms of the stage (RD2, RD3)
+// second Laplacian; the fluxes are added to the slow terms of the stage (RD2, RD3); delta1: as in k_slow_terms
 template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd, Tune tn) {
+k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd, Tune tn, double delta1) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
@@ -1681,6 +1684,11 @@ k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd,
         sb[e] = real(e) ? sb[e] + (fx * fr.e2.x + fy * fr.e2.y + fz * fr.e2.z) : 0.0;
     }
     st_row<E>(me + F_SVA * NVP, sa); st_row<E>(me + F_SVB * NVP, sb);
+    if (delta1 > 0.0) {                              // stage 1 without divergence damping: V*' = delta1 slowV (see k_slow_terms)
+#pragma unroll
+        for (int e = 0; e < E; ++e) { sa[e] *= delta1; sb[e] *= delta1; }
+        st_row<E>(me + F_VAS * NVP, sa); st_row<E>(me + F_VBS * NVP, sb);
+    }
     // vertical momentum on interior interfaces
     lap_gather<G, E>(X + X_Q4 * NVP, XREC, nb, w, L.col, L.k0, q);
     ld_rw<E>(me + F_SW * NVP, t);
