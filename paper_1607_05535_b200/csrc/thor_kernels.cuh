@@ -37,18 +37,9 @@ constexpr unsigned kFull = 0xffffffffu;
 #ifndef THOR_KP_MINB
 #define THOR_KP_MINB 5
 #endif
-#ifndef THOR_NOSMEM
-#define THOR_NOSMEM 0     // bit 0: k_vertical, bit 1: k_momentum, bit 2: k_slow_terms read their stencil weights straight
-#endif                    // from global memory (L1 hits after the first touch) instead of staging them in shared memory
-#ifndef THOR_PFL1
-#define THOR_PFL1 0       // bit 0: k_vertical, bit 1: k_stage_prepare issue prefetch.global.L1 for the rows they read late
-#endif
 #ifndef THOR_GEOMPF
 #define THOR_GEOMPF 1     // 1: the look-ahead also prefetches the stencil data (neighbour slots, weights) of the block ahead
 #endif
-#ifndef THOR_EVL
-#define THOR_EVL 0        // 1: stencil data (neighbour slots, weights, frames) is loaded with the L2 evict_last policy, so
-#endif                    // that the slab streaming through the 126 MB L2 does not push it out between launches
 constexpr int kWarpsPerBlock = THOR_WPB;
 constexpr int kColPad = 64;      // columns are padded to a multiple of this (>= columns per block of any shape)
 constexpr int kEosTerms = 11;    // degree of the binomial series of Eq. 36 in deviation form
@@ -157,14 +148,6 @@ struct Walk {
 __device__ __forceinline__ void bulk_prefetch_l2(const void* p, unsigned bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
-// L1 prefetch of rows [f0, f0 + nf) of the lane group's own column (one lane per 128-byte line issues): the later
-// loads of those rows become L1 hits, without holding registers across the code in between
-template <int G, int E>
-__device__ __forceinline__ void prefetch_own_rows_l1(const double* me, int gl, int f0, int nf) {
-    constexpr int NVP = G * E, LPL = 16 / E;          // lanes per 128-byte line
-    if ((gl % LPL) == 0)
-        for (int f = f0; f < f0 + nf; ++f) asm volatile("prefetch.global.L1 [%0];" ::"l"(me + f * NVP));
-}
 // rows [f0, f0 + nf) of every column of block `bid`, issued by the first warp of the calling block
 template <int G, int E>
 __device__ __forceinline__ void prefetch_block_rows(const double* S, int bid, int f0, int nf) {
@@ -214,31 +197,6 @@ struct Map {
     }
 };
 
-// loads of per-column stencil data (small arrays every step kernel re-reads)
-__device__ __forceinline__ int4 ldg_geom(const int4* p) {
-#if THOR_EVL
-    unsigned long long pol;
-    int4 r;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    asm volatile("ld.global.nc.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
-    return r;
-#else
-    return __ldg(p);
-#endif
-}
-__device__ __forceinline__ double2 ldg_geom(const double2* p) {
-#if THOR_EVL
-    unsigned long long pol;
-    double2 r;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
-    return r;
-#else
-    return __ldg(p);
-#endif
-}
-
 template <int E>
 __device__ __forceinline__ void ld_nc(const double* p, double (&v)[E]) {     // rows nobody writes in this kernel
 #pragma unroll
@@ -272,7 +230,7 @@ __device__ __forceinline__ void st_row(double* p, const double (&v)[E]) {
 struct Frame { double3 e1, e2, r; };
 __device__ __forceinline__ Frame ld_frame(const double* frame, int col) {   // [Npad][12]
     const double2* p = reinterpret_cast<const double2*>(frame) + 6 * size_t(col);
-    const double2 a = ldg_geom(p), b = ldg_geom(p + 1), c = ldg_geom(p + 2), d = ldg_geom(p + 3), e = ldg_geom(p + 4);
+    const double2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2), d = __ldg(p + 3), e = __ldg(p + 4);
     return Frame{make_double3(a.x, a.y, b.x), make_double3(b.y, c.x, c.y), make_double3(d.x, d.y, e.x)};
 }
 
@@ -282,7 +240,7 @@ __device__ __forceinline__ Frame ld_frame(const double* frame, int col) {   // [
 template <int G>
 __device__ __forceinline__ void stage_weights(const double* src, double* dst, int n2, int gl) {
     for (int i = gl; i < n2; i += G)
-        reinterpret_cast<double2*>(dst)[i] = ldg_geom(reinterpret_cast<const double2*>(src) + i);
+        reinterpret_cast<double2*>(dst)[i] = __ldg(reinterpret_cast<const double2*>(src) + i);
 }
 
 // value at layer k-1 (fill below the ground)
@@ -633,9 +591,6 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
     double* me = S + size_t(L.col) * Map<G, E>::REC + L.k0;
     const int nv = g.nv;
     const double gam = g.Cp / (g.Cp - g.Rd), kv = g.Rd / (g.Cp - g.Rd);
-#if THOR_PFL1 & 2
-    if (stage > 1) prefetch_own_rows_l1<G, E>(me, L.gl, F_RHON, 7);
-#endif
     bool real[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) real[e] = (L.k0 + e < nv) && (L.col < g.N);
@@ -826,16 +781,6 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     const double kv = g.Rd / (g.Cp - g.Rd), cph = g.Cp / g.Rd;
     // per column group: 14 divergence weights (+2 pad), 12 gradient weights, the frames of the column and its
     // 6 neighbours (7 x 12), 6 Laplacian weights (+2 pad), 8 neighbour slots
-#if THOR_NOSMEM & 4
-    (void)CPB;
-    const double* wdv = g.wdiv2 + size_t(L.col) * 16;
-    const double* wgv = g.wgrad2 + size_t(L.col) * 12;
-    const double* wlp = g.wlap + size_t(L.col) * 8;
-    const int4 n03 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[7] = {L.col, n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    const double* frm = g.frame + size_t(L.col) * 12;
-#else
     __shared__ double wsm[CPB][16 + 12 + 84 + 8];
     __shared__ int nsm[CPB][8];
     double* wdv = wsm[threadIdx.x / G];
@@ -849,10 +794,9 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     for (int i = L.gl; i < 8; i += G) nbs[i] = i == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 8 + i - 1);
     __syncwarp();
     for (int i = L.gl; i < 42; i += G)
-        reinterpret_cast<double2*>(frm)[i] = ldg_geom(reinterpret_cast<const double2*>(g.frame) + 6 * size_t(nbs[i / 6]) + i % 6);
+        reinterpret_cast<double2*>(frm)[i] = __ldg(reinterpret_cast<const double2*>(g.frame) + 6 * size_t(nbs[i / 6]) + i % 6);
     const int nb[7] = {nbs[0], nbs[1], nbs[2], nbs[3], nbs[4], nbs[5], nbs[6]};
     __syncwarp();
-#endif
 
     double p0[E];
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], ga[E], gb[E];
@@ -870,11 +814,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     for (int j = 0; j < 7; ++j) {
         const double* q = S + size_t(nb[j]) * REC + L.k0;
         const double wa = wdv[2 * j], wb = wdv[2 * j + 1];
-#if THOR_NOSMEM & 4
-        const double* f = g.frame + size_t(nb[j]) * 12;
-#else
         const double* f = frm + 12 * j;
-#endif
         double a[E], b[E], tj[E], pj[E], irj[E], Wj[E], Wup[E];
         ld_nc<E>(q + F_VAT * NVP, a);  ld_nc<E>(q + F_VBT * NVP, b);  ld_nc<E>(q + F_TH * NVP, tj);
         ld_nc<E>(q + F_PT * NVP, pj);  ld_nc<E>(q + F_IRT * NVP, irj); ld_nc<E>(q + F_WT * NVP, Wj);
@@ -1119,19 +1059,13 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
-#if THOR_NOSMEM & 2
-    const double* wgv = g.wgrad2 + size_t(L.col) * 12;
-#else
     __shared__ double wsm[kWarpsPerBlock * 32 / G][12];
     double* wgv = wsm[threadIdx.x / G];
     stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, wgv, 6, L.gl);
-#endif
-    const int4 n03 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-#if !(THOR_NOSMEM & 2)
     __syncwarp();
-#endif
     double ga[E], gb[E], ri[E], va[E], vb[E], sa[E], sb[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) ga[e] = gb[e] = va[e] = vb[e] = 0.0;
@@ -1348,25 +1282,16 @@ __device__ __forceinline__ void vertical_block(const Geom& g, double* __restrict
 #endif
     }
     if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_SVA, 2);               // the next momentum kernel starts here
-#if THOR_NOSMEM & 1
-    const double* wdv = g.wdiv2 + size_t(L.col) * 16;
-#else
     __shared__ double wsm[kWarpsPerBlock * 32 / G][16];
     double* wdv = wsm[threadIdx.x / G];
     stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
-#endif
-    const int4 n03 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = ldg_geom(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     constexpr size_t REC = Map<G, E>::REC;
     const double* const nbp[6] = {S + size_t(n03.x) * REC + L.k0, S + size_t(n03.y) * REC + L.k0, S + size_t(n03.z) * REC + L.k0,
                                   S + size_t(n03.w) * REC + L.k0, S + size_t(n47.x) * REC + L.k0, S + size_t(n47.y) * REC + L.k0};
-#if !(THOR_NOSMEM & 1)
     __syncwarp();
-#endif
     double* me = S + size_t(L.col) * REC + L.k0;
-#if THOR_PFL1 & 1
-    prefetch_own_rows_l1<G, E>(me, L.gl, first == 2 ? int(F_SRHO) : int(F_RHOS), F_PT + 1 - (first == 2 ? int(F_SRHO) : int(F_RHOS)));
-#endif
     if constexpr (DD)
         vertical_column<G, E, true>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first, Xdd + size_t(L.col) * (size_t(XF) * Map<G, E>::NVP) + L.k0);
     else
