@@ -383,6 +383,44 @@ def test_next2_hot_jupiter_forcing_parity():
     assert np.abs(Y.ref[3] - base[3]).max() > 1e4 * np.abs(st.get()[3] - Y.ref[3]).max()
 
 
+@pytest.mark.parametrize("case", ["held_suarez", "hot_jupiter"])
+def test_next2_paper_setups_parity_50_steps(case):
+    """NEXT-2 at the paper's own resolution and set-up (level 5 x 37 layers, L452-L454 / L529): 50 large steps of the
+    benchmark run, element by element against the oracle.  Earth: dt = 1000 s, D = 0.004837, the equatorial T_eq column
+    in hydrostatic balance (+ 1e-3 K of seeded noise so that the comparison is not one of exact symmetries);
+    hot Jupiter: dt = 600 s, D = 0.01992, isothermal 1600 K."""
+    level, nv, n = 5, 37, 6
+    rng = np.random.default_rng(77)
+    if case == "held_suarez":
+        planet, dt, D = dict(ti.EARTH, z_top=32.0e3), 1000.0, 0.004837
+        g, G, Gf = _setup(level, nv, planet)
+        _, _, z_h = ti.vertical_grid(planet, nv)
+        pcol, Tcol = ti.benchmark_column(planet, z_h, 1.0e5, ti.held_suarez_equator_profile(planet, ti.HELD_SUAREZ))
+        p = np.tile(pcol, (G.N, 1))
+        rho = p / (planet["Rd"] * (np.tile(Tcol, (G.N, 1)) + rng.uniform(-1e-3, 1e-3, size=p.shape)))
+        run = lambda geo, x, k: geo.step_held_suarez(*x, k, dt, n, ti.HELD_SUAREZ, D, D)
+    else:
+        planet, dt, D = dict(ti.PAPER_HOT_JUPITER), 600.0, 0.01992
+        g, G, Gf = _setup(level, nv, planet)
+        rho, _, _, p = ti.rest_state(planet, nv, G.N, 1.0e5, 1600.0)
+        rho = p / (planet["Rd"] * (1600.0 + rng.uniform(-1e-3, 1e-3, size=p.shape)))
+        run = lambda geo, x, k: geo.step_hot_jupiter(*x, k, dt, n, ti.HOT_JUPITER_FORCING, D, D)
+    s = (rho, np.zeros((G.N, nv, 3)), np.zeros((G.N, nv + 1)), p)
+    st = thor.State(g, *s)
+    st.set_diffusion(D)
+    if case == "held_suarez":
+        st.set_held_suarez(ti.HELD_SUAREZ)
+    else:
+        st.set_hot_jupiter(ti.HOT_JUPITER_FORCING)
+    st.step(50, dt, n)
+    Y = Yardstick(G, Gf, s, run, seeds=SEEDS[:1]).advance(50)
+    _compare(st.get(), Y, TOL_100, "%s paper set-up level 5 x 37, 50 steps" % case)
+    m, _ = st.diagnostics()
+    mr, _ = G.diagnostics(*Y.ref)
+    assert abs(m - mr) <= 1e-13 * mr
+    st.close()
+
+
 def test_held_suarez_benchmark_spins_up_midlatitude_jets():
     """End to end (base path + NEXT-1 + NEXT-2): the paper's Earth benchmark as section 7.1 states it (L452-L454:
     level 5, 37 layers from 0 to 32 km, dt = 1000 s, D from Table 1, at rest with the equatorial T_eq profile in
