@@ -113,6 +113,7 @@ def _declare(L):
     L.orc_step_hot_jupiter.argtypes = [ctypes.c_void_p, _D, _D, _D, _D, ctypes.c_int, ctypes.c_double, ctypes.c_int, _D,
                                        ctypes.c_double, ctypes.c_double]
     L.orc_forcing_hot_jupiter.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D]
+    L.orc_set_energy_fixer.argtypes = [ctypes.c_int]
     L.orc_num_threads.restype = ctypes.c_int
     L.orc_set_num_threads.argtypes = [ctypes.c_int]
     return L
@@ -210,10 +211,16 @@ class Geometry:
         self._L.orc_hlap(self._h, _p(s), _p(out))
         return out
 
-    def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None, D_hyp=0.0, D_div=0.0):
+    def step(self, rho, V, W, p, n_large, dt, n_sub, forcing=None, D_hyp=0.0, D_div=0.0, energy_fixer=False):
         """n_large large steps; returns new (rho, V, W, p); inputs are not modified.  D_hyp, D_div:
         non-dimensional diffusion parameter of Eq. 49 for the hyper-diffusion / divergence damping
-        (NEXT-1; 0 = off = the base path)."""
+        (NEXT-1; 0 = off = the base path).  energy_fixer: NEXT-4, reading RE1 (L215)."""
+        if energy_fixer:
+            self._L.orc_set_energy_fixer(1)
+            try:
+                return self.step(rho, V, W, p, n_large, dt, n_sub, forcing, D_hyp, D_div)
+            finally:
+                self._L.orc_set_energy_fixer(0)
         rho, V, W, p = (_c(x).copy() for x in (rho, V, W, p))
         assert rho.shape == (self.N, self.nv) and V.shape == (self.N, self.nv, 3)
         assert W.shape == (self.N, self.nv + 1) and p.shape == (self.N, self.nv)

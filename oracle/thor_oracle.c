@@ -988,6 +988,15 @@ double orc_kd(double D, double dbar, double dt);
 /* D_hyp, D_div: the non-dimensional diffusion parameter of Eq. 49 for the hyper-diffusion and for the
  * divergence damping (the paper uses the same value for both, L367); 0 switches a term off, and
  * (0, 0) is the base path of SURVEY 8(a), arithmetic untouched. */
+/* NEXT-4, energy fixer (L215: "a scheme proposed by Williamson et al. (2009), which globally uniform adjusts the
+ * internal energy at all grid points"; the paper's own runs leave it off).  Reading RE1: after the
+ * dynamics of a large step and before its forcing, the total energy E' (orc_diagnostics, R10) is brought back to its
+ * value E before the step by ONE temperature increment for all cells, dT = (E - E')/(Cv M) with M the total mass:
+ * rho unchanged, p <- p + rho Rd dT, which adds Cv dT M = E - E' of internal energy.  Off by default. */
+static int g_efix = 0;
+void orc_set_energy_fixer(int on) { g_efix = on; }
+void orc_diagnostics(const orc_geom *G, const double *rho, const double *V, const double *W, const double *p,
+                     double *mass, double *energy);
 static const orc_held_suarez *g_hs = NULL;   /* set by orc_step_held_suarez for the duration of its call */
 static const orc_hot_jupiter *g_hj = NULL;   /* likewise, orc_step_hot_jupiter */
 
@@ -1005,6 +1014,8 @@ void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, do
     }
     for (int i = 0; i < N; i++) { W[(size_t)i * (nv + 1)] = 0.0; W[(size_t)i * (nv + 1) + nv] = 0.0; }
     for (int step = 0; step < n_large; step++) {
+        double M0 = 0.0, E0 = 0.0;
+        if (g_efix) orc_diagnostics(G, rho, V, W, p, &M0, &E0);
         memcpy(w->rho_n, rho, 8 * nc); memcpy(w->V_n, V, 24 * nc); memcpy(w->W_n, W, 8 * ni); memcpy(w->p_n, p, 8 * nc);
 #pragma omp parallel for schedule(static)
         for (size_t c = 0; c < nc; c++) w->rt_n[c] = eos_rt(&G->P, w->p_n[c]);
@@ -1039,6 +1050,12 @@ void orc_step_diffusion(const orc_geom *G, double *rho, double *V, double *W, do
             for (size_t c = 0; c < ni; c++) w->W_t[c] = w->W_t[c] + w->W_s[c];
         }
         memcpy(rho, w->rho_t, 8 * nc); memcpy(V, w->V_t, 24 * nc); memcpy(W, w->W_t, 8 * ni); memcpy(p, w->p_t, 8 * nc);
+        if (g_efix) {                                              /* RE1 */
+            double M1, E1;
+            orc_diagnostics(G, rho, V, W, p, &M1, &E1);
+            const double dT = (E0 - E1) / ((G->P.Cp - G->P.Rd) * M1);
+            for (size_t c = 0; c < nc; c++) p[c] = p[c] + rho[c] * G->P.Rd * dT;
+        }
         if (g_hj) forcing_hot_jupiter(G, dt, rho, p, g_hj);
         else if (g_hs) forcing_held_suarez(G, dt, rho, V, p, g_hs);
         else forcing(G, dt, rho, V, p, T_eq, k_T, k_v);

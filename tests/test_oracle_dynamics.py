@@ -383,6 +383,43 @@ def test_total_energy_closed_forms(ogrid):
     assert abs((E - E_int) - E_kv) <= 1e-8 * E_kv
 
 
+# ------------------------------------------------------------------------------------- energy fixer RE1
+def test_energy_fixer_restores_total_energy_by_one_uniform_temperature_increment(ogrid):
+    """NEXT-4, reading RE1 (L215, "globally uniform adjusts the internal energy at all grid points"): with the fixer
+    on, an unforced run keeps the total energy of R10 (pinned by test_total_energy_closed_forms) to round-off while
+    the same run without it drifts by orders of magnitude more; the adjustment of one step is ONE temperature
+    increment dT = (E - E')/(Cv M) for every cell, density untouched; off is the base path bit for bit."""
+    xyz, nbr, C = ogrid(2, True)
+    nv, n, dt = 6, 4, 900.0
+    planet = ti.EARTH
+    G = oracle.Geometry(xyz, nbr, nv, planet, C)
+    rho, V, W, p = ti.rest_state(planet, nv, G.N, 1e5, 300.0)
+    x, y, z = xyz[:, 0:1], xyz[:, 1:2], xyz[:, 2:3]
+    rho = p / (planet["Rd"] * 300.0 * (1 + 0.01 * x * z + 0.005 * y))
+    vel = 15.0 * np.cross(np.array([0.3, 0.2, 1.0]), xyz)[:, None, :] * np.ones((1, nv, 1))
+    s0 = (rho, rho[..., None] * vel, W, p)
+    m0, e0 = G.diagnostics(*s0)
+    plain = G.step(*s0, 1, dt, n)
+    fixed = G.step(*s0, 1, dt, n, energy_fixer=True)
+    m1, e1 = G.diagnostics(*plain)
+    mf, ef = G.diagnostics(*fixed)
+    assert abs(e1 - e0) > 1e-9 * e0                                   # the dynamics alone do change E: a real test
+    assert abs(ef - e0) <= 2e-15 * e0
+    assert np.array_equal(fixed[0], plain[0]) and np.array_equal(fixed[1], plain[1]) and np.array_equal(fixed[2], plain[2])
+    dT = (fixed[3] - plain[3]) / (plain[0] * planet["Rd"])
+    expect = (e0 - e1) / ((planet["Cp"] - planet["Rd"]) * m1)
+    assert np.abs(dT - expect).max() <= 1e-6 * abs(expect) + 1e-12     # uniform; p - p' itself is rounded at ulp(p)
+    # many steps: E stays, mass stays
+    run = G.step(*s0, 20, dt, n, energy_fixer=True)
+    mr, er = G.diagnostics(*run)
+    m20, e20 = G.diagnostics(*G.step(*s0, 20, dt, n))
+    assert abs(er - e0) <= 1e-14 * e0 and abs(mr - m0) <= 1e-13 * m0
+    assert abs(e20 - e0) > 100 * abs(er - e0)
+    # off = the base path
+    again = G.step(*s0, 1, dt, n, energy_fixer=False)
+    assert all(np.array_equal(a, b) for a, b in zip(again, plain))
+
+
 # ------------------------------------------------------------------------------------- forcing R9
 def test_forcing_limits(ogrid):
     cfg = ti.CONFIGS[0]
