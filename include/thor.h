@@ -153,6 +153,13 @@ typedef struct {
 } thor_hot_jupiter;
 int thor_state_set_hot_jupiter(thor_state *state, const thor_hot_jupiter *hj);
 
+/* NEXT-4 (L215): the energy fixer "proposed by Williamson et al. (2009), which globally uniform adjusts the internal
+ * energy at all grid points".  Reading RE1: after the dynamics of every large step and before its forcing, the total
+ * energy (as thor_diagnostics defines it) is brought back to its value before the step by ONE temperature increment for
+ * all cells, dT = (E - E')/(Cv M); rho is unchanged, p <- p + rho Rd dT.  The sums run on the device (k_diag partial
+ * sums per column, one-block compensated sum).  on = 0 (the default, and what the paper's runs use): off. */
+int thor_state_set_energy_fixer(thor_state *state, int on);
+
 /* Only the hot loop: n_substeps acoustic substeps (steps a4-a9 of DESIGN.md) of length delta on the
  * stage data left by the last thor_step.  which: 1 = explicit horizontal momentum kernel only,
  * 2 = divergence + column-solve kernel only, 3 = both.  For measurement; the state it leaves is

@@ -67,6 +67,7 @@ _SIGNATURES = {
     "thor_state_destroy": (None, [_V]),
     "thor_step": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.POINTER(thor_forcing)]),
     "thor_state_set_diffusion": (ctypes.c_int, [_V, ctypes.c_double, ctypes.c_double]),
+    "thor_state_set_energy_fixer": (ctypes.c_int, [_V, ctypes.c_int]),
     "thor_state_set_held_suarez": (ctypes.c_int, [_V, ctypes.POINTER(thor_held_suarez)]),
     "thor_state_set_hot_jupiter": (ctypes.c_int, [_V, ctypes.POINTER(thor_hot_jupiter)]),
     "thor_acoustic_substeps": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int]),
@@ -186,6 +187,10 @@ def thor_step(state, n_large, dt, n_acoustic_substeps, forcing=None):
 
 def thor_state_set_diffusion(state, D_hyper, D_div):
     _check(load_library().thor_state_set_diffusion(state, float(D_hyper), float(D_div)))
+
+
+def thor_state_set_energy_fixer(state, on):
+    _check(load_library().thor_state_set_energy_fixer(state, int(bool(on))))
 
 
 def thor_state_set_held_suarez(state, hs):
@@ -348,6 +353,10 @@ class State:
     def set_diffusion(self, D_hyper, D_div=None):
         """NEXT-1: hyper-diffusion and divergence damping parameter D of Eq. 49 (D_div defaults to D_hyper, L367)."""
         thor_state_set_diffusion(self._h, D_hyper, D_hyper if D_div is None else D_div)
+
+    def set_energy_fixer(self, on=True):
+        """NEXT-4: the energy fixer of L215 (reading RE1) for the following steps."""
+        thor_state_set_energy_fixer(self._h, on)
 
     def set_held_suarez(self, hs):
         thor_state_set_held_suarez(self._h, hs)

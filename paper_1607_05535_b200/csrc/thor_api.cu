@@ -91,10 +91,12 @@ struct thor_state {
     double *tab_Teq = nullptr, *tab_kT = nullptr, *tab_kv = nullptr;   // [Npad][NVP]
     bool has_Teq = false, has_kT = false, has_kv = false;
     double *col_mass = nullptr, *col_energy = nullptr;
+    int efix = 0;                    // NEXT-4: energy fixer of L215 (RE1) on
+    double* efix_dev = nullptr;      // device [M, E before the step; M', E' after its dynamics]
     bool stepped = false;
     int walk = 0;                    // direction of the last launch (0 ascending, 1 descending)
     // one large step captured as a CUDA graph, per starting walk direction (replayed while the key holds)
-    struct GraphKey { double dt = 0, D_hyp = 0, D_div = 0; HeldSuarez hs{}; HotJupiter hj{}; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
+    struct GraphKey { double dt = 0, D_hyp = 0, D_div = 0; int efix = 0; HeldSuarez hs{}; HotJupiter hj{}; int n = 0; const double *Teq = nullptr, *kT = nullptr, *kv = nullptr; char tune[96] = {0}; };
     GraphKey gkey;
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     int gwalk_end[2] = {0, 0};
@@ -596,7 +598,7 @@ static void drop_graphs(thor_state* s);
 void thor_state_destroy(thor_state* s) {
     if (!s) return;
     cudaFree(s->S); cudaFree(s->X); cudaFree(s->stage_buf); cudaFree(s->tab_Teq); cudaFree(s->tab_kT); cudaFree(s->tab_kv);
-    cudaFree(s->col_mass); cudaFree(s->col_energy);
+    cudaFree(s->col_mass); cudaFree(s->col_energy); cudaFree(s->efix_dev);
     drop_graphs(s);
     delete s;
 }
@@ -680,6 +682,13 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
     const double Kd_div = (s->X && s->D_div > 0.0) ? s->D_div * dbar * dbar * dbar * dbar / dt : 0.0;
     // every launch walks the columns opposite to the one before it (L2 hand-over)
     auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
+    // NEXT-4 (RE1): total mass and energy of a state in the Phi^n rows -> two device scalars
+    auto sum_state = [&](double* out) {
+        THOR_DISPATCH(k_diag, nv, Npad, st, g, S, s->col_mass, s->col_energy);
+        k_sum_columns<<<1, 1024, 0, st>>>(hg.N, s->col_mass, s->col_energy, out);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    };
+    if (s->efix) sum_state(s->efix_dev);
     for (int stage = 1; stage <= 3; ++stage) {                         // Eq. 30
         const int ns = stage == 1 ? 1 : (stage == 2 ? n / 2 : n);      // L252, L312-L316
         const double delta = stage == 1 ? dt / 3.0 : dt / n;
@@ -716,7 +725,14 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
             if (int rc = launch_vertical(s->grid, g, S, delta, first, t2, st, Kd_div > 0.0 ? s->X : nullptr)) return rc;
         }
     }
-    THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, s->hs, s->hj, dt, dir(tn.ks));
+    if (s->efix) {
+        // dynamics -> Phi^n rows without forcing; its mass and energy; one uniform temperature increment, then the forcing
+        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, Forcing{nullptr, nullptr, nullptr}, HeldSuarez{}, HotJupiter{}, dt, dir(tn.ks));
+        sum_state(s->efix_dev + 2);
+        THOR_DISPATCH(k_finish_fix, nv, Npad, st, g, S, F, s->hs, s->hj, dt, dir(tn.ks), s->efix_dev);
+    } else {
+        THOR_DISPATCH(k_finish, nv, Npad, st, g, S, F, s->hs, s->hj, dt, dir(tn.ks));
+    }
     return THOR_OK;
 }
 
@@ -752,7 +768,7 @@ int thor_step(thor_state* s, int n_large, double dt, int n, const thor_forcing* 
     if (use_graph) {
         thor_state::GraphKey key;
         std::memset(&key, 0, sizeof(key));
-        key.dt = dt; key.n = n; key.D_hyp = s->D_hyp; key.D_div = s->D_div; key.hs = s->hs; key.hj = s->hj; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
+        key.dt = dt; key.n = n; key.efix = s->efix; key.D_hyp = s->D_hyp; key.D_div = s->D_div; key.hs = s->hs; key.hj = s->hj; key.Teq = F.T_eq; key.kT = F.k_T; key.kv = F.k_v;
         if (const char* e = std::getenv("THOR_B200_TUNE")) std::strncpy(key.tune, e, sizeof(key.tune) - 1);
         if (std::memcmp(&key, &s->gkey, sizeof(key)) != 0) {
             drop_graphs(s);
@@ -803,6 +819,18 @@ int thor_state_set_diffusion(thor_state* s, double D_hyper, double D_div) {
     }
     s->D_hyp = D_hyper;
     s->D_div = D_div;
+    return THOR_OK;
+}
+
+int thor_state_set_energy_fixer(thor_state* s, int on) {
+    if (!s) return fail(THOR_EINVAL, "thor_state_set_energy_fixer: null state");
+    if (on && !s->efix_dev) {
+        const cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&s->efix_dev), 4 * sizeof(double));
+        if (e != cudaSuccess)
+            return fail(e == cudaErrorMemoryAllocation ? THOR_ENOMEM : THOR_ECUDA,
+                        std::string("thor_state_set_energy_fixer: ") + cudaGetErrorString(e));
+    }
+    s->efix = on ? 1 : 0;
     return THOR_OK;
 }
 

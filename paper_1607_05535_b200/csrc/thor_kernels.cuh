@@ -781,22 +781,35 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     const double kv = g.Rd / (g.Cp - g.Rd), cph = g.Cp / g.Rd;
     // per column group: 14 divergence weights (+2 pad), 12 gradient weights, the frames of the column and its
     // 6 neighbours (7 x 12), 6 Laplacian weights (+2 pad), 8 neighbour slots
-    __shared__ double wsm[CPB][16 + 12 + 84 + 8];
-    __shared__ int nsm[CPB][8];
-    double* wdv = wsm[threadIdx.x / G];
-    double* wgv = wdv + 16;
-    double* frm = wgv + 12;
-    double* wlp = frm + 84;
-    int* nbs = nsm[threadIdx.x / G];
-    stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
-    stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, wgv, 6, L.gl);
-    if (HYP) stage_weights<G>(g.wlap + size_t(L.col) * 8, wlp, 4, L.gl);
-    for (int i = L.gl; i < 8; i += G) nbs[i] = i == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 8 + i - 1);
-    __syncwarp();
-    for (int i = L.gl; i < 42; i += G)
-        reinterpret_cast<double2*>(frm)[i] = __ldg(reinterpret_cast<const double2*>(g.frame) + 6 * size_t(nbs[i / 6]) + i % 6);
-    const int nb[7] = {nbs[0], nbs[1], nbs[2], nbs[3], nbs[4], nbs[5], nbs[6]};
-    __syncwarp();
+    // The base kernel stages them in shared memory (registers are what limits it); the hyper-diffusion variant, which
+    // is short of shared-memory bandwidth rather than registers, reads them straight from global memory -- L1 hits
+    // after the first touch (measured: profiles/r02c_variants.md).
+    const double *wdv, *wgv, *wlp, *frm;
+    int nb[7];
+    if constexpr (HYP) {
+        (void)CPB;
+        wdv = g.wdiv2 + size_t(L.col) * 16; wgv = g.wgrad2 + size_t(L.col) * 12; wlp = g.wlap + size_t(L.col) * 8;
+        const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
+        const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+        nb[0] = L.col; nb[1] = n03.x; nb[2] = n03.y; nb[3] = n03.z; nb[4] = n03.w; nb[5] = n47.x; nb[6] = n47.y;
+        frm = nullptr;
+    } else {
+        __shared__ double wsm[CPB][16 + 12 + 84 + 8];
+        __shared__ int nsm[CPB][8];
+        double* ws = wsm[threadIdx.x / G];
+        int* nbs = nsm[threadIdx.x / G];
+        stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, ws, 8, L.gl);
+        stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, ws + 16, 6, L.gl);
+        for (int i = L.gl; i < 8; i += G) nbs[i] = i == 0 ? L.col : __ldg(g.nbr + size_t(L.col) * 8 + i - 1);
+        __syncwarp();
+        for (int i = L.gl; i < 42; i += G)
+            reinterpret_cast<double2*>(ws + 28)[i] = __ldg(reinterpret_cast<const double2*>(g.frame) + 6 * size_t(nbs[i / 6]) + i % 6);
+#pragma unroll
+        for (int j = 0; j < 7; ++j) nb[j] = nbs[j];
+        wdv = ws; wgv = ws + 16; frm = ws + 28; wlp = ws + 112;
+        __syncwarp();
+    }
+    auto frame_of = [&](int j) { return HYP ? g.frame + size_t(nb[j]) * 12 : frm + 12 * j; };
 
     double p0[E];
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], ga[E], gb[E];
@@ -814,7 +827,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     for (int j = 0; j < 7; ++j) {
         const double* q = S + size_t(nb[j]) * REC + L.k0;
         const double wa = wdv[2 * j], wb = wdv[2 * j + 1];
-        const double* f = frm + 12 * j;
+        const double* f = frame_of(j);
         double a[E], b[E], tj[E], pj[E], irj[E], Wj[E], Wup[E];
         ld_nc<E>(q + F_VAT * NVP, a);  ld_nc<E>(q + F_VBT * NVP, b);  ld_nc<E>(q + F_TH * NVP, tj);
         ld_nc<E>(q + F_PT * NVP, pj);  ld_nc<E>(q + F_IRT * NVP, irj); ld_nc<E>(q + F_WT * NVP, Wj);
@@ -883,7 +896,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     double Wc3[K3 ? E : 1];
     if constexpr (K3) interp_c3<G, E>(g.vk + 512 + L.k0, W, Wc3, L.gl);
     ld_again<E>(me + F_VAT * NVP, a0); ld_again<E>(me + F_VBT * NVP, b0); ld_again<E>(me + F_IRT * NVP, ir0);
-    const double* f0 = frm;
+    const double* f0 = frame_of(0);
     const double e1x = f0[0], e1y = f0[1], e1z = f0[2], e2x = f0[3], e2y = f0[4], e2z = f0[5];
     const double rx = f0[6], ry = f0[7], rz = f0[8];
     double Mx[E], My[E], Mz[E];                                              // full momentum M = V + I_c[W] r
@@ -1059,13 +1072,19 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
-    __shared__ double wsm[kWarpsPerBlock * 32 / G][12];
-    double* wgv = wsm[threadIdx.x / G];
-    stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, wgv, 6, L.gl);
+    const double* wgv;                 // DD: straight from global memory (as k_slow_terms_hyp), else staged
+    if constexpr (DD) {
+        wgv = g.wgrad2 + size_t(L.col) * 12;
+    } else {
+        __shared__ double wsm[kWarpsPerBlock * 32 / G][12];
+        double* ws = wsm[threadIdx.x / G];
+        stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, ws, 6, L.gl);
+        wgv = ws;
+    }
     const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
     const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
     const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    __syncwarp();
+    if constexpr (!DD) __syncwarp();
     double ga[E], gb[E], ri[E], va[E], vb[E], sa[E], sb[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) ga[e] = gb[e] = va[e] = vb[e] = 0.0;
@@ -1424,14 +1443,23 @@ k_vertical_staged(Geom g, TileTab tt, double* __restrict__ S, double delta, int 
 // End of the large step: Phi^(n+1) = Phi^[t] + Phi* (Fig. 6 large-step 4), then the PROFX forcing
 // (Eq. 51-52, backward Euler with the large step, R9).
 // ---------------------------------------------------------------------------------------------
-template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, double dt, Tune tn) {
+//
+// FIX (NEXT-4, the energy fixer of L215, reading RE1): the step's dynamics are already in the Phi^n rows (a first
+// k_finish launch without forcing put them there and the diagnostics kernels summed their mass and energy): bring
+// the total energy back to its value before the step with ONE temperature increment for all cells,
+// dT = (E - E')/(Cv M), rho unchanged, p <- p + rho Rd dT; then the forcing.  efix: device [M, E, M', E'].
+template <int G, int E, bool FIX>
+__device__ __forceinline__ void finish_block(const Geom& g, double* __restrict__ S, const Forcing& F, const HeldSuarez& H,
+                                             const HotJupiter& J, double dt, const Tune& tn, const double* __restrict__ efix) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
     if (wk.ahead_bid >= 0) {
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
-        prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAT, 5);
+        if (FIX) {
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_RHON, 4); prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PN, 1);
+        } else {
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAS, 2);   prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PS, 4);
+            prefetch_block_rows<G, E>(S, wk.ahead_bid, F_PT, 1);    prefetch_block_rows<G, E>(S, wk.ahead_bid, F_VAT, 5);
+        }
 #if THOR_GEOMPF
         prefetch_block_geom<G>(g.frame, wk.ahead_bid, 96);
         if (!H.on && !J.on) {
@@ -1449,9 +1477,16 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
 #pragma unroll
         for (int e = 0; e < E; ++e) out[e] += d[e];
     };
-    sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p);
     const Frame fr = ld_frame(g.frame, L.col);
-    {
+    if constexpr (FIX) {
+        ld_rw<E>(me + F_RHON * NVP, rho); ld_rw<E>(me + F_PN * NVP, p);
+        ld_rw<E>(me + F_VXN * NVP, vx);   ld_rw<E>(me + F_VYN * NVP, vy); ld_rw<E>(me + F_VZN * NVP, vz);
+        const double dT = (__ldg(efix + 1) - __ldg(efix + 3)) / ((g.Cp - g.Rd) * __ldg(efix + 2));
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+            if (L.k0 + e < g.nv && L.col < g.N) p[e] = p[e] + rho[e] * g.Rd * dT;
+    } else {
+        sum(F_RHOT, F_RHOS, rho); sum(F_PT, F_PS, p);
         double va[E], vb[E];
         sum(F_VAT, F_VAS, va); sum(F_VBT, F_VBS, vb);
 #pragma unroll
@@ -1460,9 +1495,9 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
             vy[e] = va[e] * fr.e1.y + vb[e] * fr.e2.y;
             vz[e] = va[e] * fr.e1.z + vb[e] * fr.e2.z;
         }
+        sum(F_WT, F_WS, a);
+        st_row<E>(me + F_WN * NVP, a);
     }
-    sum(F_WT, F_WS, a);
-    st_row<E>(me + F_WN * NVP, a);
     if (J.on) {
         // Eq. 59-61 (G15, RJ1): T_eq = T_vert(z) + beta_trop(sigma, z) dT_EP cos(lon) cos(lat); cos(lon) cos(lat) = x of the unit vector
         const double p0 = __shfl_sync(kFull, p[0], 0, G), rho0 = __shfl_sync(kFull, rho[0], 0, G);
@@ -1525,8 +1560,44 @@ k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, 
             p[e] = (L.k0 + e < g.nv && L.col < g.N) ? rho[e] * g.Rd * T : p[e];
         }
     }
-    st_row<E>(me + F_RHON * NVP, rho); st_row<E>(me + F_PN * NVP, p);
+    if (!FIX) st_row<E>(me + F_RHON * NVP, rho);
+    st_row<E>(me + F_PN * NVP, p);
     st_row<E>(me + F_VXN * NVP, vx);   st_row<E>(me + F_VYN * NVP, vy); st_row<E>(me + F_VZN * NVP, vz);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_finish(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, double dt, Tune tn) {
+    finish_block<G, E, false>(g, S, F, H, J, dt, tn, nullptr);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+k_finish_fix(Geom g, double* __restrict__ S, Forcing F, HeldSuarez H, HotJupiter J, double dt, Tune tn,
+             const double* __restrict__ efix) {
+    finish_block<G, E, true>(g, S, F, H, J, dt, tn, efix);
+}
+
+// Deterministic sum of the per-column partials of k_diag (device order; one block): Neumaier-compensated partial
+// sums per thread over a strided range, then a fixed tree in shared memory.  out[0] = mass, out[1] = energy.
+__global__ void __launch_bounds__(1024)
+k_sum_columns(int N, const double* __restrict__ col_mass, const double* __restrict__ col_energy, double* __restrict__ out) {
+    __shared__ double sm[1024], se[1024];
+    double m = 0.0, cm = 0.0, en = 0.0, ce = 0.0;
+    for (int i = threadIdx.x; i < N; i += 1024) {
+        const double x = col_mass[i], y = col_energy[i];
+        double t = m + x;
+        cm += (fabs(m) >= fabs(x)) ? (m - t) + x : (x - t) + m;
+        m = t;
+        t = en + y;
+        ce += (fabs(en) >= fabs(y)) ? (en - t) + y : (y - t) + en;
+        en = t;
+    }
+    sm[threadIdx.x] = m + cm; se[threadIdx.x] = en + ce;
+    __syncthreads();
+    for (int s = 512; s >= 1; s >>= 1) {
+        if (threadIdx.x < s) { sm[threadIdx.x] += sm[threadIdx.x + s]; se[threadIdx.x] += se[threadIdx.x + s]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[0] = sm[0]; out[1] = se[0]; }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -547,6 +547,46 @@ def test_next3_spring_dynamics_on_the_device(level):
     gd.close()
 
 
+@pytest.mark.parametrize("nv,forced", [(8, False), (32, True)])
+def test_next4_energy_fixer_parity(nv, forced):
+    """NEXT-4 (L215, reading RE1): with the fixer on, the GPU keeps the total energy where the oracle keeps it and
+    matches the oracle's state element by element; off again is the plain step."""
+    import torch
+    planet = ti.EARTH
+    g, G, Gf = _setup(3, nv, planet)
+    s = _random_state(G, planet, 900 + nv, vel=15.0)
+    F = None
+    if forced:
+        rng = np.random.default_rng(4)
+        F = dict(T_eq=280.0 + 20.0 * rng.random(s[0].shape), k_T=np.full(s[0].shape, 1.0 / 86400.0),
+                 k_v=np.full(s[0].shape, 0.2 / 86400.0))
+    dt, n = 600.0, 4
+    stream = torch.cuda.Stream()
+    st = thor.State(g, *s, cuda_stream=stream.cuda_stream)          # graph replay from the second step on
+    st.set_energy_fixer(True)
+    m0, e0 = st.diagnostics()
+    run = lambda geo, x, k: geo.step(*x, k, dt, n, F, energy_fixer=True)
+    Y = Yardstick(G, Gf, s, run)
+    st.step(1, dt, n, F)
+    _compare(st.get(), Y.advance(1), TOL_1, "energy fixer nv=%d forced=%s, 1 step" % (nv, forced))
+    st.step(9, dt, n, F)
+    _compare(st.get(), Y.advance(9), TOL_1 * 10, "energy fixer nv=%d forced=%s, 10 steps" % (nv, forced))
+    m1, e1 = st.diagnostics()
+    mr, er = G.diagnostics(*Y.ref)
+    assert abs(m1 - mr) <= 1e-13 * mr and abs(e1 - er) <= 1e-12 * er
+    plain = G.step(*s, 10, dt, n, F)
+    if not forced:
+        assert abs(e1 - e0) <= 1e-13 * e0                                        # E is kept ...
+        assert abs(G.diagnostics(*plain)[1] - e0) > 100 * abs(e1 - e0)           # ... where the plain run loses it
+    assert np.abs(plain[3] - Y.ref[3]).max() > 1e3 * np.abs(st.get()[3] - Y.ref[3]).max()   # the fixer is not a no-op
+    st.set_energy_fixer(False)
+    st.set(*s)
+    st.step(10, dt, n, F)
+    Yp = Yardstick(G, Gf, s, lambda geo, x, k: geo.step(*x, k, dt, n, F)).advance(10)
+    _compare(st.get(), Yp, TOL_1 * 10, "energy fixer off nv=%d, 10 steps" % nv)
+    st.close()
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""
