@@ -63,7 +63,10 @@ def ncu_warm_traffic(workload, kernel_prefix):
         return None
     i_id, i_k, i_m, i_v = head.index("ID"), head.index("Kernel Name"), head.index("Metric Name"), head.index("Metric Value")
     for r in rd:
-        name = r[i_k].split("thor::")[-1]
+        name = r[i_k]
+        for pre in ("void ", "thor::"):
+            if name.startswith(pre):
+                name = name[len(pre):]
         if name.startswith(kernel_prefix + "<") or name.startswith(kernel_prefix + "("):
             if r[i_m] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
                 per_launch[r[i_id]] = per_launch.get(r[i_id], 0.0) + float(r[i_v].replace(",", ""))

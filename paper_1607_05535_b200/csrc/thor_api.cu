@@ -101,6 +101,11 @@ struct thor_state {
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     int gwalk_end[2] = {0, 0};
     int gkernels = 0;
+    // the launch sequence of thor_acoustic_substeps as a graph (one cached entry; same reason, same rules)
+    struct SubKey { double delta = 0; int n = 0, which = 0, walk0 = 0; char tune[96] = {0}; };
+    SubKey skey;
+    cudaGraphExec_t sexec = nullptr;
+    int swalk_end = 0, skernels = 0;
 };
 
 namespace {
@@ -737,6 +742,7 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
 }
 
 static void drop_graphs(thor_state* s) {
+    if (s->sexec) { cudaGraphExecDestroy(s->sexec); s->sexec = nullptr; }
     for (cudaGraphExec_t& e : s->gexec)
         if (e) { cudaGraphExecDestroy(e); e = nullptr; }
 }
@@ -872,13 +878,49 @@ int thor_acoustic_substeps(thor_state* s, int n_substeps, double delta, int whic
     const Geom g = make_geom(s->grid);
     const TunePair tn = tune();
     auto dir = [&](Tune t) { t.rev = tn.zigzag ? (s->walk ^= 1) : 0; return t; };
-    for (int i = 0; i < n_substeps; ++i) {
-        if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1));
-        TunePair t2 = tn;
-        if (which & 2) t2.k2 = dir(tn.k2);
-        if (which & 2)
-            if (int rc = launch_vertical(s->grid, g, s->S, delta, 0, t2, s->stream)) return rc;
+    auto launch_all = [&]() -> int {
+        for (int i = 0; i < n_substeps; ++i) {
+            if (which & 1) THOR_DISPATCH(k_momentum, h.nv, Npad, s->stream, g, s->S, delta, dir(tn.k1));
+            TunePair t2 = tn;
+            if (which & 2) t2.k2 = dir(tn.k2);
+            if (which & 2)
+                if (int rc = launch_vertical(s->grid, g, s->S, delta, 0, t2, s->stream)) return rc;
+        }
+        return THOR_OK;
+    };
+    // as in thor_step: on a non-default stream the sequence is captured once and replayed (the substep kernels run
+    // back to back inside a large step's graph; timing them with per-launch host gaps would measure the host)
+    if (!(tn.graph && s->stream != nullptr && n_substeps > 0)) {
+        if (int rc = launch_all()) return rc;
+        CU(cudaGetLastError());
+        return THOR_OK;
     }
+    thor_state::SubKey key;
+    std::memset(&key, 0, sizeof(key));
+    key.delta = delta; key.n = n_substeps; key.which = which; key.walk0 = s->walk & 1;
+    if (const char* e = std::getenv("THOR_B200_TUNE")) std::strncpy(key.tune, e, sizeof(key.tune) - 1);
+    if (!s->sexec || std::memcmp(&key, &s->skey, sizeof(key)) != 0) {
+        if (s->sexec) { cudaGraphExecDestroy(s->sexec); s->sexec = nullptr; }
+        const long long l0 = g_launches.load();
+        const int w0 = s->walk;
+        cudaGraph_t graph = nullptr;
+        CU(cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+        const int rc = launch_all();
+        const cudaError_t e = cudaStreamEndCapture(s->stream, &graph);
+        s->swalk_end = s->walk;
+        s->walk = w0;
+        s->skernels = int(g_launches.load() - l0);
+        g_launches.store(l0);
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_acoustic_substeps: graph capture: ") + cudaGetErrorString(e));
+        const cudaError_t ei = cudaGraphInstantiate(&s->sexec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) return fail(THOR_ECUDA, std::string("thor_acoustic_substeps: graph instantiate: ") + cudaGetErrorString(ei));
+        std::memcpy(&s->skey, &key, sizeof(key));
+    }
+    CU(cudaGraphLaunch(s->sexec, s->stream));
+    s->walk = s->swalk_end;
+    g_launches.fetch_add(s->skernels, std::memory_order_relaxed);
     CU(cudaGetLastError());
     return THOR_OK;
 }
