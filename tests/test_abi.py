@@ -71,3 +71,6 @@ def test_device_entry_points_fail_loudly_without_a_gpu():
     assert e.value.code == thor.THOR_ECUDA
     with pytest.raises(thor.ThorError):
         g.apply_grad(np.ones((N, 4)))
+    with pytest.raises(thor.ThorError) as e:                       # NEXT-3: the device grid generator needs a device too
+        thor.Grid(1, 4, ti.EARTH, on_device=True)
+    assert e.value.code == thor.THOR_ECUDA
