@@ -407,8 +407,8 @@ def run_cuda(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workload_config(WORKLOAD, N, world),
-                           l2="one large step streams the 33-row column-record slab (%d MB) > 126 MB L2; no flush" % (
-                               33 * 8 * cells * (64 if nv > 32 else 32) // nv // 1000000)),
+                           l2="one large step streams the 30-row column-record slab (%d MB) > 126 MB L2; no flush" % (
+                               30 * 8 * cells * (64 if nv > 32 else 32) // nv // 1000000)),
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes,
                     "ms_per_step": e2e_s / args.steps * 1e3},
