@@ -513,6 +513,35 @@ def test_next3_stretched_layers_and_order_k(nv, order_k, ratio, D):
     g.close()
 
 
+def test_next3_paper_resolution_stretched_order3_30_steps():
+    """NEXT-3 at the paper's benchmark resolution (level 5 x 37 layers): layers stretched 5:1, Eq. 8-9 of order 3,
+    NEXT-1 and the Held-Suarez forcing on, 30 large steps from the benchmark's initial column (rebalanced on the
+    stretched layers) -- element by element against the oracle."""
+    level, nv, n, dt, D = 5, 37, 6, 1000.0, 0.004837
+    planet = dict(ti.EARTH, z_top=32.0e3)
+    z_h = ti.stretched_interfaces(planet, nv, 5.0)
+    g = thor.Grid(level, nv, planet, z_interfaces=z_h, order_k=3)
+    v = g.view
+    G = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], z_interfaces=z_h, vert_order=3)
+    Gf = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], fma=True, z_interfaces=z_h, vert_order=3)
+    pcol, Tcol = ti.benchmark_column(planet, z_h, 1.0e5, ti.held_suarez_equator_profile(planet, ti.HELD_SUAREZ))
+    rng = np.random.default_rng(5)
+    p = np.tile(pcol, (G.N, 1))
+    rho = p / (planet["Rd"] * (np.tile(Tcol, (G.N, 1)) + rng.uniform(-1e-3, 1e-3, size=p.shape)))
+    s = (rho, np.zeros((G.N, nv, 3)), np.zeros((G.N, nv + 1)), p)
+    st = thor.State(g, *s)
+    st.set_diffusion(D)
+    st.set_held_suarez(ti.HELD_SUAREZ)
+    st.step(30, dt, n)
+    Y = Yardstick(G, Gf, s, lambda geo, x, k: geo.step_held_suarez(*x, k, dt, n, ti.HELD_SUAREZ, D, D), seeds=SEEDS[:1]).advance(30)
+    _compare(st.get(), Y, TOL_100, "next3 level 5 x 37 stretched 5:1, k=3, NEXT-1 + Held-Suarez, 30 steps")
+    m, _ = st.diagnostics()
+    mr, _ = G.diagnostics(*Y.ref)
+    assert abs(m - mr) <= 1e-13 * mr
+    st.close()
+    g.close()
+
+
 @pytest.mark.parametrize("level", [3, 5, 6])
 def test_next3_spring_dynamics_on_the_device(level):
     """NEXT-3: thor_grid_create_device iterates Eq. 10-12 on the GPU.  Same update, same stopping test: the points agree
