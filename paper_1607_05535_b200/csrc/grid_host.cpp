@@ -428,6 +428,39 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
         g.d_area[d] = area;
     }
 
+    // --- lattice neighbours: rotate the slots of every interior lattice point to the fixed direction order and
+    // check the arithmetic the kernels use (Morton increments inside the rhombus) against the table
+    {
+        const unsigned nn = 1u << (2 * level), XM = 0xAAAAAAAAu & (nn - 1), YM = 0x55555555u & (nn - 1);
+        bool ok = level >= 2;
+        for (int d = 0; ok && d < N; ++d) {
+            if (unsigned(d) >= 10u * nn) continue;
+            const unsigned r = unsigned(d) >> (2 * level), m = unsigned(d) & (nn - 1), x = m & XM, y = m & YM;
+            if (x == 0 || x == XM || y == 0 || y == YM) continue;
+            const unsigned xp = ((m | YM) + 1) & XM, xn = ((m & XM) - 1) & XM, yp = ((m | XM) + 1) & YM, yn = ((m & YM) - 1) & YM;
+            const unsigned base = r * nn;
+            const int want[6] = {int(base + (xp | y)), int(base + (x | yp)), int(base + (xn | yp)),
+                                 int(base + (xn | y)), int(base + (x | yn)), int(base + (xp | yn))};
+            int* nb = &g.d_nbr[size_t(d) * 6];
+            int k0 = -1;
+            for (int k = 0; k < 6; ++k)
+                if (nb[k] == want[0]) k0 = k;
+            if (k0 < 0) { ok = false; break; }
+            if (k0 > 0) {
+                std::rotate(nb, nb + k0, nb + 6);
+                double* wl = &g.d_wlap[size_t(d) * 6];
+                std::rotate(wl, wl + k0, wl + 6);
+                double* wd = &g.d_wdiv[size_t(d) * 21 + 3];
+                std::rotate(wd, wd + 3 * k0, wd + 18);
+                double* wg = &g.d_wgrad[size_t(d) * 18];
+                std::rotate(wg, wg + 3 * k0, wg + 18);
+            }
+            for (int k = 0; k < 6; ++k)
+                if (nb[k] != want[k]) ok = false;
+        }
+        g.lattice_nbr = ok;
+    }
+
     // --- tangent basis per column and the stencils contracted with it.  e1 = z x r (x x r next to the
     // poles), e2 = r x e1: no smoothness is needed, the weights absorb the basis of every neighbour.
     g.d_basis.assign(size_t(N) * 6, 0.0);

@@ -47,6 +47,11 @@ struct HostGrid {
     double dz = 0;                 // z_top / nv (mean thickness)
     // NEXT-3: Eq. 8-9 of order kord (1 or 3) in the explicit slow terms (RV1, RV2).  kord = 3: Lagrange weights of
     // the four nearest nodes, 0 for the nodes the column's end cuts off (the order falls by one per missing node)
+    // Interior lattice points of a rhombus (1 <= I <= n-2, 1 <= J-1 <= n-2) have their six neighbours at the fixed
+    // lattice offsets (1,0), (0,1), (-1,1), (-1,0), (0,-1), (1,-1), counter-clockwise, in the same rhombus: their
+    // device slots are rotated to start at (1,0), so that the kernels can COMPUTE the neighbour columns from the
+    // column's own Morton index instead of loading them (true when the generator has verified it for every such column)
+    bool lattice_nbr = false;
     int kord = 1;
     std::vector<double> ihw;       // [4][nv] centre k-2, k-1, k, k+1 -> lower interface of layer k (0 for k = 0)
     std::vector<double> icw;       // [4][nv] interface k-1, k, k+1, k+2 -> centre of layer k

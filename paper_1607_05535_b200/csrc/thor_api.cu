@@ -306,6 +306,7 @@ Geom make_geom(const thor_grid* grid) {
     g.dd_idx = d.dd_idx; g.dd_coef = d.dd_coef;
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
     g.wl = d.wl; g.wh = d.wh; g.idz = d.idz; g.vk = d.vk; g.kord = h.kord;
+    g.lvl2 = h.lattice_nbr ? 2 * h.level : -1;
     g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);

@@ -106,6 +106,9 @@ struct Geom {                 // device pointers, device column order, padded to
     // centre of layer k (0 for the nodes the column's end cuts off, and on pads); used when kord == 3
     const double* vk;
     int kord;
+    // >= 0: twice the grid level; interior lattice points of a rhombus then have their neighbour columns COMPUTED
+    // from their own Morton index (HostGrid::lattice_nbr); -1: always the nbr table
+    int lvl2;
     double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
@@ -196,6 +199,28 @@ struct Map {
         k0 = gl * E;
     }
 };
+
+// The six neighbour columns of `col`.  Device order: rhombus r owns columns r n^2 .. (r+1) n^2 - 1 along the Morton
+// curve of its lattice (I in the odd bits, J-1 in the even bits).  A lattice point that is not on the rim of its
+// rhombus has its neighbours at the offsets (1,0), (0,1), (-1,1), (-1,0), (0,-1), (1,-1) -- the slot order the host
+// generator gives such columns -- so their indices follow from the column's own by Morton increments: no load, and
+// the gathers that depend on them can be issued at once.  Rim columns, the poles and pad columns read the table.
+__device__ __forceinline__ void neighbours(const Geom& g, int col, int (&nb)[6]) {
+    if (g.lvl2 >= 0) {
+        const unsigned nn = 1u << g.lvl2, XM = 0xAAAAAAAAu & (nn - 1), YM = 0x55555555u & (nn - 1);
+        const unsigned m = unsigned(col) & (nn - 1), x = m & XM, y = m & YM;
+        if (unsigned(col) < 10u * nn && x != 0 && x != XM && y != 0 && y != YM) {
+            const unsigned base = unsigned(col) - m;
+            const unsigned xp = ((m | YM) + 1) & XM, xn = (x - 1) & XM, yp = ((m | XM) + 1) & YM, yn = (y - 1) & YM;
+            nb[0] = int(base + (xp | y));  nb[1] = int(base + (x | yp));  nb[2] = int(base + (xn | yp));
+            nb[3] = int(base + (xn | y));  nb[4] = int(base + (x | yn));  nb[5] = int(base + (xp | yn));
+            return;
+        }
+    }
+    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
+    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
+    nb[0] = n03.x; nb[1] = n03.y; nb[2] = n03.z; nb[3] = n03.w; nb[4] = n47.x; nb[5] = n47.y;
+}
 
 template <int E>
 __device__ __forceinline__ void ld_nc(const double* p, double (&v)[E]) {     // rows nobody writes in this kernel
@@ -786,12 +811,15 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     // after the first touch (measured: profiles/r02c_variants.md).
     const double *wdv, *wgv, *wlp, *frm;
     int nb[7];
-    if constexpr (HYP) {
+    constexpr bool DIRECT = HYP;
+    if constexpr (DIRECT) {
         (void)CPB;
         wdv = g.wdiv2 + size_t(L.col) * 16; wgv = g.wgrad2 + size_t(L.col) * 12; wlp = g.wlap + size_t(L.col) * 8;
-        const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-        const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-        nb[0] = L.col; nb[1] = n03.x; nb[2] = n03.y; nb[3] = n03.z; nb[4] = n03.w; nb[5] = n47.x; nb[6] = n47.y;
+        int n6[6];
+        neighbours(g, L.col, n6);
+        nb[0] = L.col;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) nb[j + 1] = n6[j];
         frm = nullptr;
     } else {
         __shared__ double wsm[CPB][16 + 12 + 84 + 8];
@@ -809,7 +837,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
         wdv = ws; wgv = ws + 16; frm = ws + 28; wlp = ws + 112;
         __syncwarp();
     }
-    auto frame_of = [&](int j) { return HYP ? g.frame + size_t(nb[j]) * 12 : frm + 12 * j; };
+    auto frame_of = [&](int j) { return DIRECT ? g.frame + size_t(nb[j]) * 12 : frm + 12 * j; };
 
     double p0[E];
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], ga[E], gb[E];
@@ -1072,19 +1100,11 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
     constexpr int NVP = Map<G, E>::NVP;
     constexpr size_t REC = Map<G, E>::REC;
     double* me = S + size_t(L.col) * REC + L.k0;
-    const double* wgv;                 // DD: straight from global memory (as k_slow_terms_hyp), else staged
-    if constexpr (DD) {
-        wgv = g.wgrad2 + size_t(L.col) * 12;
-    } else {
-        __shared__ double wsm[kWarpsPerBlock * 32 / G][12];
-        double* ws = wsm[threadIdx.x / G];
-        stage_weights<G>(g.wgrad2 + size_t(L.col) * 12, ws, 6, L.gl);
-        wgv = ws;
-    }
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
-    const int nb[6] = {n03.x, n03.y, n03.z, n03.w, n47.x, n47.y};
-    if constexpr (!DD) __syncwarp();
+    // the 12 gradient weights are read straight from global memory where they are used: one 96-byte line per column,
+    // L1 hits after the first touch, and nothing waits for them before the gathers can be issued
+    const double* wgv = g.wgrad2 + size_t(L.col) * 12;
+    int nb[6];
+    neighbours(g, L.col, nb);
     double ga[E], gb[E], ri[E], va[E], vb[E], sa[E], sb[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) ga[e] = gb[e] = va[e] = vb[e] = 0.0;
@@ -1301,15 +1321,12 @@ __device__ __forceinline__ void vertical_block(const Geom& g, double* __restrict
 #endif
     }
     if (wk.in_tail) prefetch_block_rows<G, E>(S, wk.bid, F_SVA, 2);               // the next momentum kernel starts here
-    __shared__ double wsm[kWarpsPerBlock * 32 / G][16];
-    double* wdv = wsm[threadIdx.x / G];
-    stage_weights<G>(g.wdiv2 + size_t(L.col) * 16, wdv, 8, L.gl);
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(L.col) * 8) + 1);
+    const double* wdv = g.wdiv2 + size_t(L.col) * 16;      // read where used (one 128-byte line per column, L1 hits)
+    int nb[6];
+    neighbours(g, L.col, nb);
     constexpr size_t REC = Map<G, E>::REC;
-    const double* const nbp[6] = {S + size_t(n03.x) * REC + L.k0, S + size_t(n03.y) * REC + L.k0, S + size_t(n03.z) * REC + L.k0,
-                                  S + size_t(n03.w) * REC + L.k0, S + size_t(n47.x) * REC + L.k0, S + size_t(n47.y) * REC + L.k0};
-    __syncwarp();
+    const double* const nbp[6] = {S + size_t(nb[0]) * REC + L.k0, S + size_t(nb[1]) * REC + L.k0, S + size_t(nb[2]) * REC + L.k0,
+                                  S + size_t(nb[3]) * REC + L.k0, S + size_t(nb[4]) * REC + L.k0, S + size_t(nb[5]) * REC + L.k0};
     double* me = S + size_t(L.col) * REC + L.k0;
     if constexpr (DD)
         vertical_column<G, E, true>(g, me, me, nbp, wdv, L.gl, L.k0, delta, first, Xdd + size_t(L.col) * (size_t(XF) * Map<G, E>::NVP) + L.k0);
@@ -1626,9 +1643,7 @@ __device__ __forceinline__ void lap_gather(const double* base, size_t stride, co
     }
 }
 __device__ __forceinline__ void ld_lap_weights(const Geom& g, int col, int (&nb)[6], double (&w)[6]) {
-    const int4 n03 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8));
-    const int4 n47 = __ldg(reinterpret_cast<const int4*>(g.nbr + size_t(col) * 8) + 1);
-    nb[0] = n03.x; nb[1] = n03.y; nb[2] = n03.z; nb[3] = n03.w; nb[4] = n47.x; nb[5] = n47.y;
+    neighbours(g, col, nb);
     const double2* wp = reinterpret_cast<const double2*>(g.wlap + size_t(col) * 8);
     const double2 a = __ldg(wp), b = __ldg(wp + 1), c = __ldg(wp + 2);
     w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x; w[5] = c.y;

@@ -86,3 +86,40 @@ def test_operator_accuracy_on_library_grids():
         e[lvl] = (math.sqrt(np.sum(G.Ac * err ** 2) / G.Ac.sum()), np.abs(err).max())
     assert 1.8 < math.log2(e[4][0] / e[5][0]) < 2.2
     assert 1.7 < math.log2(e[4][1] / e[5][1]) < 2.3
+
+
+@pytest.mark.parametrize("level", [2, 3, 4])
+def test_interior_lattice_points_have_the_six_fixed_neighbour_offsets(level):
+    """What the kernels' computed neighbour indices rest on (thor_kernels.cuh: neighbours()): the device order is
+    rhombus by rhombus along the Morton curve of (I, J-1), and a lattice point that is not on the rim of its rhombus has
+    its six neighbours in the same rhombus at the offsets (1,0), (0,1), (-1,1), (-1,0), (0,-1), (1,-1), counter-clockwise."""
+    g = thor.Grid(level, 4, ti.EARTH)
+    v = g.view
+    n, N = 1 << level, g.n_cols
+    order, nbr = v["device_order"], v["nbr"]
+    rank = np.empty(N, dtype=np.int64)
+    rank[order] = np.arange(N)
+
+    def lattice(m):
+        I = sum(((m >> (2 * b + 1)) & 1) << b for b in range(16))
+        J = sum(((m >> (2 * b)) & 1) << b for b in range(16))
+        return I, J
+
+    want = [(1, 0), (0, 1), (-1, 1), (-1, 0), (0, -1), (1, -1)]
+    seen = 0
+    for d in range(10 * n * n):
+        r, m = divmod(d, n * n)
+        I, J = lattice(m)
+        if not (1 <= I <= n - 2 and 1 <= J <= n - 2):
+            continue
+        offs = []
+        for k in range(6):
+            rn, mn = divmod(int(rank[nbr[order[d], k]]), n * n)
+            assert rn == r
+            In, Jn = lattice(mn)
+            offs.append((In - I, Jn - J))
+        i0 = offs.index((1, 0))
+        assert offs[i0:] + offs[:i0] == want, (d, offs)
+        seen += 1
+    assert seen == 10 * (n - 2) ** 2
+    g.close()
