@@ -169,6 +169,17 @@ int thor_acoustic_substeps(thor_state *state, int n_substeps, double delta, int 
 /* Total mass sum(rho A_c r_k^2 dz) and total energy sum((Cv p/Rd + |rho v|^2/(2 rho) + rho g z) A_c r_k^2 dz) (R10). */
 int thor_diagnostics(const thor_state *state, thor_diag *out);
 
+/* The same diagnostics for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no cudaMalloc, cudaFree or host allocation in this call.  The per-column partial
+ * sums and the two results live in a file-scope device array of the library (1 MiB, held by every GPU that loads the
+ * library until the process exits) and are summed on the device (one block, compensated partial sums, fixed order):
+ * the result agrees with thor_diagnostics to rounding of the sum (relative 1e-15), not bit for bit.
+ * Limit: at most 65 536 columns, i.e. grid levels 0..6; larger grids get THOR_EINVAL (use thor_diagnostics).
+ * Every call, on every state, shares that array and it keeps the last call's contents (the call clears what it must):
+ * calls that overlap on the GPU (different streams or threads) race -- serialise them.  Synchronises the state's
+ * stream; the state must live on the current device. */
+int thor_diagnostics_noalloc(const thor_state *state, thor_diag *out);
+
 /* Config-1 operators at radius r_k (unit-sphere operator / r_k): Eq. 6 divergence of vec
  * [n_cols][n_layers][3] -> out [n_cols][n_layers]; Eq. 7 gradient (difference form, projected with
  * Eq. 28) of s [n_cols][n_layers] -> out [n_cols][n_layers][3].  Host arrays, canonical order. */

@@ -72,6 +72,7 @@ _SIGNATURES = {
     "thor_state_set_hot_jupiter": (ctypes.c_int, [_V, ctypes.POINTER(thor_hot_jupiter)]),
     "thor_acoustic_substeps": (ctypes.c_int, [_V, ctypes.c_int, ctypes.c_double, ctypes.c_int]),
     "thor_diagnostics": (ctypes.c_int, [_V, ctypes.POINTER(thor_diag)]),
+    "thor_diagnostics_noalloc": (ctypes.c_int, [_V, ctypes.POINTER(thor_diag)]),
     "thor_apply_div": (ctypes.c_int, [_V, _D, _D]),
     "thor_apply_grad": (ctypes.c_int, [_V, _D, _D]),
     "thor_apply_div_device": (ctypes.c_int, [_V, _V, _V, _V, _V, _V]),
@@ -217,6 +218,12 @@ def thor_acoustic_substeps(state, n_substeps, delta, which=3):
 def thor_diagnostics(state):
     d = thor_diag()
     _check(load_library().thor_diagnostics(state, ctypes.byref(d)))
+    return d.total_mass, d.total_energy
+
+
+def thor_diagnostics_noalloc(state):
+    d = thor_diag()
+    _check(load_library().thor_diagnostics_noalloc(state, ctypes.byref(d)))
     return d.total_mass, d.total_energy
 
 
@@ -369,6 +376,10 @@ class State:
 
     def diagnostics(self):
         return thor_diagnostics(self._h)
+
+    def diagnostics_noalloc(self):
+        """thor_diagnostics without any allocation (static device scratch; at most 65 536 columns)."""
+        return thor_diagnostics_noalloc(self._h)
 
     def close(self):
         if self._h is not None:

@@ -539,6 +539,35 @@ int spring_dynamics_device(int N, double* xyz, const int* nbr, const int* deg, c
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------
+// thor_diagnostics_noalloc: the per-column partial sums of k_diag and the two results of k_sum_columns live in a
+// file-scope device array instead of buffers from cudaMalloc.  Every GPU that loads the library holds the array
+// (1 MiB + 256 B) until the process exits.  In HOST code the array's name is a host-side stand-in, not a device
+// address: the address the kernels get comes from cudaGetSymbolAddress, looked up once per device with that device
+// current.  All calls share the array: calls that overlap on the GPU race.
+// ---------------------------------------------------------------------------------------------
+constexpr int kNoAllocMaxCols = 65536;                       // grid levels 0..6 (level 6: 40 962 columns)
+static __device__ __align__(256) double g_noalloc_scratch[2 * kNoAllocMaxCols + 32];
+
+namespace {
+int noalloc_scratch_address(double** out) {
+    static std::mutex mu;
+    static double* ptr[64] = {};
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(THOR_ECUDA, "thor_diagnostics_noalloc: device index out of range");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        double* p = nullptr;
+        CU(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_noalloc_scratch));
+        if (!p) return fail(THOR_ECUDA, "thor_diagnostics_noalloc: cudaGetSymbolAddress returned a null address");
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return THOR_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char* thor_last_error(void) { return g_err.c_str(); }
@@ -948,6 +977,36 @@ int thor_diagnostics(const thor_state* s, thor_diag* out) {
     };
     out->total_mass = ksum(m);
     out->total_energy = ksum(e);
+    return THOR_OK;
+}
+
+int thor_diagnostics_noalloc(const thor_state* s, thor_diag* out) {
+    if (!s || !out) return fail(THOR_EINVAL, "thor_diagnostics_noalloc: null argument");
+    const HostGrid& h = s->grid->h;
+    if (h.N > kNoAllocMaxCols)
+        return fail(THOR_EINVAL, "thor_diagnostics_noalloc: " + std::to_string(h.N) + " columns exceed the static scratch of " +
+                                     std::to_string(kNoAllocMaxCols) + " columns (grid level <= 6); use thor_diagnostics");
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev != s->grid->d.device)
+        return fail(THOR_EINVAL, "thor_diagnostics_noalloc: state lives on CUDA device " + std::to_string(s->grid->d.device) +
+                                     ", current device is " + std::to_string(dev));
+    double* scratch = nullptr;
+    if (int rc = noalloc_scratch_address(&scratch)) return rc;
+    double *col_mass = scratch, *col_energy = scratch + kNoAllocMaxCols, *res = scratch + 2 * kNoAllocMaxCols;
+    const Geom g = make_geom(s->grid);
+    // the array keeps the last call's contents: the two result slots are cleared so that a launch that did not run
+    // cannot hand back the previous call's numbers; the per-column slots 0..N-1 are all rewritten by k_diag
+    CU(cudaMemsetAsync(res, 0, 2 * sizeof(double), s->stream));
+    THOR_DISPATCH(k_diag, h.nv, s->grid->d.Npad, s->stream, g, s->S, col_mass, col_energy);
+    k_sum_columns<<<1, 1024, 0, s->stream>>>(h.N, col_mass, col_energy, res);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU(cudaGetLastError());
+    double r[2] = {0.0, 0.0};
+    CU(cudaMemcpyAsync(r, res, sizeof(r), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    out->total_mass = r[0];
+    out->total_energy = r[1];
     return THOR_OK;
 }
 
