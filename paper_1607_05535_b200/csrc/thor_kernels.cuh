@@ -1135,16 +1135,34 @@ __device__ __forceinline__ void momentum_block(const Geom& g, double* __restrict
         ld_nc<E>(Xdd + size_t(L.col) * XREC + L.k0 + d3row * NVP, d0);
 #pragma unroll
         for (int e = 0; e < E; ++e) fa[e] = fb[e] = 0.0;
-#pragma unroll 6
-        for (int q = 0; q < 18; ++q) {
-            const int m = __ldg(di + q);
-            const double2 c = __ldg(dc + q);
-            double dm[E];
-            ld_nc<E>(Xdd + size_t(m) * XREC + L.k0 + d3row * NVP, dm);
+        // the 18 column indices up front (five 128-bit loads), then the D3 rows in batches of kDdBatch gathers that are
+        // all requested before the first is used (measured: profiles/r02c_variants.md)
+#ifndef THOR_DD_BATCH
+#define THOR_DD_BATCH 18
+#endif
+        constexpr int kDdBatch = THOR_DD_BATCH;
+        int mi[20];
 #pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const double dd = dm[e] - d0[e];
-                fa[e] = fma(c.x, dd, fa[e]); fb[e] = fma(c.y, dd, fb[e]);
+        for (int q4 = 0; q4 < 5; ++q4) {
+            const int4 t = __ldg(reinterpret_cast<const int4*>(di) + q4);
+            mi[4 * q4] = t.x; mi[4 * q4 + 1] = t.y; mi[4 * q4 + 2] = t.z; mi[4 * q4 + 3] = t.w;
+        }
+#pragma unroll
+        for (int q0 = 0; q0 < 18; q0 += kDdBatch) {
+            double dm[kDdBatch][E];
+#pragma unroll
+            for (int b = 0; b < kDdBatch; ++b)
+                if (q0 + b < 18) ld_nc<E>(Xdd + size_t(mi[q0 + b]) * XREC + L.k0 + d3row * NVP, dm[b]);
+#pragma unroll
+            for (int b = 0; b < kDdBatch; ++b) {
+                if (q0 + b < 18) {
+                    const double2 c = __ldg(dc + q0 + b);
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {
+                        const double dd = dm[b][e] - d0[e];
+                        fa[e] = fma(c.x, dd, fa[e]); fb[e] = fma(c.y, dd, fb[e]);
+                    }
+                }
             }
         }
 #pragma unroll
