@@ -114,6 +114,7 @@ def _declare(L):
                                        ctypes.c_double, ctypes.c_double]
     L.orc_forcing_hot_jupiter.argtypes = [ctypes.c_void_p, ctypes.c_double, _D, _D, _D]
     L.orc_set_energy_fixer.argtypes = [ctypes.c_int]
+    L.orc_geom_set_shallow.argtypes = [ctypes.c_void_p, ctypes.c_int]
     L.orc_num_threads.restype = ctypes.c_int
     L.orc_set_num_threads.argtypes = [ctypes.c_int]
     return L
@@ -145,7 +146,7 @@ class Geometry:
     NEXT-3: z_interfaces = nv+1 increasing interface altitudes from 0 to z_top (None: uniform layers, R6);
     vert_order = the k of Eq. 8-9 (odd; 1 = linear, the paper's choice)."""
 
-    def __init__(self, xyz, nbr, nv, planet, C=None, fma=False, z_interfaces=None, vert_order=1):
+    def __init__(self, xyz, nbr, nv, planet, C=None, fma=False, z_interfaces=None, vert_order=1, shallow=False):
         L = self._L = _load(fma)
         self.xyz = _c(xyz)
         self.nbr = np.ascontiguousarray(nbr, dtype=np.int32)
@@ -178,6 +179,11 @@ class Geometry:
                 self.z_c = 0.5 * (zi[:-1] + zi[1:])
         self.r_c = planet["radius"] + self.z_c
         self.r_h = planet["radius"] + self.z_h
+        self.shallow = bool(shallow)
+        if self.shallow:                      # NEXT-4, reading RS1: every radius is the planetary radius
+            L.orc_geom_set_shallow(self._h, 1)
+            self.r_c = np.full(nv, float(planet["radius"]))
+            self.r_h = np.full(nv + 1, float(planet["radius"]))
 
     def __del__(self):
         try:

@@ -52,6 +52,8 @@ typedef struct {
     /* NEXT-3 (orc_geom_set_vertical; readings RV1-RV3 of DESIGN.md): layers of unequal thickness and Eq. 8-9 of
      * order kord > 1.  uniform != 0 (the default) is the path above, arithmetic untouched. */
     int uniform, kord;
+    /* NEXT-4 (orc_geom_set_shallow; reading RS1 of DESIGN.md): the shallow-atmosphere approximation of L178 */
+    int shallow;
     double *z_h;  /* [nv+1] interface altitudes, z_h[0] = 0, z_h[nv] = z_top; the centre is the midpoint of its layer */
     double *xyz;  /* [N][3] unit-sphere positions P_i */
     int *nbr;     /* [N][6] neighbours, counter-clockwise seen from outside; -1 pads pentagons */
@@ -444,6 +446,25 @@ int orc_geom_set_vertical(orc_geom *G, const double *z_h, int kord) {
     return 0;
 }
 
+/* NEXT-4, shallow-atmosphere approximation (L178: "The spherical components of the fluid equations that depend on 1/r
+ * are changed to the constant 1/A ... In order to conserve axial angular momentum some metric terms have to be neglected
+ * and also the Coriolis terms involved in the horizontal components of planet's angular velocity", the "traditional
+ * approximations").  The paper prints no equations for it; reading RS1:
+ *   (i)   every radius in the discrete operators is the planetary radius A: r_k = r_h,k = A (horizontal operators / A,
+ *         D_c without its r^2 factors, cell volume A_c A^2 dz); altitudes z are unchanged;
+ *   (ii)  Coriolis keeps the radial component of Omega only: C = 2 Omega sin(lat) r x V, on the horizontal momentum
+ *         alone; W neither feels nor causes a Coriolis force;
+ *   (iii) the metric terms that couple horizontal and vertical motion are dropped: the horizontal momentum equation
+ *         advects the horizontal velocity u_h = V/rho only (no rho v_h v_r / r term), and the vertical momentum equation
+ *         advects w = I_c[W]/rho as a scalar (no -rho |v_h|^2 / r term).  The curvature terms of the horizontal flow on
+ *         the sphere of radius A (u v tan(lat)/A ...) stay: they are what the Cartesian form of Eq. 28 produces.
+ * on = 0 restores the deep atmosphere. */
+void orc_geom_set_shallow(orc_geom *G, int on) {
+    G->shallow = on ? 1 : 0;
+    for (int k = 0; k < G->nv; k++) G->r_c[k] = G->P.radius + (on ? 0.0 : G->z_c[k]);
+    for (int k = 0; k <= G->nv; k++) G->r_h[k] = G->P.radius + (on ? 0.0 : G->z_h[k]);
+}
+
 /* Eq. 24 (L210) and its inverse */
 static double eos_p(const orc_planet *P, double rt) {
     double gam = P->Cp / (P->Cp - P->Rd);
@@ -552,7 +573,10 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
             size_t c = (size_t)i * nv + k;
             double wc = I_ck(G, W, k);
             w->Wc[c] = wc;
-            for (int d = 0; d < 3; d++) w->u[3 * c + d] = (w->V_t[3 * c + d] + wc * rh[d]) / w->rho_t[c];
+            if (G->shallow)                                   /* RS1 (iii): the horizontal velocity alone is advected */
+                for (int d = 0; d < 3; d++) w->u[3 * c + d] = w->V_t[3 * c + d] / w->rho_t[c];
+            else
+                for (int d = 0; d < 3; d++) w->u[3 * c + d] = (w->V_t[3 * c + d] + wc * rh[d]) / w->rho_t[c];
         }
     }
 
@@ -578,6 +602,31 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
                 }
             }
             free(X); free(uj);
+        }
+    }
+
+    /* RS1 (iii): w = I_c[W]/rho advected as a scalar, A_w = div_h(V w) + D_c[W I_h[w]]  (scratch: di3, free here) */
+    double *Aw = w->di3;
+    if (G->shallow) {
+#pragma omp parallel for schedule(static)
+        for (size_t c = 0; c < nc; c++) {
+            double wv = w->Wc[c] / w->rho_t[c];
+            for (int d = 0; d < 3; d++) w->vec[3 * c + d] = w->V_t[3 * c + d] * wv;
+        }
+        orc_hdiv(G, w->vec, w->sc1);
+#pragma omp parallel
+        {
+            double *X = (double *)calloc(nv + 1, sizeof(double));
+            double *wv = (double *)malloc(sizeof(double) * nv);
+#pragma omp for schedule(static)
+            for (int i = 0; i < N; i++) {
+                const double *W = w->W_t + (size_t)i * (nv + 1);
+                for (int k = 0; k < nv; k++) wv[k] = w->Wc[(size_t)i * nv + k] / w->rho_t[(size_t)i * nv + k];
+                X[0] = 0.0; X[nv] = 0.0;
+                for (int k = 1; k < nv; k++) X[k] = W[k] * I_hk(G, wv, k);
+                for (int k = 0; k < nv; k++) Aw[(size_t)i * nv + k] = w->sc1[(size_t)i * nv + k] + D_c(G, X, k);
+            }
+            free(X); free(wv);
         }
     }
 
@@ -612,11 +661,19 @@ static void slow_terms(const orc_geom *G, orc_work *w) {
                 /* Coriolis C = 2 Omega z x M (Eq. 21), rotation axis through the polar vertices */
                 double M[3], Cor[3];
                 for (int d = 0; d < 3; d++) M[d] = w->V_t[3 * c + d] + w->Wc[c] * rh[d];
-                Cor[0] = -2.0 * P->omega * M[1];
-                Cor[1] = 2.0 * P->omega * M[0];
-                Cor[2] = 0.0;
+                if (G->shallow) {                     /* RS1 (ii): f r x V, f = 2 Omega sin(lat), sin(lat) = z of r */
+                    const double f = 2.0 * P->omega * rh[2];
+                    const double *V = w->V_t + 3 * c;
+                    Cor[0] = f * (rh[1] * V[2] - rh[2] * V[1]);
+                    Cor[1] = f * (rh[2] * V[0] - rh[0] * V[2]);
+                    Cor[2] = f * (rh[0] * V[1] - rh[1] * V[0]);
+                } else {
+                    Cor[0] = -2.0 * P->omega * M[1];
+                    Cor[1] = 2.0 * P->omega * M[0];
+                    Cor[2] = 0.0;
+                }
                 double Ar = dot3(A, rh), Cr = dot3(Cor, rh);                   /* Eq. 29 */
-                Fr[k] = Ar + Cr;
+                Fr[k] = G->shallow ? Aw[c] : Ar + Cr;                          /* RS1 (iii) */
                 for (int d = 0; d < 3; d++) {                                   /* Eq. 28 (G5) */
                     double Ah = A[d] - Ar * rh[d], Ch = Cor[d] - Cr * rh[d];
                     w->slowV[3 * c + d] = -w->gradp[3 * c + d] - Ah - Ch;       /* RHS of Eq. 33 */
