@@ -97,6 +97,17 @@ int thor_grid_create(int level, int n_layers, const thor_planet *planet, thor_gr
  * of the target; where the column ends first the missing nodes are dropped (RV1).  Other orders: THOR_EINVAL. */
 int thor_grid_create_vertical(int level, int n_layers, const thor_planet *planet, const double *z_interfaces,
                               int order_k, thor_grid **out);
+/* NEXT-4 (section 3): the same grid for the SHALLOW-ATMOSPHERE approximation, one of the three the paper says
+ * "have been implemented in the model and the user can switch them on and off" (L184) without printing their
+ * equations.  Reading RS1: (i) every radius in the discrete operators is the planetary radius A (horizontal
+ * operators over A, the vertical divergence without its r^2 factors, cell volume A_c A^2 dz); (ii) Coriolis from the
+ * radial component of Omega only, f r x V with f = 2 Omega sin(lat), on the horizontal momentum alone; (iii) no metric
+ * coupling between horizontal and vertical motion: the horizontal equation advects the horizontal velocity, the
+ * vertical one advects w as a scalar.  States made on this grid are stepped with those equations; everything else
+ * (acoustic substeps, NEXT-1, forcings, diagnostics) is the same code reading the changed per-layer tables.
+ * z_interfaces as in thor_grid_create_vertical (NULL = uniform layers); the vertical interpolation is linear. */
+int thor_grid_create_shallow(int level, int n_layers, const thor_planet *planet, const double *z_interfaces,
+                             thor_grid **out);
 /* NEXT-3 (section 2.3, Eq. 10-12): the same grid with the spring-dynamics relaxation -- by far the slowest
  * part of set-up from level 6 on -- iterated on the current CUDA device (one kernel launch per step, the same update
  * and the same stopping test as the host loop; positions agree with thor_grid_create's to rounding accumulated over the

@@ -26,9 +26,13 @@
  *                              stretched layers (k = 1, 3), uniform interfaces = the uniform path, dense solve of the
  *                              fast equations on stretched layers, order k changes the slow terms only (RV2)
  *   NEXT-4 (orc_set_energy_fixer): E restored to round-off where the plain run drifts, rho untouched, one uniform dT
+ *   NEXT-4 (orc_geom_set_shallow; tests/test_oracle_shallow.py): layer-independent operators, f r x V closed form,
+ *                              solid-body rotation (horizontal curvature term kept, radial one gone), scalar advection
+ *                              of w closed form, rest state, mass
  *   total energy (orc_diagnostics): P15, four closed forms (Cv, the 1/2, z_c, r_c, I_c)
  *   PARITY UNPINNED (readings the paper prints nothing for; constrained by the invariants above only): the window
- *   RV1 and the split RV2 of the order-k interpolation, the place and form RE1 of the energy fixer, and, as before,
+ *   RV1 and the split RV2 of the order-k interpolation, the place and form RE1 of the energy fixer, which terms the
+ *   shallow-atmosphere approximation drops (RS1), and, as before,
  *   the discrete advection form R7, the stage convention R1 (pinned in its ORDER by P14, not in value), the forcing
  *   convention R9, and the NEXT-1 readings RD2-RD4 (which state the fluxes use, where F_p enters, the
  *   form of the divergence-damping term; Eq. 43-46 are lost or damaged in PAPER.md) -- the paper fixes

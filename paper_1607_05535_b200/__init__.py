@@ -57,6 +57,7 @@ _SIGNATURES = {
     "thor_grid_create": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.POINTER(thor_planet), ctypes.POINTER(_V)]),
     "thor_grid_create_vertical": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.POINTER(thor_planet), _D, ctypes.c_int,
                                                  ctypes.POINTER(_V)]),
+    "thor_grid_create_shallow": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.POINTER(thor_planet), _D, ctypes.POINTER(_V)]),
     "thor_grid_create_device": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.POINTER(thor_planet), _D, ctypes.c_int,
                                                ctypes.POINTER(_V)]),
     "thor_grid_get": (ctypes.c_int, [_V, ctypes.POINTER(thor_grid_view)]),
@@ -134,6 +135,14 @@ def thor_grid_create_vertical(level, n_layers, planet, z_interfaces=None, order_
     h = _V()
     _check(load_library().thor_grid_create_vertical(int(level), int(n_layers), ctypes.byref(P), _ptr(z), int(order_k),
                                                     ctypes.byref(h)))
+    return h
+
+
+def thor_grid_create_shallow(level, n_layers, planet, z_interfaces=None):
+    P = thor_planet(**{k: float(planet[k]) for k in ("radius", "omega", "gravity", "Rd", "Cp", "p_ref", "z_top")})
+    z = None if z_interfaces is None else _f64(z_interfaces, (int(n_layers) + 1,))
+    h = _V()
+    _check(load_library().thor_grid_create_shallow(int(level), int(n_layers), ctypes.byref(P), _ptr(z), ctypes.byref(h)))
     return h
 
 
@@ -264,9 +273,13 @@ def thor_last_error():
 # conveniences (ownership + shapes); still no arithmetic
 # ---------------------------------------------------------------------------------------------
 class Grid:
-    def __init__(self, level, n_layers, planet, z_interfaces=None, order_k=1, on_device=False):
+    def __init__(self, level, n_layers, planet, z_interfaces=None, order_k=1, on_device=False, shallow=False):
         self.planet = dict(planet)
-        if on_device:
+        if shallow:
+            if order_k != 1 or on_device:
+                raise ThorError(THOR_EINVAL, "shallow-atmosphere grids: linear vertical interpolation, host generator")
+            self._h = thor_grid_create_shallow(level, n_layers, planet, z_interfaces)
+        elif on_device:
             self._h = thor_grid_create_device(level, n_layers, planet, z_interfaces, order_k)
         elif z_interfaces is None and order_k == 1:
             self._h = thor_grid_create(level, n_layers, planet)

@@ -211,7 +211,7 @@ double tri_area(V3 a, V3 b, V3 c) {   // spherical excess
 }  // namespace
 
 int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces, int kord,
-                    SpringFn spring) {
+                    SpringFn spring, bool shallow) {
     if (level < 0 || level > 9 || nv < 2 || nv > 128) return THOR_EINVAL;
     if (kord != 1 && kord != 3) return THOR_EINVAL;
     if (z_interfaces) {
@@ -497,8 +497,10 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
     g.rhinv.resize(nv); g.wl.assign(nv, 0.0); g.wh.assign(nv, 0.0); g.idz.assign(nv, 0.0);
     for (int k = 0; k < nv; ++k) {
         const double zl = g.zh[k], zu = g.zh[k + 1], dzk = z_interfaces ? zu - zl : g.dz;
-        const double zc = z_interfaces ? 0.5 * (zl + zu) : (k + 0.5) * g.dz, rc = P.radius + zc;
-        const double rl = P.radius + zl, ru = P.radius + zu;
+        const double zc = z_interfaces ? 0.5 * (zl + zu) : (k + 0.5) * g.dz;
+        // RS1 (i): in the shallow atmosphere every radius is the planetary radius; altitudes are unchanged
+        const double rc = P.radius + (shallow ? 0.0 : zc);
+        const double rl = P.radius + (shallow ? 0.0 : zl), ru = P.radius + (shallow ? 0.0 : zu);
         g.zc[k] = zc;
         g.rinv[k] = 1.0 / rc;
         g.dlo[k] = rl * rl / (rc * rc * dzk);
@@ -515,6 +517,7 @@ int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const 
     // Eq. 8-9 (L90-L94) at order 3: L_j(zt) = prod_(i != j) (zt - z_i)/(z_j - z_i) over the window of RV1 -- the two
     // nearest nodes on each side of the target, cut at the ends of the column
     g.kord = kord;
+    g.shallow = shallow;
     g.ihw.assign(size_t(4) * nv, 0.0);
     g.icw.assign(size_t(4) * nv, 0.0);
     auto lagrange = [](const double* z, int n, double zt, int j) {

@@ -52,6 +52,10 @@ struct HostGrid {
     // device slots are rotated to start at (1,0), so that the kernels can COMPUTE the neighbour columns from the
     // column's own Morton index instead of loading them (true when the generator has verified it for every such column)
     bool lattice_nbr = false;
+    // NEXT-4 (reading RS1): shallow-atmosphere approximation -- every radius in the vertical tables is the planetary
+    // radius (1/r_k = 1/A, no r^2 factors in D_c, volume A^2 dz); the slow-term kernels switch their Coriolis and
+    // advection terms on the same flag
+    bool shallow = false;
     int kord = 1;
     std::vector<double> ihw;       // [4][nv] centre k-2, k-1, k, k+1 -> lower interface of layer k (0 for k = 0)
     std::vector<double> icw;       // [4][nv] interface k-1, k, k+1, k+2 -> centre of layer k
@@ -70,6 +74,6 @@ using SpringFn = int (*)(int N, double* xyz, const int* nbr, const int* deg, con
 // kord: order of Eq. 8-9 in the explicit slow terms, 1 (the paper's choice, L94) or 3.  spring: nullptr = the host loop.
 // z_interfaces: nullptr (uniform layers, R6) or nv+1 strictly increasing altitudes from 0 to P.z_top.
 int build_host_grid(int level, int nv, const thor_planet& P, HostGrid& g, const double* z_interfaces = nullptr, int kord = 1,
-                    SpringFn spring = nullptr);
+                    SpringFn spring = nullptr, bool shallow = false);
 
 }  // namespace thor

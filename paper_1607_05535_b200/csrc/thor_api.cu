@@ -307,6 +307,7 @@ Geom make_geom(const thor_grid* grid) {
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
     g.wl = d.wl; g.wh = d.wh; g.idz = d.idz; g.vk = d.vk; g.kord = h.kord;
     g.lvl2 = h.lattice_nbr ? 2 * h.level : -1;
+    g.shallow = h.shallow ? 1 : 0;
     g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
@@ -574,13 +575,13 @@ const char* thor_last_error(void) { return g_err.c_str(); }
 long long thor_launch_count(void) { return g_launches.load(); }
 
 static int grid_create(int level, int n_layers, const thor_planet* planet, const double* z_interfaces, int order_k,
-                       SpringFn spring, thor_grid** out) {
+                       SpringFn spring, thor_grid** out, bool shallow = false) {
     if (!planet || !out) return fail(THOR_EINVAL, "thor_grid_create: null argument");
     thor_grid* g = new (std::nothrow) thor_grid();
     if (!g) return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
     int rc;
     try {
-        rc = build_host_grid(level, n_layers, *planet, g->h, z_interfaces, order_k, spring);
+        rc = build_host_grid(level, n_layers, *planet, g->h, z_interfaces, order_k, spring, shallow);
     } catch (const std::bad_alloc&) {
         delete g;
         return fail(THOR_ENOMEM, "thor_grid_create: out of host memory");
@@ -601,6 +602,10 @@ int thor_grid_create(int level, int n_layers, const thor_planet* planet, thor_gr
 int thor_grid_create_vertical(int level, int n_layers, const thor_planet* planet, const double* z_interfaces,
                               int order_k, thor_grid** out) {
     return grid_create(level, n_layers, planet, z_interfaces, order_k, nullptr, out);
+}
+
+int thor_grid_create_shallow(int level, int n_layers, const thor_planet* planet, const double* z_interfaces, thor_grid** out) {
+    return grid_create(level, n_layers, planet, z_interfaces, 1, nullptr, out, true);
 }
 
 int thor_grid_create_device(int level, int n_layers, const thor_planet* planet, const double* z_interfaces,
@@ -736,9 +741,12 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         const bool fuse1 = stage == 1 && !(Kd_div > 0.0);
         const double d1s = (fuse1 && !(Kd_hyp > 0.0)) ? delta : 0.0, d1d = (fuse1 && Kd_hyp > 0.0) ? delta : 0.0;
         if (Kd_hyp > 0.0) {
-            if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
+            if (g.shallow) THOR_DISPATCH(k_slow_terms_hyp_sh, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
+            else if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
             else THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
             THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks), d1d);
+        } else if (g.shallow) {
+            THOR_DISPATCH(k_slow_terms_sh, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);
         } else if (g.kord == 3) {
             THOR_DISPATCH(k_slow_terms_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);
         } else {

@@ -109,6 +109,7 @@ struct Geom {                 // device pointers, device column order, padded to
     // >= 0: twice the grid level; interior lattice points of a rhombus then have their neighbour columns COMPUTED
     // from their own Morton index (HostGrid::lattice_nbr); -1: always the nbr table
     int lvl2;
+    int shallow;              // NEXT-4 (RS1): shallow-atmosphere approximation (the slow-term kernels branch on it at launch)
     double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
@@ -784,7 +785,10 @@ k_stage_prepare(Geom g, double* __restrict__ S, int stage, double delta, Tune tn
 // delta1 > 0 (stage 1 of the base path): also the stage's explicit horizontal step, which with V*(0) = 0 and
 // p*(0) = 0 is V*' = delta1 slowV (Eq. 33) -- the slow term is in registers here, so no k_momentum launch.
 // ---------------------------------------------------------------------------------------------
-template <int G, int E, bool HYP, bool K3>
+// SH (NEXT-4, reading RS1): the shallow-atmosphere form -- the radii are already A in the per-layer tables; here the
+// horizontal equation advects the horizontal velocity only, w = I_c[W]/rho is advected as a scalar into the vertical
+// one, and Coriolis is f r x V with f = 2 Omega sin(lat) on the horizontal momentum alone.
+template <int G, int E, bool HYP, bool K3, bool SH = false>
 __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restrict__ S, const Tune& tn,
                                                  double* __restrict__ X, int dd, double delta1) {
     const Walk wk(tn);
@@ -841,8 +845,13 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
 
     double p0[E];
     double divV[E], divhV[E], divtV[E], Ax[E], Ay[E], Az[E], ga[E], gb[E];
+    double Aw[SH ? E : 1];                                 // RS1 (iii): scalar advection of w
 #pragma unroll
     for (int e = 0; e < E; ++e) divV[e] = divhV[e] = divtV[e] = Ax[e] = Ay[e] = Az[e] = ga[e] = gb[e] = 0.0;
+    if constexpr (SH) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) Aw[e] = 0.0;
+    }
     // NEXT-1: first Laplacians sum_j wlap_j (s_j - s_0) of rho, v_x, v_y, v_z, w, T
     double s0[HYP ? 6 : 1][E], lp[HYP ? 6 : 1][E];
     if (HYP) {
@@ -880,9 +889,16 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
             divV[e] += d;
             divhV[e] = fma(cph * pj[e] * irj[e], d, divhV[e]);                // h_j = Cp p_j/(Rd rho_j)
             divtV[e] = fma(tj[e], d, divtV[e]);
+            if constexpr (SH) {                                                   // u_h,j (w_j . V_j) and w_j (w_j . V_j)
+                Ax[e] = fma(fma(a[e], f[0], b[e] * f[3]), t, Ax[e]);
+                Ay[e] = fma(fma(a[e], f[1], b[e] * f[4]), t, Ay[e]);
+                Az[e] = fma(fma(a[e], f[2], b[e] * f[5]), t, Az[e]);
+                Aw[e] = fma(wc, t, Aw[e]);
+            } else {
             Ax[e] = fma(fma(a[e], f[0], fma(b[e], f[3], wc * f[6])), t, Ax[e]);   // u_j (w_j . V_j), u = (V + I_c[W] r)/rho
             Ay[e] = fma(fma(a[e], f[1], fma(b[e], f[4], wc * f[7])), t, Ay[e]);
             Az[e] = fma(fma(a[e], f[2], fma(b[e], f[5], wc * f[8])), t, Az[e]);
+            }
         }
         if (HYP) {
             double rj[E], wj[E], sj[6][E];
@@ -915,6 +931,7 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
         divV[e] *= ri[e]; divhV[e] *= ri[e]; divtV[e] *= ri[e];
         Ax[e] *= ri[e]; Ay[e] *= ri[e]; Az[e] *= ri[e];
         ga[e] *= ri[e]; gb[e] *= ri[e];
+        if constexpr (SH) Aw[e] *= ri[e];
     }
     // the column's own rows again (L1 hits), one at a time
     double rho[E], W[E], Wup[E], a0[E], b0[E], ir0[E];
@@ -932,9 +949,15 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     for (int e = 0; e < E; ++e) {
         double wc = 0.5 * (W[e] + Wup[e]);
         if constexpr (K3) wc = Wc3[e];
+        if constexpr (SH) {                                  // the horizontal momentum alone (RS1 ii, iii)
+            Mx[e] = fma(a0[e], e1x, b0[e] * e2x);
+            My[e] = fma(a0[e], e1y, b0[e] * e2y);
+            Mz[e] = fma(a0[e], e1z, b0[e] * e2z);
+        } else {
         Mx[e] = fma(a0[e], e1x, fma(b0[e], e2x, wc * rx));
         My[e] = fma(a0[e], e1y, fma(b0[e], e2y, wc * ry));
         Mz[e] = fma(a0[e], e1z, fma(b0[e], e2z, wc * rz));
+        }
     }
 
     // vertical flux divergences D_c[W I_h[q]] for q = u_x, u_y, u_z, h, theta, and D_c[W]
@@ -965,6 +988,14 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
     vflux(q0, t);
 #pragma unroll
     for (int e = 0; e < E; ++e) { Az[e] += t[e]; q0[e] = cph * p0[e] * ir0[e]; }
+    if constexpr (SH) {                                      // + D_c[W I_h[w]], w = I_c[W]/rho
+        double qw[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) qw[e] = (K3 ? Wc3[K3 ? e : 0] : 0.5 * (W[e] + Wup[e])) * ir0[e];
+        vflux(qw, t);
+#pragma unroll
+        for (int e = 0; e < E; ++e) Aw[e] += t[e];
+    }
     double DhW[E], DtW[E], DW[E];
     vflux(q0, DhW);
     ld_again<E>(me + F_TH * NVP, q0); vflux(q0, DtW);
@@ -986,13 +1017,17 @@ __device__ __forceinline__ void slow_terms_block(const Geom& g, double* __restri
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         const bool real = (L.k0 + e < nv) && (L.col < g.N);
-        const double Cx = -2.0 * g.omega * My[e], Cy = 2.0 * g.omega * Mx[e];       // 2 Omega z x M
+        double Cx = -2.0 * g.omega * My[e], Cy = 2.0 * g.omega * Mx[e], Cz = 0.0;   // 2 Omega z x M
+        if constexpr (SH) {                                                         // f r x V, f = 2 Omega sin(lat)
+            const double fc = 2.0 * g.omega * rz;
+            Cx = fc * (ry * Mz[e] - rz * My[e]); Cy = fc * (rz * Mx[e] - rx * Mz[e]); Cz = fc * (rx * My[e] - ry * Mx[e]);
+        }
         const double Ar = Ax[e] * rx + Ay[e] * ry + Az[e] * rz;
-        const double Cr = Cx * rx + Cy * ry;
-        Fr[e] = Ar + Cr;
+        const double Cr = SH ? Cx * rx + Cy * ry + Cz * rz : Cx * rx + Cy * ry;
+        if constexpr (SH) Fr[e] = Aw[e]; else Fr[e] = Ar + Cr;
         const double sx = -(Ax[e] - Ar * rx) - (Cx - Cr * rx);                      // Eq. 28 (G5)
         const double sy = -(Ay[e] - Ar * ry) - (Cy - Cr * ry);
-        const double sz = -(Az[e] - Ar * rz) - (0.0 - Cr * rz);
+        const double sz = -(Az[e] - Ar * rz) - (Cz - Cr * rz);
         sa[e] = real ? (sx * e1x + sy * e1y + sz * e1z) - ga[e] : 0.0;
         sb[e] = real ? (sx * e2x + sy * e2y + sz * e2z) - gb[e] : 0.0;
         srho[e] = real ? -divV[e] - DW[e] : 0.0;
@@ -1058,6 +1093,17 @@ template <int G, int E>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
 k_slow_terms_hyp(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
     slow_terms_block<G, E, true, false>(g, S, tn, X, dd, delta1);
+}
+// NEXT-4: the same two kernels in the shallow-atmosphere form (RS1; linear vertical interpolation only)
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
+k_slow_terms_sh(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, false, false, true>(g, S, tn, X, dd, delta1);
+}
+template <int G, int E>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3)
+k_slow_terms_hyp_sh(Geom g, double* __restrict__ S, Tune tn, double* __restrict__ X, int dd, double delta1) {
+    slow_terms_block<G, E, true, false, true>(g, S, tn, X, dd, delta1);
 }
 // NEXT-3: the same two kernels with Eq. 8-9 of order 3 in the vertical interpolations (RV2)
 template <int G, int E>

@@ -616,6 +616,46 @@ def test_next4_energy_fixer_parity(nv, forced):
     st.close()
 
 
+@pytest.mark.parametrize("nv,D,stretched", [(8, 0.0, False), (32, 0.0, False), (32, 0.004837, False), (37, 0.004837, True)])
+def test_next4_shallow_atmosphere_parity(nv, D, stretched):
+    """NEXT-4 (L178, reading RS1): a grid made with thor_grid_create_shallow steps the shallow-atmosphere equations;
+    element by element against the oracle's orc_geom_set_shallow path after 1 and 5 large steps, with and without
+    NEXT-1 and on stretched layers; and it is not the deep answer."""
+    level, planet = 3, dict(ti.EARTH, radius=6.371e5)         # a small planet: r/A up to 1.06, so deep and shallow differ
+    z_h = ti.stretched_interfaces(planet, nv, 4.0) if stretched else None
+    g = thor.Grid(level, nv, planet, z_interfaces=z_h, shallow=True)
+    v = g.view
+    G = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], z_interfaces=z_h, shallow=True)
+    Gf = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], fma=True, z_interfaces=z_h, shallow=True)
+    rng = np.random.default_rng(70 + nv)
+    N = g.n_cols
+    zi = np.asarray(z_h) if stretched else np.arange(nv + 1) * planet["z_top"] / nv
+    pcol = ti.hydrostatic_column(planet, zi, 1.0e5, np.full(nv, 290.0))
+    p = np.tile(pcol, (N, 1))
+    rho = p / (planet["Rd"] * 290.0 * (1 + rng.uniform(-1e-2, 1e-2, size=(N, nv))))
+    u = rng.uniform(-3.0, 3.0, size=(N, nv, 3))
+    u -= np.sum(u * v["xyz"][:, None, :], axis=-1, keepdims=True) * v["xyz"][:, None, :]
+    W = np.zeros((N, nv + 1))
+    W[:, 1:nv] = rho[:, 1:] * rng.uniform(-0.3, 0.3, size=(N, nv - 1))
+    s = (rho, rho[..., None] * u, W, p)
+    dt, n = 300.0, 4
+    st = thor.State(g, *s)
+    st.set_diffusion(D, D)
+    Y = Yardstick(G, Gf, s, _base_run(n, dt, None, (D, D)))
+    st.step(1, dt, n)
+    _compare(st.get(), Y.advance(1), TOL_1, "shallow nv=%d D=%g stretched=%s, 1 step" % (nv, D, stretched))
+    st.step(4, dt, n)
+    _compare(st.get(), Y.advance(4), TOL_1 * 5, "shallow nv=%d D=%g stretched=%s, 5 steps" % (nv, D, stretched))
+    m, e = st.diagnostics()
+    mr, er = G.diagnostics(*Y.ref)
+    assert abs(m - mr) <= 1e-13 * mr and abs(e - er) <= 1e-12 * er
+    Gd = oracle.Geometry(v["xyz"], v["nbr"], nv, planet, v["cv_vertex"], z_interfaces=z_h)
+    deep = Gd.step(*s, 5, dt, n, None, D, D)
+    assert np.abs(deep[1] - Y.ref[1]).max() > 1e3 * np.abs(st.get()[1] - Y.ref[1]).max()
+    st.close()
+    g.close()
+
+
 def test_graph_replay_is_bit_identical_to_direct_launches():
     """On a non-default stream thor_step replays a large step as a CUDA graph (after one directly
     launched step); the state must be bit-identical to direct launches on the default stream."""
