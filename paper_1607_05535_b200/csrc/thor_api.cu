@@ -307,7 +307,6 @@ Geom make_geom(const thor_grid* grid) {
     g.rinv = d.rinv; g.dlo = d.dlo; g.dhi = d.dhi; g.vol = d.vol; g.zc = d.zc; g.rhinv = d.rhinv;
     g.wl = d.wl; g.wh = d.wh; g.idz = d.idz; g.vk = d.vk; g.kord = h.kord;
     g.lvl2 = h.lattice_nbr ? 2 * h.level : -1;
-    g.shallow = h.shallow ? 1 : 0;
     g.omega = h.P.omega; g.gravity = h.P.gravity; g.Rd = h.P.Rd; g.Cp = h.P.Cp; g.p_ref = h.P.p_ref;
     // binomial series of Eq. 36 in deviation form: q_k = C(gamma, k+1)/gamma
     const double gam = h.P.Cp / (h.P.Cp - h.P.Rd);
@@ -741,11 +740,11 @@ static int launch_large_step(thor_state* s, const Geom& g, const TunePair& tn, c
         const bool fuse1 = stage == 1 && !(Kd_div > 0.0);
         const double d1s = (fuse1 && !(Kd_hyp > 0.0)) ? delta : 0.0, d1d = (fuse1 && Kd_hyp > 0.0) ? delta : 0.0;
         if (Kd_hyp > 0.0) {
-            if (g.shallow) THOR_DISPATCH(k_slow_terms_hyp_sh, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
+            if (hg.shallow) THOR_DISPATCH(k_slow_terms_hyp_sh, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
             else if (g.kord == 3) THOR_DISPATCH(k_slow_terms_hyp_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
             else THOR_DISPATCH(k_slow_terms_hyp, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, 0.0);
             THOR_DISPATCH(k_diff2, nv, Npad, st, g, S, s->X, Kd_hyp, dir(tn.ks), d1d);
-        } else if (g.shallow) {
+        } else if (hg.shallow) {            // NEXT-4 (RS1): the shallow-atmosphere form is chosen here, on the host
             THOR_DISPATCH(k_slow_terms_sh, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);
         } else if (g.kord == 3) {
             THOR_DISPATCH(k_slow_terms_k3, nv, Npad, st, g, S, dir(tn.ks), s->X, dd, d1s);

@@ -77,6 +77,9 @@ enum XField : int {
     XF
 };
 
+// NOTE: the struct is a kernel parameter, so its layout decides the constant-bank offsets the kernels read their scalars
+// from.  Shifting the fields after lvl2 by 8 bytes made k_slow_terms (at its 128-register cap) 5 us slower per launch
+// (profiles/r02c_variants.md): flags that only choose a kernel variant belong on the host (HostGrid), not in here.
 struct Geom {                 // device pointers, device column order, padded to Npad columns
     int N, Npad, nv;
     const int* nbr;           // [Npad][8]   6 neighbours (pentagons, pad columns: self), 2 x self
@@ -109,7 +112,6 @@ struct Geom {                 // device pointers, device column order, padded to
     // >= 0: twice the grid level; interior lattice points of a rhombus then have their neighbour columns COMPUTED
     // from their own Morton index (HostGrid::lattice_nbr); -1: always the nbr table
     int lvl2;
-    int shallow;              // NEXT-4 (RS1): shallow-atmosphere approximation (the slow-term kernels branch on it at launch)
     double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
