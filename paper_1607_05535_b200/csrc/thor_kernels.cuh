@@ -21,6 +21,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cstddef>
+
 namespace thor {
 
 constexpr unsigned kFull = 0xffffffffu;
@@ -115,6 +117,9 @@ struct Geom {                 // device pointers, device column order, padded to
     double omega, gravity, Rd, Cp, p_ref;
     double eosq[kEosTerms + 1];   // q_k = C(gamma, k+1)/gamma, k = 0..kEosTerms
 };
+// measured (profiles/r02c_variants.md): with the scalar block 8 bytes further on (or at the head of the struct) the
+// large step of config 3 is 1053 us instead of 1037 us; 16 or 32 bytes further on it is 1037 us again
+static_assert(offsetof(Geom, omega) % 16 == 8, "keep the scalar block of Geom where the kernels were tuned (see above)");
 
 struct Forcing {              // [Npad][NVP] each, may be null (Eq. 51-52)
     const double *T_eq, *k_T, *k_v;
