@@ -1239,7 +1239,7 @@ k_momentum(Geom g, double* __restrict__ S, double delta, Tune tn) {
 // the same kernel with NEXT-1's divergence damping added to Eq. 33; d3row: the X row that holds the 3-D
 // divergence of the current momentum (X_D3N in the first substep of a stage, where V^[t] + V*(0) = V^n; X_D3 after)
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 8)      // 64 registers, 8 blocks per SM: measured, profiles/r02c_variants.md
 k_momentum_dd(Geom g, double* __restrict__ S, double delta, Tune tn, const double* __restrict__ Xdd, double Kd_div, int d3row) {
     momentum_block<G, E, true>(g, S, delta, tn, Xdd, Kd_div, d3row);
 }
@@ -1722,7 +1722,7 @@ __device__ __forceinline__ void ld_lap_weights(const Geom& g, int col, int (&nb)
 
 // second Laplacian; the fluxes are added to the slow terms of the stage (RD2, RD3); delta1: as in k_slow_terms
 template <int G, int E>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 5)      // 5 blocks per SM: measured, profiles/r02c_variants.md
 k_diff2(Geom g, double* __restrict__ S, const double* __restrict__ X, double Kd, Tune tn, double delta1) {
     const Walk wk(tn);
     Map<G, E> L(wk.bid);
